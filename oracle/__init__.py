@@ -1,0 +1,177 @@
+"""float64 CPU oracle for the Soft-DTW value / gradient / barycenter path (TEST INFRASTRUCTURE).
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  The product
+(``paper_2404_12134_b200``) never imports it and it never imports the product.
+
+The arithmetic lives in ``sdtw_oracle.c`` (plain C, IEEE double, OpenMP over pairs only);
+this module only compiles it with gcc and marshals numpy arrays through ctypes.
+Citations (PAPER.md line numbers) are in the C file's header.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "sdtw_oracle.c"
+_LIB = _HERE / "libsdtw_oracle.so"
+_lib = None
+
+_c_double_p = ctypes.POINTER(ctypes.c_double)
+_c_float_p = ctypes.POINTER(ctypes.c_float)
+_c_i64_p = ctypes.POINTER(ctypes.c_int64)
+
+
+def build(force: bool = False) -> Path:
+    """Compile sdtw_oracle.c -> libsdtw_oracle.so (no-op when up to date)."""
+    if force or (not _LIB.exists()) or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".tmp{os.getpid()}.so")
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-fPIC", "-shared", "-fopenmp",
+               "-o", str(tmp), str(_SRC), "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(str(_LIB))
+        _lib.oracle_num_threads.restype = ctypes.c_int
+    return _lib
+
+
+def _d(a):
+    return a.ctypes.data_as(_c_double_p)
+
+
+def _chk(rc):
+    if rc != 0:
+        raise RuntimeError(f"oracle returned {rc}")
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def cost_matrix(x, z):
+    """Def. 3 with squared-Euclidean delta: (n, m) float64."""
+    x = _as2d(x)
+    z = _as2d(z)
+    n, d = x.shape
+    m = z.shape[0]
+    D = np.empty((n, m), np.float64)
+    _chk(_load().oracle_cost_matrix(_d(x), ctypes.c_int64(n), _d(z), ctypes.c_int64(m), ctypes.c_int(d), _d(D)))
+    return D
+
+
+def _as2d(a):
+    a = np.asarray(a, np.float64)
+    if a.ndim == 1:
+        a = a[:, None]
+    return np.ascontiguousarray(a)
+
+
+def forward_R(D, gamma):
+    """eq. 5 on a given cost matrix; returns the (n+2, m+2) bordered R (rows/cols 0..n / 0..m valid)."""
+    D = np.ascontiguousarray(D, np.float64)
+    n, m = D.shape
+    R = np.full((n + 2, m + 2), np.nan, np.float64)
+    _chk(_load().oracle_forward_R(_d(D), ctypes.c_int64(n), ctypes.c_int64(m), ctypes.c_double(gamma), _d(R)))
+    return R
+
+
+def pair(x, z, gamma, want_grad=True, want_E=False, want_R=False, mode="full"):
+    """One (x, z) pair.  Returns dict(value, grad (m,d) or None, E (n,m) or None, R or None)."""
+    x = _as2d(x)
+    z = _as2d(z)
+    n, d = x.shape
+    m = z.shape[0]
+    assert z.shape[1] == d
+    value = ctypes.c_double(0.0)
+    grad = np.zeros((m, d), np.float64) if want_grad else None
+    lib = _load()
+    if mode == "checkpointed":
+        assert not want_E and not want_R
+        _chk(lib.oracle_pair_checkpointed(_d(x), ctypes.c_int64(n), _d(z), ctypes.c_int64(m), ctypes.c_int(d),
+                                          ctypes.c_double(gamma), ctypes.byref(value),
+                                          _d(grad) if want_grad else None))
+        return dict(value=value.value, grad=grad, E=None, R=None)
+    E = np.empty((n, m), np.float64) if want_E else None
+    R = np.empty((n + 2, m + 2), np.float64) if want_R else None
+    _chk(lib.oracle_pair_full(_d(x), ctypes.c_int64(n), _d(z), ctypes.c_int64(m), ctypes.c_int(d),
+                              ctypes.c_double(gamma), ctypes.byref(value), _d(grad) if want_grad else None,
+                              _d(E) if want_E else None, _d(R) if want_R else None))
+    return dict(value=value.value, grad=grad, E=E, R=R)
+
+
+def backward_E_normalised(D, R, gamma):
+    """The probability-flow form of the reverse DP (self-check of the textbook form)."""
+    D = np.ascontiguousarray(D, np.float64)
+    R = np.ascontiguousarray(R, np.float64)
+    n, m = D.shape
+    assert R.shape == (n + 2, m + 2)
+    E = np.empty((n, m), np.float64)
+    _chk(_load().oracle_backward_E_normalised(_d(D), ctypes.c_int64(n), ctypes.c_int64(m), ctypes.c_double(gamma),
+                                              _d(R), _d(E)))
+    return E
+
+
+def dtw(x, z):
+    """eq. 1 (classic DTW, squared-Euclidean delta)."""
+    x = _as2d(x)
+    z = _as2d(z)
+    v = ctypes.c_double(0.0)
+    _chk(_load().oracle_dtw(_d(x), ctypes.c_int64(x.shape[0]), _d(z), ctypes.c_int64(z.shape[0]),
+                            ctypes.c_int(x.shape[1]), ctypes.byref(v)))
+    return v.value
+
+
+def _f32_inputs(Z, X_concat, offsets):
+    Z = np.ascontiguousarray(Z, np.float32)
+    if Z.ndim == 1:
+        Z = Z[:, None]
+    X = np.ascontiguousarray(X_concat, np.float32)
+    if X.ndim == 1:
+        X = X[:, None]
+    off = np.ascontiguousarray(offsets, np.int64)
+    assert X.shape[1] == Z.shape[1] and off[0] == 0 and off[-1] == X.shape[0]
+    return Z, X, off
+
+
+def value_grad(Z, X_concat, offsets, gamma, want_grad=True, mode="full", nthreads=0):
+    """Mirror of the C-ABI sdtw_value_grad: fp32 inputs promoted to float64.
+    Returns (values (N,) float64, grad (m, d) float64 or None)."""
+    Z, X, off = _f32_inputs(Z, X_concat, offsets)
+    m, d = Z.shape
+    N = len(off) - 1
+    values = np.zeros(N, np.float64)
+    grad = np.zeros((m, d), np.float64) if want_grad else None
+    _chk(_load().oracle_value_grad_f32(Z.ctypes.data_as(_c_float_p), ctypes.c_int64(m), ctypes.c_int(d),
+                                       X.ctypes.data_as(_c_float_p), off.ctypes.data_as(_c_i64_p), ctypes.c_int(N),
+                                       ctypes.c_double(gamma), _d(values), _d(grad) if want_grad else None,
+                                       ctypes.c_int(1 if mode == "checkpointed" else 0), ctypes.c_int(nthreads)))
+    return values, grad
+
+
+def barycenter(Z0, X_concat, offsets, gamma, iters, step, mode="full", nthreads=0):
+    """Mirror of sdtw_barycenter: fixed-step GD in float64.
+    Returns (Z (m,d) float64, values (N,) at the last evaluated iterate, objective (iters,))."""
+    Z0, X, off = _f32_inputs(Z0, X_concat, offsets)
+    m, d = Z0.shape
+    N = len(off) - 1
+    Z = np.zeros((m, d), np.float64)
+    values = np.zeros(N, np.float64)
+    obj = np.zeros(max(iters, 1), np.float64)
+    _chk(_load().oracle_barycenter_f32(Z0.ctypes.data_as(_c_float_p), ctypes.c_int64(m), ctypes.c_int(d),
+                                       X.ctypes.data_as(_c_float_p), off.ctypes.data_as(_c_i64_p), ctypes.c_int(N),
+                                       ctypes.c_double(gamma), ctypes.c_int(iters), ctypes.c_double(step), _d(Z),
+                                       _d(values), _d(obj), ctypes.c_int(1 if mode == "checkpointed" else 0),
+                                       ctypes.c_int(nthreads)))
+    return Z, values, obj[:iters]

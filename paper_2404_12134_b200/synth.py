@@ -1,0 +1,174 @@
+"""Seeded synthetic warped-cycle inputs (stand-in for the paper's robot joint cycles).
+
+This module holds NO Soft-DTW arithmetic: it only draws the inputs that both the CUDA path
+and the float64 oracle consume (identical fp32 bytes to both).  The paper's data (robot A/B
+joint angles at 125 Hz, cycles of ~16-24k samples with variable duration, pauses and gaps,
+PAPER.md:41-45, 254-270) is private; BASELINE.json's five configs describe these synthetic
+stand-ins, and DESIGN.md section 4 states the recipe and every choice the configs leave open.
+
+Recipe (float64 math, cast to fp32 last; numpy Generator(PCG64(seed)), seed = 20240412 + cfg):
+  template, per channel:  T(t) = sum_r a_r S((t - c_r)/w_r + 1/2),  S(u) = u^2 (3 - 2u) on
+      clamp(u, 0, 1),  c_r ~ U[0,1], a_r ~ U[-1,1], w_r ~ U[0.02, 0.10]
+  per cycle:  n ~ UniformInt[lo, hi];  warp = 8 equal segments of the sample axis with slopes
+      ~ U[s_lo, s_hi];  P ~ UniformInt[0, K] dwell plateaus, each of length floor(U[f_lo,f_hi] n)
+      at a uniform start, where the slope is set to 0;  tau = cumsum(slope) normalised to
+      tau[0] = 0, tau[n-1] = 1;  sample = T(tau) + N(0, sigma^2) (noise on every sample);
+      the channels of one cycle share tau.
+  Z0 = mean over k of x_k linearly resampled (index space) to m points.
+  cfg 5: prototype = noise-free template on a uniform grid of m points; exactly 5 % of the
+      cycles get one anomalous span (2-10 % of n): scaled/shifted (s ~ U[0.5,1.5],
+      o ~ U[-0.5,0.5]) or time-reversed, chosen by a fair coin.
+Draw order per config: template (channel-major: c, a, w), then per cycle: n, slopes, plateau
+count, (length, start) per plateau, noise; cfg 5 anomalies are drawn after all cycles.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, replace
+
+import numpy as np
+
+BASE_SEED = 20240412
+
+
+@dataclass(frozen=True)
+class Config:
+    name: str
+    index: int           # 1-based index in BASELINE.json "configs"
+    N: int
+    n_lo: int
+    n_hi: int
+    m: int
+    d: int
+    gamma: float
+    iters: int           # GD iterations (0 = forward-only scoring sweep)
+    step: float          # fixed GD step (reading C12)
+    ramps: int
+    slope_lo: float
+    slope_hi: float
+    max_plateaus: int
+    plat_lo: float
+    plat_hi: float
+    sigma: float
+    anomaly_frac: float = 0.0
+
+
+# step sizes: cfg 1 is stated by BASELINE.json; cfg 2-4 follow DESIGN.md reading C12.
+CONFIGS = {
+    1: Config("tiny", 1, 8, 48, 64, 56, 1, 1.0, 10, 0.01, 6, 0.7, 1.4, 0, 0.0, 0.0, 0.05),
+    2: Config("medium", 2, 64, 900, 1100, 1000, 1, 0.1, 20, 1.25e-3, 12, 0.7, 1.4, 2, 0.01, 0.05, 0.05),
+    3: Config("multichannel", 3, 32, 9000, 11000, 10000, 4, 0.1, 10, 2.5e-3, 24, 0.7, 1.4, 3, 0.01, 0.05, 0.03),
+    4: Config("full_length", 4, 100, 27000, 33000, 30000, 1, 0.01, 5, 2.0e-4, 64, 0.6, 1.6, 4, 0.01, 0.08, 0.02),
+    5: Config("scoring_sweep", 5, 1000, 20000, 40000, 30000, 1, 0.01, 0, 0.0, 64, 0.6, 1.6, 4, 0.01, 0.08, 0.02,
+              anomaly_frac=0.05),
+}
+
+
+def scaled(cfg: Config, length_scale: float = 1.0, N: int | None = None, name: str | None = None) -> Config:
+    """A shrunken copy of a config (same generator, shorter cycles / fewer pairs) for parity
+    tests the oracle can finish in seconds.  Lengths and m are multiplied by length_scale."""
+    f = float(length_scale)
+    return replace(cfg, name=name or f"{cfg.name}_x{f:g}" + (f"_N{N}" if N else ""),
+                   n_lo=max(1, int(round(cfg.n_lo * f))), n_hi=max(1, int(round(cfg.n_hi * f))),
+                   m=max(1, int(round(cfg.m * f))), N=N if N is not None else cfg.N)
+
+
+def _smoothstep(u):
+    u = np.clip(u, 0.0, 1.0)
+    return u * u * (3.0 - 2.0 * u)
+
+
+def _template_params(rng, d, ramps):
+    c = rng.uniform(0.0, 1.0, size=(d, ramps))
+    a = rng.uniform(-1.0, 1.0, size=(d, ramps))
+    w = rng.uniform(0.02, 0.10, size=(d, ramps))
+    return c, a, w
+
+
+def _template_eval(params, tau):
+    """T(tau) for every channel: (len(tau), d) float64."""
+    c, a, w = params
+    d = c.shape[0]
+    out = np.zeros((tau.shape[0], d), np.float64)
+    for ch in range(d):
+        for r in range(c.shape[1]):
+            out[:, ch] += a[ch, r] * _smoothstep((tau - c[ch, r]) / w[ch, r] + 0.5)
+    return out
+
+
+def _warp(rng, cfg, n):
+    slopes = rng.uniform(cfg.slope_lo, cfg.slope_hi, size=8)
+    seg = np.minimum((np.arange(n) * 8) // max(n, 1), 7)
+    slope = slopes[seg].astype(np.float64)
+    n_plat = int(rng.integers(0, cfg.max_plateaus + 1)) if cfg.max_plateaus > 0 else 0
+    for _ in range(n_plat):
+        length = int(np.floor(rng.uniform(cfg.plat_lo, cfg.plat_hi) * n))
+        start = int(rng.integers(0, max(n - length, 0) + 1))
+        slope[start:start + length] = 0.0
+    tau = np.cumsum(slope)
+    tau -= tau[0]
+    if n > 1 and tau[-1] > 0:
+        tau /= tau[-1]
+    return tau
+
+
+def resampled_mean(cycles, m):
+    """Euclidean mean of the cycles after linear (index-space) resampling to m points."""
+    d = cycles[0].shape[1]
+    acc = np.zeros((m, d), np.float64)
+    for x in cycles:
+        n = x.shape[0]
+        src = np.arange(n, dtype=np.float64)
+        dst = np.linspace(0.0, n - 1.0, m) if m > 1 else np.zeros(1)
+        for ch in range(d):
+            acc[:, ch] += np.interp(dst, src, x[:, ch].astype(np.float64))
+    return acc / len(cycles)
+
+
+def make(cfg: Config | int, seed: int | None = None):
+    """Draw one configuration.  Returns a dict:
+      Z0 (m, d) float32 -- initial barycenter (cfg 1-4) or the fixed prototype (cfg 5)
+      X  (sum n_k, d) float32, offsets (N+1,) int64, lengths (N,), cfg, anomalous (N,) bool
+    """
+    if isinstance(cfg, int):
+        cfg = CONFIGS[cfg]
+    rng = np.random.Generator(np.random.PCG64(BASE_SEED + cfg.index if seed is None else seed))
+    params = _template_params(rng, cfg.d, cfg.ramps)
+    cycles = []
+    for _ in range(cfg.N):
+        n = int(rng.integers(cfg.n_lo, cfg.n_hi + 1))
+        tau = _warp(rng, cfg, n)
+        x = _template_eval(params, tau)
+        x += rng.normal(0.0, cfg.sigma, size=x.shape)
+        cycles.append(x)
+    anomalous = np.zeros(cfg.N, bool)
+    if cfg.anomaly_frac > 0:
+        n_anom = int(round(cfg.anomaly_frac * cfg.N))
+        idx = rng.choice(cfg.N, size=n_anom, replace=False)
+        for k in idx:
+            x = cycles[k]
+            n = x.shape[0]
+            span = max(1, int(rng.uniform(0.02, 0.10) * n))
+            a = int(rng.integers(0, n - span + 1))
+            if rng.integers(0, 2) == 0:
+                s = rng.uniform(0.5, 1.5)
+                o = rng.uniform(-0.5, 0.5)
+                x[a:a + span] = s * x[a:a + span] + o
+            else:
+                x[a:a + span] = x[a:a + span][::-1].copy()
+            anomalous[k] = True
+    if cfg.iters == 0:
+        grid = np.linspace(0.0, 1.0, cfg.m) if cfg.m > 1 else np.zeros(1)
+        Z0 = _template_eval(params, grid)
+    else:
+        Z0 = resampled_mean(cycles, cfg.m)
+    lengths = np.array([c.shape[0] for c in cycles], np.int64)
+    offsets = np.zeros(cfg.N + 1, np.int64)
+    np.cumsum(lengths, out=offsets[1:])
+    X = np.concatenate(cycles, axis=0).astype(np.float32)
+    return dict(Z0=np.ascontiguousarray(Z0.astype(np.float32)), X=np.ascontiguousarray(X), offsets=offsets,
+                lengths=lengths, cfg=cfg, anomalous=anomalous)
+
+
+def cells(data) -> int:
+    """DP cells of one value(+grad) evaluation: sum_k n_k * m."""
+    return int(data["lengths"].sum()) * int(data["cfg"].m)

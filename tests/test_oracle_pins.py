@@ -1,0 +1,331 @@
+"""Pins for the float64 oracle (oracle/sdtw_oracle.c) against what the paper and the mathematics fix.
+
+None of these re-uses the oracle's own recurrences: the references are brute-force enumeration of all
+complete alignment paths (Def. 1-2, eq. 3-4), closed forms, exact integer
+Delannoy counts, the gamma -> 0 sandwich around classic DTW (eq. 1), invariants of the expected alignment
+E, central finite differences ("differentiable everywhere") and symmetries.
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from paper_2404_12134_b200 import synth
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+# ----------------------------------------------------------------------------- helpers (test-side, independent)
+def all_paths(n, m):
+    """Every complete alignment path from (0,0) to (n-1,m-1) with moves (0,1), (1,0), (1,1) (Def. 1)."""
+    out = []
+
+    def rec(i, j, acc):
+        acc = acc + [(i, j)]
+        if i == n - 1 and j == m - 1:
+            out.append(acc)
+            return
+        if j + 1 < m:
+            rec(i, j + 1, acc)
+        if i + 1 < n:
+            rec(i + 1, j, acc)
+        if i + 1 < n and j + 1 < m:
+            rec(i + 1, j + 1, acc)
+
+    rec(0, 0, [])
+    return out
+
+
+def sqdist(x, z):
+    x = np.asarray(x, np.float64).reshape(len(x), -1)
+    z = np.asarray(z, np.float64).reshape(len(z), -1)
+    return ((x[:, None, :] - z[None, :, :]) ** 2).sum(-1)
+
+
+def brute_force(x, z, gamma):
+    """value = -gamma log sum_A exp(-<A,D>/gamma) (eq. 3-4) and E = sum_A p(A) A, by enumeration."""
+    D = sqdist(x, z)
+    n, m = D.shape
+    paths = all_paths(n, m)
+    costs = np.array([sum(D[i, j] for i, j in p) for p in paths])
+    cmin = costs.min()
+    w = np.exp(-(costs - cmin) / gamma)
+    value = cmin - gamma * math.log(w.sum())
+    p = w / w.sum()
+    E = np.zeros((n, m))
+    for pk, path in zip(p, paths):
+        for i, j in path:
+            E[i, j] += pk
+    return value, E, costs, paths
+
+
+def delannoy(a, b):
+    return sum(math.comb(a, k) * math.comb(b, k) * 2 ** k for k in range(min(a, b) + 1))
+
+
+def dtw_minplus(D):
+    """Classic DTW by the textbook min-plus DP in numpy (test-side re-statement of eq. 1)."""
+    n, m = D.shape
+    R = np.full((n + 1, m + 1), np.inf)
+    R[0, 0] = 0.0
+    for i in range(1, n + 1):
+        for j in range(1, m + 1):
+            R[i, j] = D[i - 1, j - 1] + min(R[i - 1, j - 1], R[i - 1, j], R[i, j - 1])
+    return R[n, m]
+
+
+def grad_from_E(E, x, z):
+    x = np.asarray(x, np.float64).reshape(len(x), -1)
+    z = np.asarray(z, np.float64).reshape(len(z), -1)
+    return 2.0 * (E.sum(0)[:, None] * z - E.T @ x)
+
+
+# ----------------------------------------------------------------------------- golden: path counts
+def test_golden_delannoy_and_path_enumeration():
+    rows = [l.split() for l in open(os.path.join(HERE, "golden", "delannoy.txt")) if l.strip() and l[0] != "#"]
+    for a, b, v in rows:
+        a, b, v = int(a), int(b), int(v)
+        assert delannoy(a, b) == v
+        if v <= 2000:
+            assert len(all_paths(a + 1, b + 1)) == v
+
+
+# ----------------------------------------------------------------------------- brute force (value, E, gradient)
+@pytest.mark.parametrize("gamma", [1.0, 0.1, 0.01])
+@pytest.mark.parametrize("shape", [(1, 1, 1), (1, 5, 1), (4, 1, 2), (2, 2, 1), (3, 4, 1), (5, 6, 1), (6, 5, 2), (6, 6, 3)])
+def test_brute_force_value_E_grad(oracle, gamma, shape):
+    n, m, d = shape
+    rng = np.random.default_rng(1000 * n + 10 * m + d)
+    x = rng.normal(size=(n, d))
+    z = rng.normal(size=(m, d))
+    v_bf, E_bf, _, _ = brute_force(x, z, gamma)
+    r = oracle.pair(x, z, gamma, want_grad=True, want_E=True, want_R=True)
+    assert abs(r["value"] - v_bf) <= 1e-12 * max(1.0, abs(v_bf))
+    assert np.abs(r["E"] - E_bf).max() <= 1e-12
+    assert np.abs(r["grad"] - grad_from_E(E_bf, x, z)).max() <= 1e-11
+    # the probability-flow form of the reverse DP must give the same E
+    D = oracle.cost_matrix(x, z)
+    assert np.abs(D - sqdist(x, z)).max() <= 1e-14
+    En = oracle.backward_E_normalised(D, r["R"], gamma)
+    assert np.abs(En - E_bf).max() <= 1e-12
+    # checkpointed mode, same numbers bitwise
+    rc = oracle.pair(x, z, gamma, mode="checkpointed")
+    assert rc["value"] == r["value"] and np.array_equal(rc["grad"], r["grad"])
+
+
+def test_R_border_and_every_cell_against_brute_force(oracle):
+    """r_00 = 0, r_i0 = r_0j = inf (eq. 5) and every interior r_ij = soft-min over paths to (i,j)."""
+    rng = np.random.default_rng(7)
+    x, z, gamma = rng.normal(size=4), rng.normal(size=5), 0.3
+    R = oracle.pair(x, z, gamma, want_R=True)["R"]
+    assert R[0, 0] == 0.0 and np.all(np.isinf(R[0, 1:6])) and np.all(np.isinf(R[1:5, 0]))
+    for i in range(1, 5):
+        for j in range(1, 6):
+            v, _, _, _ = brute_force(x[:i], z[:j], gamma)
+            assert abs(R[i, j] - v) < 1e-12
+
+
+# ----------------------------------------------------------------------------- closed forms
+def test_single_cell_and_single_row_column(oracle):
+    rng = np.random.default_rng(3)
+    for d in (1, 3):
+        x = rng.normal(size=(1, d))
+        z = rng.normal(size=(1, d))
+        r = oracle.pair(x, z, 0.5, want_E=True)
+        assert abs(r["value"] - ((x - z) ** 2).sum()) < 1e-15
+        assert r["E"].tolist() == [[1.0]]
+        assert np.allclose(r["grad"], 2 * (z - x), atol=1e-15)
+        # n = 1: a single path through every column
+        z = rng.normal(size=(7, d))
+        r = oracle.pair(x, z, 0.5, want_E=True)
+        assert abs(r["value"] - sqdist(x, z).sum()) < 1e-13
+        assert np.abs(r["E"] - 1.0).max() < 1e-13 and r["E"].shape == (1, 7)
+        assert np.allclose(r["grad"], 2 * (z - x), atol=1e-14)
+        # m = 1
+        xx = rng.normal(size=(6, d))
+        zz = rng.normal(size=(1, d))
+        r = oracle.pair(xx, zz, 0.5, want_E=True)
+        assert abs(r["value"] - sqdist(xx, zz).sum()) < 1e-13
+        assert np.abs(r["E"] - 1.0).max() < 1e-13 and r["E"].shape == (6, 1)
+        assert np.allclose(r["grad"], 2 * (6 * zz - xx.sum(0, keepdims=True)), atol=1e-13)
+
+
+@pytest.mark.parametrize("n,m", [(1, 1), (3, 3), (6, 9), (40, 55)])
+def test_zero_cost_closed_form_delannoy(oracle, n, m):
+    """x == z == const => D == 0: value = -gamma ln Del(n-1,m-1), E_ij = Del(i-1,j-1) Del(n-i,m-j)/Del(n-1,m-1)."""
+    gamma = 0.7
+    x = np.full(n, 0.25)
+    z = np.full(m, 0.25)
+    r = oracle.pair(x, z, gamma, want_E=True)
+    tot = delannoy(n - 1, m - 1)
+    assert abs(r["value"] + gamma * math.log(tot)) <= 1e-9 * max(1.0, gamma * math.log(tot))
+    Eex = np.array([[float(Fraction(delannoy(i, j) * delannoy(n - 1 - i, m - 1 - j), tot)) for j in range(m)]
+                    for i in range(n)])
+    assert np.abs(r["E"] - Eex).max() <= 1e-9
+    assert np.abs(r["grad"]).max() == 0.0
+
+
+@pytest.mark.parametrize("n,m", [(4, 4), (7, 5), (12, 20)])
+def test_constant_cost_closed_form(oracle, n, m):
+    """x == a, z == b: every cell costs delta; paths with k diagonal moves have n+m-1-k cells and there are
+    (n+m-2-k)! / (k! (n-1-k)! (m-1-k)!) of them."""
+    a, b, gamma = 0.3, -0.4, 0.25
+    delta = (a - b) ** 2
+    terms = []
+    mean_len_num = 0.0
+    for k in range(min(n, m)):
+        cnt = math.factorial(n + m - 2 - k) // (math.factorial(k) * math.factorial(n - 1 - k) * math.factorial(m - 1 - k))
+        terms.append((cnt, n + m - 1 - k))
+    Zsum = sum(c * math.exp(-delta * L / gamma) for c, L in terms)
+    v_ex = -gamma * math.log(Zsum)
+    mean_len = sum(c * math.exp(-delta * L / gamma) * L for c, L in terms) / Zsum
+    r = oracle.pair(np.full(n, a), np.full(m, b), gamma, want_E=True)
+    assert abs(r["value"] - v_ex) <= 1e-9 * abs(v_ex)
+    assert abs(r["E"].sum() - mean_len) <= 1e-9 * mean_len
+    assert abs(r["grad"].sum() - 2 * (b - a) * mean_len) <= 1e-9 * abs(2 * (b - a) * mean_len)
+
+
+# ----------------------------------------------------------------------------- gamma -> 0 (eq. 3 first case, eq. 1)
+def test_gamma_to_zero_sandwich_and_monotone(oracle):
+    rng = np.random.default_rng(11)
+    for n, m, d in [(5, 6, 1), (30, 41, 1), (25, 20, 2)]:
+        x = rng.normal(size=(n, d))
+        z = rng.normal(size=(m, d))
+        D = sqdist(x, z)
+        dtw = dtw_minplus(D)
+        assert abs(oracle.dtw(x, z) - dtw) <= 1e-12 * max(1, dtw)
+        if n * m <= 36:
+            _, _, costs, _ = brute_force(x, z, 1.0)
+            assert abs(costs.min() - dtw) < 1e-12          # eq. 1 by enumeration
+        prev = None
+        for gamma in [1.0, 0.3, 0.1, 0.01, 1e-3, 1e-5]:
+            v = oracle.pair(x, z, gamma, want_grad=False)["value"]
+            lo = dtw - gamma * math.log(delannoy(n - 1, m - 1))
+            assert lo - 1e-9 <= v <= dtw + 1e-12
+            if prev is not None:
+                assert v >= prev - 1e-12                   # d value / d gamma = -entropy <= 0
+            prev = v
+        assert abs(prev - dtw) <= 1e-5 * math.log(delannoy(n - 1, m - 1)) + 1e-12
+
+
+# ----------------------------------------------------------------------------- invariants of E, free-energy identity
+@pytest.mark.parametrize("gamma", [1.0, 0.1, 0.01])
+def test_E_invariants_and_free_energy_identity(oracle, gamma):
+    rng = np.random.default_rng(5)
+    n, m = 60, 70
+    t = np.linspace(0, 1, n)
+    x = np.sin(6 * t) + 0.05 * rng.normal(size=n)
+    z = np.sin(6 * np.linspace(0, 1, m) ** 1.2)
+    r = oracle.pair(x, z, gamma, want_E=True, want_R=True)
+    E, R = r["E"], r["R"]
+    assert E.min() >= -1e-15 and E.max() <= 1 + 1e-12
+    assert abs(E[0, 0] - 1) < 1e-12 and abs(E[-1, -1] - 1) < 1e-12
+    assert E.sum(1).min() >= 1 - 1e-12 and E.sum(0).min() >= 1 - 1e-12
+    assert max(n, m) - 1e-9 <= E.sum() <= n + m - 1 + 1e-9
+    # value = sum_s E[s] (D[s] - gamma H_s), H_s = entropy of softmax(-R[pred(s)]/gamma)   (test-side formula)
+    D = sqdist(x, z)
+    tot = 0.0
+    for i in range(1, n + 1):
+        for j in range(1, m + 1):
+            pr = np.array([R[i - 1, j - 1], R[i - 1, j], R[i, j - 1]])
+            pr = pr[np.isfinite(pr)]
+            w = np.exp(-(pr - pr.min()) / gamma)
+            w /= w.sum()
+            H = -(w[w > 0] * np.log(w[w > 0])).sum()
+            tot += E[i - 1, j - 1] * (D[i - 1, j - 1] - gamma * H)
+    assert abs(tot - r["value"]) <= 1e-9 * max(1.0, abs(r["value"]))
+    # the two reverse-DP forms agree
+    En = oracle.backward_E_normalised(D, R, gamma)
+    assert np.abs(En - E).max() < 1e-10
+
+
+# ----------------------------------------------------------------------------- finite differences
+@pytest.mark.parametrize("gamma,d", [(1.0, 1), (0.1, 1), (0.1, 3), (0.01, 1)])
+def test_gradient_finite_differences(oracle, gamma, d):
+    rng = np.random.default_rng(21 + d)
+    N, m = 3, 17
+    lens = [15, 19, 12]
+    xs = [np.cumsum(rng.normal(size=(n, d)), 0) * 0.2 for n in lens]
+    X = np.concatenate(xs).astype(np.float32)
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    Z = (np.cumsum(rng.normal(size=(m, d)), 0) * 0.2).astype(np.float32)
+    vals, G = oracle.value_grad(Z, X, off, gamma)
+
+    def obj(Zd):
+        return sum(oracle.pair(xk.astype(np.float32).astype(np.float64), Zd, gamma, want_grad=False)["value"] for xk in xs)
+
+    Zd = Z.astype(np.float64)
+    assert abs(obj(Zd) - vals.sum()) < 1e-10 * max(1, abs(vals.sum()))
+    for j in range(m):
+        for c in range(d):
+            h = 1e-5 * max(1.0, abs(Zd[j, c]))
+            Zp, Zm = Zd.copy(), Zd.copy()
+            Zp[j, c] += h
+            Zm[j, c] -= h
+            fd = (obj(Zp) - obj(Zm)) / (2 * h)
+            assert abs(fd - G[j, c]) <= 1e-6 * max(1.0, abs(G[j, c])), (j, c, fd, G[j, c])
+
+
+# ----------------------------------------------------------------------------- symmetries, scaling, additivity
+def test_symmetries_scaling_additivity(oracle):
+    rng = np.random.default_rng(9)
+    n, m, d, gamma = 14, 11, 2, 0.2
+    x = rng.normal(size=(n, d))
+    z = rng.normal(size=(m, d))
+    a = oracle.pair(x, z, gamma, want_E=True)
+    b = oracle.pair(z, x, gamma, want_E=True)
+    assert abs(a["value"] - b["value"]) < 1e-12 and np.abs(a["E"] - b["E"].T).max() < 1e-12
+    c = oracle.pair(x[::-1], z[::-1], gamma, want_E=True)
+    assert abs(a["value"] - c["value"]) < 1e-12 and np.abs(a["E"] - c["E"][::-1, ::-1]).max() < 1e-12
+    s = oracle.pair(x + 3.0, z + 3.0, gamma, want_E=True)
+    assert abs(a["value"] - s["value"]) < 1e-11
+    sc = 1.7
+    e = oracle.pair(sc * x, sc * z, gamma * sc * sc, want_E=True)
+    assert abs(e["value"] - sc * sc * a["value"]) < 1e-11 and np.abs(e["E"] - a["E"]).max() < 1e-11
+    # additivity over pairs: summed call == sum of single-pair calls
+    lens = [9, 14, 6, 11]
+    X = rng.normal(size=(sum(lens), d)).astype(np.float32)
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    Z = z.astype(np.float32)
+    vals, G = oracle.value_grad(Z, X, off, gamma)
+    Gs = np.zeros_like(G)
+    for k in range(4):
+        r = oracle.pair(X[off[k]:off[k + 1]].astype(np.float64), Z.astype(np.float64), gamma)
+        assert abs(vals[k] - r["value"]) < 1e-13 * max(1, abs(r["value"]))
+        Gs += r["grad"]
+    assert np.abs(G - Gs).max() < 1e-12
+    # thread count must not change anything (fixed k order of the final sum)
+    vals1, G1 = oracle.value_grad(Z, X, off, gamma, nthreads=1)
+    assert np.array_equal(vals, vals1) and np.array_equal(G, G1)
+
+
+# ----------------------------------------------------------------------------- checkpointed mode == full mode, cfg 2
+def test_checkpointed_mode_bitwise_on_medium_config(oracle):
+    data = synth.make(2)
+    off = data["offsets"][:5]            # 4 pairs of ~1000 x 1000 are enough to cover block edges
+    X = data["X"][:off[-1]]
+    v0, g0 = oracle.value_grad(data["Z0"], X, off, data["cfg"].gamma, mode="full")
+    v1, g1 = oracle.value_grad(data["Z0"], X, off, data["cfg"].gamma, mode="checkpointed")
+    assert np.array_equal(v0, v1) and np.array_equal(g0, g1)
+    assert np.all(np.isfinite(g0)) and np.abs(g0).max() > 0
+
+
+# ----------------------------------------------------------------------------- barycenter loop
+def test_barycenter_tiny_config_descends_and_matches_manual_loop(oracle):
+    data = synth.make(1)
+    cfg = data["cfg"]
+    Z, vals, obj = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, cfg.iters, cfg.step)
+    assert len(obj) == cfg.iters and np.all(np.diff(obj) < 0)          # monotone descent at step 0.01 (cfg 1)
+    # first objective / first update reproduce a value_grad call at Z0
+    v0, g0 = oracle.value_grad(data["Z0"], data["X"], data["offsets"], cfg.gamma)
+    assert abs(obj[0] - v0.sum()) < 1e-12 * abs(v0.sum())
+    Z1, _, _ = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, 1, cfg.step)
+    assert np.abs(Z1 - (data["Z0"].astype(np.float64) - cfg.step * g0)).max() < 1e-15
+    # iters = 0 leaves Z0 untouched
+    Zn, _, _ = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, 0, cfg.step)
+    assert np.array_equal(Zn, data["Z0"].astype(np.float64))
+    # the GD fixed point lowers the objective relative to the Euclidean-mean start
+    vend, _ = oracle.value_grad(Z.astype(np.float32), data["X"], data["offsets"], cfg.gamma, want_grad=False)
+    assert vend.sum() < obj[0]
