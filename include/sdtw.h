@@ -1,0 +1,122 @@
+/*
+ * sdtw.h -- C ABI of libsdtw: Soft-DTW value, gradient and fixed-step barycenter descent on one B200 (sm_100a).
+ *
+ * The operation (arXiv 2404.12134, "Warped Time Series Anomaly Detection", section 3.3; line numbers are those of
+ * /root/reference/PAPER.md):
+ *
+ *   pair k:  x_k in R^{n_k x d} (a cycle),  Z in R^{m x d} (the barycenter / prototype)
+ *   Def. 3 (l.119-121)   D_k[i][j] = delta(x_k[i], Z[j]) = sum_c (x_k[i][c] - Z[j][c])^2   (squared Euclidean)
+ *   eq. 3  (l.149-152)   min^gamma(a) = -gamma log sum_p exp(-a_p / gamma)
+ *   eq. 5  (l.162-167)   r_00 = 0, r_i0 = r_0j = inf, r_ij = D_ij + min^gamma(r_{i-1,j-1}, r_{i-1,j}, r_{i,j-1});
+ *                        value_k = Soft-DTW^gamma(x_k, Z) = r_{n_k, m}
+ *   eq. 6  (l.175-183)   grad_Z value_k = (dD_k/dZ)^T E_k,  E_k = d value_k / d D_k (the expected alignment matrix,
+ *                        obtained by the reverse recurrence of the paper's ref. [19]); with squared-Euclidean delta
+ *                        g_k[j][c] = sum_i E_k[i][j] * 2 * (Z[j][c] - x_k[i][c])
+ *   eq. 7  (l.187-192)   barycenter objective sum_k value_k(Z) (plain sum: lambda_k = 1, no 1/n_k; C6),
+ *                        minimised by fixed-step gradient descent (l.185):  Z <- Z - step * sum_k g_k.
+ *
+ * Conventions for every entry point
+ *   - "dev" pointers are CUDA device pointers owned by the caller (e.g. torch tensors); "host" pointers are ordinary
+ *     host memory.  The library never frees or keeps a caller pointer after the enqueued work has run.
+ *   - Layout is time-major, channel-minor: Z is [m][d], X_concat is [sum_k n_k][d], both contiguous float32.
+ *     offsets is a HOST array of N+1 int64 row indices into X_concat: offsets[0] = 0, strictly increasing,
+ *     cycle k = rows offsets[k] .. offsets[k+1]-1.  It is read during the call only.
+ *   - stream is a cudaStream_t (NULL = the legacy default stream).  Device entry points only ENQUEUE work on it: no
+ *     host synchronisation and no device-to-host copy (exception: the first call with a new (offsets, m, d) shape
+ *     uploads a few KB of plan metadata with one pageable cudaMemcpyAsync).  The caller keeps all buffers alive until
+ *     the stream has drained.  Results are bitwise reproducible run to run for fixed inputs (no atomics on data).
+ *   - Return value: SDTW_OK (0) or a negative SDTW_ERR_* code.  No exception crosses the ABI.  On an argument error
+ *     nothing is enqueued and outputs are untouched.  NaN/Inf in the DATA is not scanned for (it propagates).
+ *   - d is supported for 1 <= d <= SDTW_MAX_D (compiled maximum); 1 <= n_k, m < 2^30; 1 <= N < 2^24.
+ *   - There is no CPU fallback: on a device that is not compute capability 10.x the calls return SDTW_ERR_UNSUPPORTED.
+ */
+#ifndef SDTW_H_
+#define SDTW_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SDTW_OK 0
+#define SDTW_ERR_INVALID_ARG (-1) /* NULL required pointer, m/d/N < 1, gamma <= 0 or non-finite, empty cycle, ... */
+#define SDTW_ERR_UNSUPPORTED (-2) /* d > SDTW_MAX_D, sizes beyond the stated limits, device is not sm_100        */
+#define SDTW_ERR_WORKSPACE (-3)   /* registered workspace smaller than sdtw_workspace_bytes()                    */
+#define SDTW_ERR_CUDA (-4)        /* a CUDA runtime call failed; see sdtw_last_cuda_error()                      */
+
+#define SDTW_MAX_D 4
+
+/*
+ * sdtw_value_grad -- eq. 5 and eq. 6 for N pairs (x_k, Z), summed over k.
+ *   Z          dev  [m][d]            barycenter (read only)
+ *   X_concat   dev  [offsets[N]][d]   the N cycles back to back (read only)
+ *   offsets    HOST [N+1] int64
+ *   gamma      > 0, finite (gamma = 0, the hard-DTW case of eq. 3, is rejected)
+ *   out_values dev  [N] float32, value_k in the caller's pair order; may be NULL
+ *   out_grad   dev  [m][d] float32, sum_k g_k (plain sum, not averaged); NULL => forward only (no checkpoints are
+ *              written and no reverse pass runs -- the scoring-sweep configuration)
+ */
+int sdtw_value_grad(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                    float gamma, float* out_values, float* out_grad, void* stream);
+
+/*
+ * sdtw_barycenter -- `iters` iterations of  Z <- Z - step * sum_k g_k(Z)  (l.185, eq. 7), all on `stream`.
+ *   Z_inout       dev [m][d]   Z0 on entry, the last iterate on return (the only buffer written in place)
+ *   iters         >= 0 (0 = no-op);  step finite
+ *   out_values    dev [N], value_k at the LAST EVALUATED iterate Z^(iters-1); may be NULL
+ *   out_objective dev [iters], sum_k value_k(Z^(t)) before the t-th update; may be NULL
+ */
+int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                    float gamma, int32_t iters, float step, float* out_values, float* out_objective, void* stream);
+
+/*
+ * sdtw_gd_update -- the descent step alone: Z[t] <- Z[t] - step * G[t] for t < count (= m*d).  Used when the
+ * gradient is all-reduced across GPUs between sdtw_value_grad and the update.
+ */
+int sdtw_gd_update(float* Z_inout, const float* G, int64_t count, float step, void* stream);
+
+/*
+ * Host-buffer variants (all pointers HOST; pinned memory makes the copies asynchronous).  They copy the inputs to
+ * the device, run the device entry point, copy the results back and synchronise `stream` before returning.
+ * Used by bench.py's end-to-end leg.  Outputs may be NULL as above.
+ */
+int sdtw_value_grad_host(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                         float gamma, float* out_values, float* out_grad, void* stream);
+int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                         float gamma, int32_t iters, float step, float* out_values, float* out_objective, void* stream);
+
+/*
+ * Workspace.  sdtw_workspace_bytes() is what one call needs (tile-boundary strips, checkpoints of the forward state,
+ * per-pair gradient partials).  If a workspace has been registered with sdtw_set_workspace() it is used (it must be
+ * large enough, else SDTW_ERR_WORKSPACE, and must not be shared by calls running concurrently on different streams);
+ * otherwise the library allocates with cudaMallocAsync / cudaFreeAsync on `stream`.  sdtw_set_workspace(NULL, 0)
+ * unregisters.  The pointer must be 256-byte aligned.  Returns 0 bytes on invalid arguments.
+ */
+size_t sdtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad);
+int sdtw_set_workspace(void* dev_ptr, size_t bytes);
+
+/* Static description of a status code; the cudaError_t behind the last SDTW_ERR_CUDA on this thread. */
+const char* sdtw_status_string(int status);
+int sdtw_last_cuda_error(void);
+
+/*
+ * Instrumentation used by bench.py (not part of the numerical path).
+ *   sdtw_launch_count()   kernels launched by this library since load.
+ *   sdtw_profile_enable() when on, every sdtw_value_grad / barycenter iteration brackets its forward kernel, its
+ *                         reverse kernel and the remaining small kernels with CUDA events on the caller's stream.
+ *   sdtw_profile_read()   waits for those events and returns the accumulated milliseconds and the number of
+ *                         evaluations they cover; clears the accumulators.  Any pointer may be NULL.
+ */
+uint64_t sdtw_launch_count(void);
+int sdtw_profile_enable(int on);
+int sdtw_profile_read(double* ms_forward, double* ms_backward, double* ms_other, int64_t* evaluations);
+
+/* Compile-time tile constants, for DESIGN.md / bench.py reporting: columns per thread, steps between checkpoints. */
+int sdtw_tile_info(int32_t* cols_per_thread, int32_t* strip_cols, int32_t* ckpt_steps, int32_t* chunk_steps);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SDTW_H_ */

@@ -1,0 +1,210 @@
+"""Thin ctypes binding of libsdtw.so (include/sdtw.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/; this module converts torch tensors /
+numpy arrays to raw pointers and raises on a non-zero status.  There is no CPU fallback: if
+libsdtw.so has not been built, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+_LIBPATH = Path(__file__).resolve().parent / "libsdtw.so"
+if not _LIBPATH.exists():
+    raise ImportError(f"{_LIBPATH} is missing: build it with `python -m paper_2404_12134_b200.build` "
+                      "(there is no CPU fallback)")
+_lib = ctypes.CDLL(str(_LIBPATH))
+
+_vp, _i64, _i32, _f32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float
+_i64p = ctypes.POINTER(ctypes.c_int64)
+
+SYMBOLS = {
+    "sdtw_value_grad": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _vp, _vp]),
+    "sdtw_barycenter": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _i32, _f32, _vp, _vp, _vp]),
+    "sdtw_gd_update": (ctypes.c_int, [_vp, _vp, _i64, _f32, _vp]),
+    "sdtw_value_grad_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _vp, _vp]),
+    "sdtw_barycenter_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _i32, _f32, _vp, _vp, _vp]),
+    "sdtw_workspace_bytes": (ctypes.c_size_t, [_i64, _i32, _i64p, _i32, ctypes.c_int]),
+    "sdtw_set_workspace": (ctypes.c_int, [_vp, ctypes.c_size_t]),
+    "sdtw_status_string": (ctypes.c_char_p, [ctypes.c_int]),
+    "sdtw_last_cuda_error": (ctypes.c_int, []),
+    "sdtw_launch_count": (ctypes.c_uint64, []),
+    "sdtw_profile_enable": (ctypes.c_int, [ctypes.c_int]),
+    "sdtw_profile_read": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double)] * 3 + [_i64p]),
+    "sdtw_tile_info": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int32)] * 4),
+}
+for _name, (_res, _args) in SYMBOLS.items():
+    _fn = getattr(_lib, _name)          # AttributeError here = the library does not export what sdtw.h declares
+    _fn.restype, _fn.argtypes = _res, _args
+
+SDTW_OK, SDTW_ERR_INVALID_ARG, SDTW_ERR_UNSUPPORTED, SDTW_ERR_WORKSPACE, SDTW_ERR_CUDA = 0, -1, -2, -3, -4
+
+
+class SdtwError(RuntimeError):
+    def __init__(self, status):
+        self.status = status
+        msg = _lib.sdtw_status_string(status).decode()
+        if status == SDTW_ERR_CUDA:
+            msg += f" [cudaError {_lib.sdtw_last_cuda_error()}]"
+        super().__init__(f"libsdtw status {status}: {msg}")
+
+
+def _check(status):
+    if status != SDTW_OK:
+        raise SdtwError(status)
+
+
+def status_string(status: int) -> str:
+    return _lib.sdtw_status_string(status).decode()
+
+
+def _offsets(offsets):
+    off = np.ascontiguousarray(np.asarray(offsets, dtype=np.int64))
+    return off, off.ctypes.data_as(_i64p), len(off) - 1
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return ctypes.c_void_p(stream if isinstance(stream, int) else stream.cuda_stream)
+
+
+def _dims(Z):
+    if Z.dim() == 1:
+        return Z.shape[0], 1
+    return Z.shape[0], Z.shape[1]
+
+
+def _dev_f32(t, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous float32 CUDA tensor")
+    return t
+
+
+def sdtw_value_grad(Z, X_concat, offsets, gamma, out_values=None, out_grad=None, want_grad=True, stream=None):
+    """values[k] = Soft-DTW^gamma(x_k, Z); grad = sum_k d value_k / d Z (include/sdtw.h).  Device tensors in,
+    device tensors out (allocated here unless given).  want_grad=False runs the forward-only scoring sweep."""
+    import torch
+    Z = _dev_f32(Z, "Z")
+    X = _dev_f32(X_concat, "X_concat")
+    m, d = _dims(Z)
+    off, offp, N = _offsets(offsets)
+    if out_values is None:
+        out_values = torch.empty(N, dtype=torch.float32, device=Z.device)
+    if want_grad and out_grad is None:
+        out_grad = torch.empty_like(Z)
+    with torch.cuda.device(Z.device):
+        _check(_lib.sdtw_value_grad(_ptr(Z), m, d, _ptr(X), offp, N, float(gamma), _ptr(out_values),
+                                    _ptr(out_grad) if want_grad else None, _stream(stream)))
+    return out_values, (out_grad if want_grad else None)
+
+
+def sdtw_barycenter(Z_inout, X_concat, offsets, gamma, iters, step, out_values=None, out_objective=None, stream=None):
+    """iters fixed-step gradient-descent iterations, in place on Z_inout.  Returns (Z_inout, values, objective)."""
+    import torch
+    Z = _dev_f32(Z_inout, "Z_inout")
+    X = _dev_f32(X_concat, "X_concat")
+    m, d = _dims(Z)
+    off, offp, N = _offsets(offsets)
+    if out_values is None:
+        out_values = torch.zeros(N, dtype=torch.float32, device=Z.device)
+    if out_objective is None:
+        out_objective = torch.zeros(max(int(iters), 0), dtype=torch.float32, device=Z.device)
+    with torch.cuda.device(Z.device):
+        _check(_lib.sdtw_barycenter(_ptr(Z), m, d, _ptr(X), offp, N, float(gamma), int(iters), float(step),
+                                    _ptr(out_values), _ptr(out_objective) if iters > 0 else None, _stream(stream)))
+    return Z, out_values, out_objective
+
+
+def sdtw_gd_update(Z_inout, G, step, stream=None):
+    import torch
+    Z = _dev_f32(Z_inout, "Z_inout")
+    G = _dev_f32(G, "G")
+    assert G.numel() == Z.numel()
+    with torch.cuda.device(Z.device):
+        _check(_lib.sdtw_gd_update(_ptr(Z), _ptr(G), Z.numel(), float(step), _stream(stream)))
+    return Z
+
+
+def _host_f32(a, name):
+    """numpy float32 C-contiguous array or CPU torch tensor (pinned or not) -> (keepalive, pointer)."""
+    if a is None:
+        return None, None
+    if isinstance(a, np.ndarray):
+        if a.dtype != np.float32 or not a.flags.c_contiguous:
+            raise TypeError(f"{name} must be C-contiguous float32")
+        return a, ctypes.c_void_p(a.ctypes.data)
+    import torch
+    if isinstance(a, torch.Tensor) and (not a.is_cuda) and a.dtype == torch.float32 and a.is_contiguous():
+        return a, ctypes.c_void_p(a.data_ptr())
+    raise TypeError(f"{name} must be a float32 numpy array or CPU tensor")
+
+
+def sdtw_value_grad_host(Z, X_concat, offsets, gamma, out_values, out_grad, stream=0):
+    """Host-buffer variant: H2D copies, the device path, D2H copies and a stream sync inside one C call."""
+    kz, pz = _host_f32(Z, "Z")
+    kx, px = _host_f32(X_concat, "X_concat")
+    kv, pv = _host_f32(out_values, "out_values")
+    kg, pg = _host_f32(out_grad, "out_grad")
+    m = Z.shape[0]
+    d = 1 if len(Z.shape) == 1 else Z.shape[1]
+    off, offp, N = _offsets(offsets)
+    _check(_lib.sdtw_value_grad_host(pz, m, d, px, offp, N, float(gamma), pv, pg,
+                                     ctypes.c_void_p(stream if isinstance(stream, int) else stream.cuda_stream)))
+    return out_values, out_grad
+
+
+def sdtw_barycenter_host(Z_inout, X_concat, offsets, gamma, iters, step, out_values=None, out_objective=None, stream=0):
+    kz, pz = _host_f32(Z_inout, "Z_inout")
+    kx, px = _host_f32(X_concat, "X_concat")
+    kv, pv = _host_f32(out_values, "out_values")
+    ko, po = _host_f32(out_objective, "out_objective")
+    m = Z_inout.shape[0]
+    d = 1 if len(Z_inout.shape) == 1 else Z_inout.shape[1]
+    off, offp, N = _offsets(offsets)
+    _check(_lib.sdtw_barycenter_host(pz, m, d, px, offp, N, float(gamma), int(iters), float(step), pv, po,
+                                     ctypes.c_void_p(stream if isinstance(stream, int) else stream.cuda_stream)))
+    return Z_inout, out_values, out_objective
+
+
+def sdtw_workspace_bytes(m, d, offsets, want_grad=True) -> int:
+    off, offp, N = _offsets(offsets)
+    return int(_lib.sdtw_workspace_bytes(int(m), int(d), offp, N, 1 if want_grad else 0))
+
+
+def sdtw_set_workspace(tensor_or_none):
+    """Register a device byte buffer (torch uint8 CUDA tensor, kept alive by the caller) or None to unregister."""
+    if tensor_or_none is None:
+        _check(_lib.sdtw_set_workspace(None, 0))
+    else:
+        t = tensor_or_none
+        _check(_lib.sdtw_set_workspace(ctypes.c_void_p(t.data_ptr()), t.numel() * t.element_size()))
+
+
+def sdtw_launch_count() -> int:
+    return int(_lib.sdtw_launch_count())
+
+
+def sdtw_profile_enable(on: bool):
+    _check(_lib.sdtw_profile_enable(1 if on else 0))
+
+
+def sdtw_profile_read():
+    f, b, o = ctypes.c_double(0), ctypes.c_double(0), ctypes.c_double(0)
+    n = ctypes.c_int64(0)
+    _check(_lib.sdtw_profile_read(ctypes.byref(f), ctypes.byref(b), ctypes.byref(o), ctypes.byref(n)))
+    return dict(ms_forward=f.value, ms_backward=b.value, ms_other=o.value, evaluations=n.value)
+
+
+def sdtw_tile_info():
+    v = [ctypes.c_int32(0) for _ in range(4)]
+    _check(_lib.sdtw_tile_info(*[ctypes.byref(x) for x in v]))
+    return dict(cols_per_thread=v[0].value, strip_cols=v[1].value, ckpt_steps=v[2].value, chunk_steps=v[3].value)

@@ -1,0 +1,504 @@
+// sdtw.cu -- host side of libsdtw: argument checks, schedule/workspace plan, kernel launches, the C ABI of
+// include/sdtw.h.  The arithmetic is in sdtw_kernels.cuh.  No CPU fallback exists: a device that is not sm_100 is
+// rejected with SDTW_ERR_UNSUPPORTED.
+#include "sdtw.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <mutex>
+#include <numeric>
+#include <vector>
+
+#include "sdtw_kernels.cuh"
+
+namespace {
+using namespace sdtw;
+
+thread_local int g_last_cuda_error = 0;
+std::mutex g_mutex;
+uint64_t g_launches = 0;
+void* g_user_ws = nullptr;
+size_t g_user_ws_bytes = 0;
+bool g_profile = false;
+
+struct ProfRec { cudaEvent_t e[4]; };
+std::vector<ProfRec> g_prof;
+
+#define CUDA_TRY(expr)                                   \
+    do {                                                 \
+        cudaError_t _e = (expr);                         \
+        if (_e != cudaSuccess) {                         \
+            g_last_cuda_error = (int)_e;                 \
+            return SDTW_ERR_CUDA;                        \
+        }                                                \
+    } while (0)
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---- workspace layout -------------------------------------------------------------------------------------------
+struct Layout {
+    int NS = 0;                 // strips per pair
+    long long items = 0;
+    size_t off_counters = 0, off_prog_f = 0, off_prog_b = 0, off_VP = 0, off_VS = 0, off_ES = 0, off_CK = 0, off_Gk = 0,
+           off_G = 0, off_vals = 0;
+    size_t sync_bytes = 0;      // counters + prog_f + prog_b: cleared before every evaluation
+    size_t total = 0;
+    std::vector<PairMeta> pm;   // schedule order
+};
+
+int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, Layout& L) {
+    if (!offsets || m < 1 || d < 1 || N < 1) return SDTW_ERR_INVALID_ARG;
+    if (offsets[0] != 0) return SDTW_ERR_INVALID_ARG;
+    for (int k = 0; k < N; ++k)
+        if (offsets[k + 1] <= offsets[k]) return SDTW_ERR_INVALID_ARG;
+    if (d > SDTW_MAX_D || m >= (1LL << 30) || N >= (1 << 24)) return SDTW_ERR_UNSUPPORTED;
+    for (int k = 0; k < N; ++k)
+        if (offsets[k + 1] - offsets[k] >= (1LL << 30)) return SDTW_ERR_UNSUPPORTED;
+    L.NS = (int)((m + SW - 1) / SW);
+    L.items = (long long)N * L.NS;
+    if (L.items >= (1LL << 31)) return SDTW_ERR_UNSUPPORTED;
+    // schedule order: longest cycle first (stable), so the shortest sweeps fill the tail
+    std::vector<int> order(N);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+        return (offsets[a + 1] - offsets[a]) > (offsets[b + 1] - offsets[b]);
+    });
+    L.pm.resize(N);
+    long long vs_floats = 0, ck_floats = 0;
+    for (int ps = 0; ps < N; ++ps) {
+        const int k = order[ps];
+        PairMeta& pm = L.pm[ps];
+        pm.k = k;
+        pm.x_off = offsets[k];
+        pm.n = (int)(offsets[k + 1] - offsets[k]);
+        pm.C = (pm.n + 31 + CH - 1) / CH;
+        pm.vs_stride = pm.C * CH + 64;
+        pm.vs_off = vs_floats;
+        vs_floats += (long long)pm.vs_stride * L.NS;
+        pm.ck_stride = (long long)(pm.C * (CH / TR) + 1) * CK_FLOATS;
+        pm.ck_off = ck_floats;
+        if (want_grad) ck_floats += pm.ck_stride * L.NS;
+    }
+    size_t o = 0;
+    L.off_counters = o; o += 256;
+    L.off_prog_f = o;   o += align_up((size_t)L.items * 4, 256);
+    L.off_prog_b = o;   o += align_up((size_t)L.items * 4, 256);
+    L.sync_bytes = o;
+    L.off_VP = o;       o += align_up((size_t)L.items * 8, 256);
+    L.off_vals = o;     o += align_up((size_t)N * 4, 256);
+    L.off_VS = o;       o += align_up((size_t)vs_floats * 4, 256);
+    if (want_grad) {
+        L.off_ES = o;   o += align_up((size_t)vs_floats * 4, 256);
+        L.off_CK = o;   o += align_up((size_t)ck_floats * 4, 256);
+        L.off_Gk = o;   o += align_up((size_t)N * (size_t)m * (size_t)d * 4, 256);
+        L.off_G = o;    o += align_up((size_t)m * (size_t)d * 4, 256);
+    }
+    L.total = o;
+    return SDTW_OK;
+}
+
+// ---- device / plan cache ----------------------------------------------------------------------------------------
+struct DeviceInfo { int dev = -1, sms = 0, cc_major = 0; bool ok = false; };
+
+int get_device(DeviceInfo& di) {
+    static DeviceInfo cache[64];
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return SDTW_ERR_UNSUPPORTED;
+    if (!cache[dev].ok) {
+        cudaDeviceProp prop;
+        CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+        cache[dev].dev = dev;
+        cache[dev].sms = prop.multiProcessorCount;
+        cache[dev].cc_major = prop.major;
+        cache[dev].ok = true;
+    }
+    di = cache[dev];
+    if (di.cc_major != 10) return SDTW_ERR_UNSUPPORTED;
+    return SDTW_OK;
+}
+
+struct Plan {
+    int dev = -1;
+    int64_t m = 0;
+    int32_t d = 0, N = 0;
+    bool want_grad = false;
+    std::vector<int64_t> offsets;
+    Layout L;
+    PairMeta* d_pm = nullptr;
+    cudaEvent_t uploaded = nullptr;
+    uint64_t stamp = 0;
+};
+std::vector<Plan*> g_plans;
+uint64_t g_stamp = 0;
+
+int get_plan(int dev, int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, cudaStream_t stream,
+             Plan** out) {
+    for (Plan* pl : g_plans) {
+        if (pl->dev == dev && pl->m == m && pl->d == d && pl->N == N && pl->want_grad == want_grad &&
+            std::memcmp(pl->offsets.data(), offsets, sizeof(int64_t) * (size_t)(N + 1)) == 0) {
+            pl->stamp = ++g_stamp;
+            CUDA_TRY(cudaStreamWaitEvent(stream, pl->uploaded, 0));
+            *out = pl;
+            return SDTW_OK;
+        }
+    }
+    Plan* pl = new Plan();
+    int rc = build_layout(m, d, offsets, N, want_grad, pl->L);
+    if (rc != SDTW_OK) { delete pl; return rc; }
+    pl->dev = dev; pl->m = m; pl->d = d; pl->N = N; pl->want_grad = want_grad;
+    pl->offsets.assign(offsets, offsets + N + 1);
+    cudaError_t e = cudaMalloc(&pl->d_pm, sizeof(PairMeta) * (size_t)N);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_pm, pl->L.pm.data(), sizeof(PairMeta) * (size_t)N, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pl->uploaded, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventRecord(pl->uploaded, stream);
+    if (e != cudaSuccess) {
+        g_last_cuda_error = (int)e;
+        if (pl->d_pm) cudaFree(pl->d_pm);
+        delete pl;
+        return SDTW_ERR_CUDA;
+    }
+    pl->stamp = ++g_stamp;
+    if (g_plans.size() >= 8) {   // evict the least recently used plan
+        auto it = std::min_element(g_plans.begin(), g_plans.end(), [](Plan* a, Plan* b) { return a->stamp < b->stamp; });
+        cudaFree((*it)->d_pm);
+        cudaEventDestroy((*it)->uploaded);
+        delete *it;
+        g_plans.erase(it);
+    }
+    g_plans.push_back(pl);
+    *out = pl;
+    return SDTW_OK;
+}
+
+// ---- kernel launch helpers --------------------------------------------------------------------------------------
+template <typename K>
+int persistent_grid(K kernel, int smem_bytes, int sms, long long items, int* grid) {
+    CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    int occ = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, WARPS * 32, smem_bytes));
+    if (occ < 1) return SDTW_ERR_UNSUPPORTED;
+    long long want = (items + WARPS - 1) / WARPS;
+    long long cap = (long long)sms * occ;
+    *grid = (int)std::max(1LL, std::min(want, cap));
+    return SDTW_OK;
+}
+
+template <int D>
+int launch_forward(const Params& P, bool ckpt, int sms, cudaStream_t stream) {
+    const int smem = WARPS * fwd_smem_floats<D>() * 4;
+    int grid = 1, rc;
+    if (ckpt) {
+        rc = persistent_grid(forward_kernel<D, true>, smem, sms, P.num_items, &grid);
+        if (rc) return rc;
+        forward_kernel<D, true><<<grid, WARPS * 32, smem, stream>>>(P);
+    } else {
+        rc = persistent_grid(forward_kernel<D, false>, smem, sms, P.num_items, &grid);
+        if (rc) return rc;
+        forward_kernel<D, false><<<grid, WARPS * 32, smem, stream>>>(P);
+    }
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return SDTW_OK;
+}
+
+template <int D>
+int launch_backward(const Params& P, int sms, cudaStream_t stream) {
+    const int smem = WARPS * bwd_smem_floats<D>() * 4;
+    int grid = 1;
+    int rc = persistent_grid(backward_kernel<D>, smem, sms, P.num_items, &grid);
+    if (rc) return rc;
+    backward_kernel<D><<<grid, WARPS * 32, smem, stream>>>(P);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return SDTW_OK;
+}
+
+int dispatch_forward(int d, const Params& P, bool ckpt, int sms, cudaStream_t s) {
+    switch (d) {
+        case 1: return launch_forward<1>(P, ckpt, sms, s);
+        case 2: return launch_forward<2>(P, ckpt, sms, s);
+        case 3: return launch_forward<3>(P, ckpt, sms, s);
+        case 4: return launch_forward<4>(P, ckpt, sms, s);
+    }
+    return SDTW_ERR_UNSUPPORTED;
+}
+int dispatch_backward(int d, const Params& P, int sms, cudaStream_t s) {
+    switch (d) {
+        case 1: return launch_backward<1>(P, sms, s);
+        case 2: return launch_backward<2>(P, sms, s);
+        case 3: return launch_backward<3>(P, sms, s);
+        case 4: return launch_backward<4>(P, sms, s);
+    }
+    return SDTW_ERR_UNSUPPORTED;
+}
+
+bool finite_pos(float g) { return std::isfinite(g) && g > 0.f; }
+
+// one evaluation: values (+ gradient) at Z.  If Z_update != nullptr the descent step is fused into the reduction.
+int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, const float* X, float gamma,
+             float* out_values, float* out_objective, float* out_grad, float* Z_update, float step, cudaStream_t stream) {
+    const Layout& L = pl.L;
+    Params P{};
+    P.Z = Z; P.X = X; P.pm = pl.d_pm;
+    P.counters = reinterpret_cast<unsigned*>(ws + L.off_counters);
+    P.prog_f = reinterpret_cast<unsigned*>(ws + L.off_prog_f);
+    P.prog_b = reinterpret_cast<unsigned*>(ws + L.off_prog_b);
+    P.VP = reinterpret_cast<double*>(ws + L.off_VP);
+    P.VS = reinterpret_cast<float*>(ws + L.off_VS);
+    P.ES = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_ES) : nullptr;
+    P.CK = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_CK) : nullptr;
+    P.Gk = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_Gk) : nullptr;
+    P.m = (int)pl.m; P.N = pl.N; P.NS = L.NS;
+    P.num_items = (unsigned)L.items;
+    const double kappa = 1.0 / ((double)gamma * std::log(2.0));
+    P.sqrtk = (float)std::sqrt(kappa);
+    P.gscale = (float)(2.0 / (double)P.sqrtk);
+    // the kernels see gamma only through the rounded sqrtk; undo exactly that scale on the way out
+    const double inv_kappa = 1.0 / ((double)P.sqrtk * (double)P.sqrtk);
+
+    ProfRec pr{};
+    if (g_profile) for (auto& e : pr.e) CUDA_TRY(cudaEventCreate(&e));
+    CUDA_TRY(cudaMemsetAsync(ws + L.off_counters, 0, L.sync_bytes, stream));
+    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[0], stream));
+    int rc = dispatch_forward(pl.d, P, pl.want_grad, di.sms, stream);
+    if (rc) return rc;
+    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[1], stream));
+    if (pl.want_grad) {
+        rc = dispatch_backward(pl.d, P, di.sms, stream);
+        if (rc) return rc;
+    }
+    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[2], stream));
+    if (out_values || out_objective) {
+        finalize_values_kernel<<<1, 256, 0, stream>>>(P.VP, pl.d_pm, pl.N, L.NS, inv_kappa, out_values, out_objective);
+        ++g_launches;
+        CUDA_TRY(cudaGetLastError());
+    }
+    if (pl.want_grad) {
+        const long long md = (long long)pl.m * pl.d;
+        const int blocks = (int)((md + 255) / 256);
+        reduce_pairs_kernel<<<blocks, 256, 0, stream>>>(P.Gk, pl.N, md, out_grad, Z_update, step);
+        ++g_launches;
+        CUDA_TRY(cudaGetLastError());
+    }
+    if (g_profile) {
+        CUDA_TRY(cudaEventRecord(pr.e[3], stream));
+        g_prof.push_back(pr);
+    }
+    return SDTW_OK;
+}
+
+int check_common(const void* Z, int64_t m, int32_t d, const void* X, const int64_t* offsets, int32_t N, float gamma) {
+    if (!Z || !X || !offsets || m < 1 || d < 1 || N < 1 || !finite_pos(gamma)) return SDTW_ERR_INVALID_ARG;
+    if (offsets[0] != 0) return SDTW_ERR_INVALID_ARG;
+    for (int k = 0; k < N; ++k)
+        if (offsets[k + 1] <= offsets[k]) return SDTW_ERR_INVALID_ARG;
+    if (d > SDTW_MAX_D) return SDTW_ERR_UNSUPPORTED;
+    return SDTW_OK;
+}
+
+struct Workspace {
+    char* ptr = nullptr;
+    bool owned = false;
+    cudaStream_t stream = nullptr;
+    int acquire(size_t bytes, cudaStream_t s) {
+        stream = s;
+        if (g_user_ws) {
+            if (g_user_ws_bytes < bytes) return SDTW_ERR_WORKSPACE;
+            ptr = static_cast<char*>(g_user_ws);
+            return SDTW_OK;
+        }
+        void* q = nullptr;
+        CUDA_TRY(cudaMallocAsync(&q, bytes, s));
+        ptr = static_cast<char*>(q);
+        owned = true;
+        return SDTW_OK;
+    }
+    ~Workspace() { if (owned && ptr) cudaFreeAsync(ptr, stream); }
+};
+
+}  // namespace
+
+// =================================================================================================================
+extern "C" {
+
+int sdtw_value_grad(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                    float gamma, float* out_values, float* out_grad, void* stream_) {
+    int rc = check_common(Z, m, d, X_concat, offsets, N, gamma);
+    if (rc) return rc;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    DeviceInfo di;
+    rc = get_device(di);
+    if (rc) return rc;
+    Plan* pl = nullptr;
+    rc = get_plan(di.dev, m, d, offsets, N, out_grad != nullptr, stream, &pl);
+    if (rc) return rc;
+    Workspace ws;
+    rc = ws.acquire(pl->L.total, stream);
+    if (rc) return rc;
+    return evaluate(*pl, ws.ptr, di, Z, X_concat, gamma, out_values, nullptr, out_grad, nullptr, 0.f, stream);
+}
+
+int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                    float gamma, int32_t iters, float step, float* out_values, float* out_objective, void* stream_) {
+    int rc = check_common(Z_inout, m, d, X_concat, offsets, N, gamma);
+    if (rc) return rc;
+    if (iters < 0 || !std::isfinite(step)) return SDTW_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    DeviceInfo di;
+    rc = get_device(di);
+    if (rc) return rc;
+    if (iters == 0) return SDTW_OK;
+    Plan* pl = nullptr;
+    rc = get_plan(di.dev, m, d, offsets, N, true, stream, &pl);
+    if (rc) return rc;
+    Workspace ws;
+    rc = ws.acquire(pl->L.total, stream);
+    if (rc) return rc;
+    for (int it = 0; it < iters; ++it) {
+        float* vals = (it == iters - 1) ? out_values : nullptr;
+        float* obj = out_objective ? out_objective + it : nullptr;
+        rc = evaluate(*pl, ws.ptr, di, Z_inout, X_concat, gamma, vals, obj, nullptr, Z_inout, step, stream);
+        if (rc) return rc;
+    }
+    return SDTW_OK;
+}
+
+int sdtw_gd_update(float* Z_inout, const float* G, int64_t count, float step, void* stream_) {
+    if (!Z_inout || !G || count < 1 || !std::isfinite(step)) return SDTW_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    DeviceInfo di;
+    int rc = get_device(di);
+    if (rc) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    gd_update_kernel<<<(int)((count + 255) / 256), 256, 0, stream>>>(Z_inout, G, count, step);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return SDTW_OK;
+}
+
+// ---- host-buffer variants ---------------------------------------------------------------------------------------
+namespace {
+struct DevBuf {
+    void* p = nullptr;
+    cudaStream_t s = nullptr;
+    int alloc(size_t bytes, cudaStream_t st) { s = st; CUDA_TRY(cudaMallocAsync(&p, bytes, st)); return SDTW_OK; }
+    ~DevBuf() { if (p) cudaFreeAsync(p, s); }
+};
+}  // namespace
+
+int sdtw_value_grad_host(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                         float gamma, float* out_values, float* out_grad, void* stream_) {
+    int rc = check_common(Z, m, d, X_concat, offsets, N, gamma);
+    if (rc) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const size_t zb = (size_t)m * d * 4, xb = (size_t)offsets[N] * d * 4;
+    DevBuf dZ, dX, dV, dG;
+    if ((rc = dZ.alloc(zb, stream)) || (rc = dX.alloc(xb, stream)) || (rc = dV.alloc((size_t)N * 4, stream)) ||
+        (rc = dG.alloc(zb, stream)))
+        return rc;
+    CUDA_TRY(cudaMemcpyAsync(dZ.p, Z, zb, cudaMemcpyHostToDevice, stream));
+    CUDA_TRY(cudaMemcpyAsync(dX.p, X_concat, xb, cudaMemcpyHostToDevice, stream));
+    rc = sdtw_value_grad((const float*)dZ.p, m, d, (const float*)dX.p, offsets, N, gamma, out_values ? (float*)dV.p : nullptr,
+                         out_grad ? (float*)dG.p : nullptr, stream_);
+    if (rc) return rc;
+    if (out_values) CUDA_TRY(cudaMemcpyAsync(out_values, dV.p, (size_t)N * 4, cudaMemcpyDeviceToHost, stream));
+    if (out_grad) CUDA_TRY(cudaMemcpyAsync(out_grad, dG.p, zb, cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));
+    return SDTW_OK;
+}
+
+int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                         float gamma, int32_t iters, float step, float* out_values, float* out_objective, void* stream_) {
+    int rc = check_common(Z_inout, m, d, X_concat, offsets, N, gamma);
+    if (rc) return rc;
+    if (iters < 0 || !std::isfinite(step)) return SDTW_ERR_INVALID_ARG;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const size_t zb = (size_t)m * d * 4, xb = (size_t)offsets[N] * d * 4;
+    DevBuf dZ, dX, dV, dO;
+    if ((rc = dZ.alloc(zb, stream)) || (rc = dX.alloc(xb, stream)) || (rc = dV.alloc((size_t)N * 4, stream)) ||
+        (rc = dO.alloc((size_t)std::max(iters, 1) * 4, stream)))
+        return rc;
+    CUDA_TRY(cudaMemcpyAsync(dZ.p, Z_inout, zb, cudaMemcpyHostToDevice, stream));
+    CUDA_TRY(cudaMemcpyAsync(dX.p, X_concat, xb, cudaMemcpyHostToDevice, stream));
+    rc = sdtw_barycenter((float*)dZ.p, m, d, (const float*)dX.p, offsets, N, gamma, iters, step,
+                         out_values ? (float*)dV.p : nullptr, out_objective ? (float*)dO.p : nullptr, stream_);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(Z_inout, dZ.p, zb, cudaMemcpyDeviceToHost, stream));
+    if (out_values && iters > 0) CUDA_TRY(cudaMemcpyAsync(out_values, dV.p, (size_t)N * 4, cudaMemcpyDeviceToHost, stream));
+    if (out_objective && iters > 0) CUDA_TRY(cudaMemcpyAsync(out_objective, dO.p, (size_t)iters * 4, cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));
+    return SDTW_OK;
+}
+
+// ---- workspace, status, instrumentation -------------------------------------------------------------------------
+size_t sdtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad) {
+    Layout L;
+    if (build_layout(m, d, offsets, N, want_grad != 0, L) != SDTW_OK) return 0;
+    return L.total;
+}
+
+int sdtw_set_workspace(void* dev_ptr, size_t bytes) {
+    std::lock_guard<std::mutex> lock(g_mutex);
+    if (dev_ptr && (reinterpret_cast<uintptr_t>(dev_ptr) & 255u)) return SDTW_ERR_INVALID_ARG;
+    if (!dev_ptr && bytes) return SDTW_ERR_INVALID_ARG;
+    g_user_ws = dev_ptr;
+    g_user_ws_bytes = dev_ptr ? bytes : 0;
+    return SDTW_OK;
+}
+
+const char* sdtw_status_string(int status) {
+    switch (status) {
+        case SDTW_OK: return "ok";
+        case SDTW_ERR_INVALID_ARG: return "invalid argument";
+        case SDTW_ERR_UNSUPPORTED: return "unsupported (d > SDTW_MAX_D, size beyond limits, or device is not sm_100)";
+        case SDTW_ERR_WORKSPACE: return "registered workspace too small";
+        case SDTW_ERR_CUDA: return "CUDA runtime error (see sdtw_last_cuda_error)";
+    }
+    return "unknown status";
+}
+
+int sdtw_last_cuda_error(void) { return g_last_cuda_error; }
+
+uint64_t sdtw_launch_count(void) {
+    std::lock_guard<std::mutex> lock(g_mutex);
+    return g_launches;
+}
+
+int sdtw_profile_enable(int on) {
+    std::lock_guard<std::mutex> lock(g_mutex);
+    g_profile = on != 0;
+    return SDTW_OK;
+}
+
+int sdtw_profile_read(double* ms_forward, double* ms_backward, double* ms_other, int64_t* evaluations) {
+    std::lock_guard<std::mutex> lock(g_mutex);
+    double f = 0, b = 0, o = 0;
+    for (auto& pr : g_prof) {
+        CUDA_TRY(cudaEventSynchronize(pr.e[3]));
+        float t = 0;
+        CUDA_TRY(cudaEventElapsedTime(&t, pr.e[0], pr.e[1])); f += t;
+        CUDA_TRY(cudaEventElapsedTime(&t, pr.e[1], pr.e[2])); b += t;
+        CUDA_TRY(cudaEventElapsedTime(&t, pr.e[2], pr.e[3])); o += t;
+        for (auto& e : pr.e) cudaEventDestroy(e);
+    }
+    if (ms_forward) *ms_forward = f;
+    if (ms_backward) *ms_backward = b;
+    if (ms_other) *ms_other = o;
+    if (evaluations) *evaluations = (int64_t)g_prof.size();
+    g_prof.clear();
+    return SDTW_OK;
+}
+
+int sdtw_tile_info(int32_t* cols_per_thread, int32_t* strip_cols, int32_t* ckpt_steps, int32_t* chunk_steps) {
+    if (cols_per_thread) *cols_per_thread = W;
+    if (strip_cols) *strip_cols = SW;
+    if (ckpt_steps) *ckpt_steps = TR;
+    if (chunk_steps) *chunk_steps = CH;
+    return SDTW_OK;
+}
+
+}  // extern "C"
