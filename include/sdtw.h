@@ -90,9 +90,11 @@ int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_co
 /*
  * Workspace.  sdtw_workspace_bytes() is what one call needs (tile-boundary strips, checkpoints of the forward state,
  * per-pair gradient partials).  If a workspace has been registered with sdtw_set_workspace() it is used (it must be
- * large enough, else SDTW_ERR_WORKSPACE, and must not be shared by calls running concurrently on different streams);
- * otherwise the library allocates with cudaMallocAsync / cudaFreeAsync on `stream`.  sdtw_set_workspace(NULL, 0)
- * unregisters.  The pointer must be 256-byte aligned.  Returns 0 bytes on invalid arguments.
+ * large enough, else SDTW_ERR_WORKSPACE); otherwise the library keeps one grow-only device buffer per GPU
+ * (cudaMalloc on first use / when a larger problem arrives -- that call blocks the host while allocating).  Calls
+ * that share the buffer from different streams are ordered on it with an event, so they are safe but not concurrent.
+ * sdtw_set_workspace(NULL, 0) unregisters the caller's buffer and frees the library-owned one of the current device.
+ * The pointer must be 256-byte aligned.  sdtw_workspace_bytes returns 0 on invalid arguments.
  */
 size_t sdtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad);
 int sdtw_set_workspace(void* dev_ptr, size_t bytes);

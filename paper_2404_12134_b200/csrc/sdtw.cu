@@ -298,24 +298,40 @@ int check_common(const void* Z, int64_t m, int32_t d, const void* X, const int64
     return SDTW_OK;
 }
 
+// Workspace: the caller's registered buffer, else a grow-only buffer owned by the library (one per device).  Calls
+// are serialised on the buffer by an event: a call on another stream waits for the previous call's work.
+struct WsCache { char* ptr = nullptr; size_t bytes = 0; cudaEvent_t last_use = nullptr; };
+WsCache g_ws_cache[64];
+
 struct Workspace {
     char* ptr = nullptr;
-    bool owned = false;
+    WsCache* cache = nullptr;
     cudaStream_t stream = nullptr;
-    int acquire(size_t bytes, cudaStream_t s) {
+    int acquire(size_t bytes, int dev, cudaStream_t s) {
         stream = s;
+        cache = &g_ws_cache[dev];
+        if (!cache->last_use) CUDA_TRY(cudaEventCreateWithFlags(&cache->last_use, cudaEventDisableTiming));
+        else CUDA_TRY(cudaStreamWaitEvent(s, cache->last_use, 0));
         if (g_user_ws) {
             if (g_user_ws_bytes < bytes) return SDTW_ERR_WORKSPACE;
             ptr = static_cast<char*>(g_user_ws);
             return SDTW_OK;
         }
-        void* q = nullptr;
-        CUDA_TRY(cudaMallocAsync(&q, bytes, s));
-        ptr = static_cast<char*>(q);
-        owned = true;
+        if (cache->bytes < bytes) {
+            if (cache->ptr) {                       // rare: the problem grew; wait for earlier users, then regrow
+                CUDA_TRY(cudaEventSynchronize(cache->last_use));
+                CUDA_TRY(cudaFree(cache->ptr));
+                cache->ptr = nullptr; cache->bytes = 0;
+            }
+            void* q = nullptr;
+            CUDA_TRY(cudaMalloc(&q, bytes));
+            cache->ptr = static_cast<char*>(q);
+            cache->bytes = bytes;
+        }
+        ptr = cache->ptr;
         return SDTW_OK;
     }
-    ~Workspace() { if (owned && ptr) cudaFreeAsync(ptr, stream); }
+    ~Workspace() { if (cache && cache->last_use) cudaEventRecord(cache->last_use, stream); }
 };
 
 }  // namespace
@@ -336,7 +352,7 @@ int sdtw_value_grad(const float* Z, int64_t m, int32_t d, const float* X_concat,
     rc = get_plan(di.dev, m, d, offsets, N, out_grad != nullptr, stream, &pl);
     if (rc) return rc;
     Workspace ws;
-    rc = ws.acquire(pl->L.total, stream);
+    rc = ws.acquire(pl->L.total, di.dev, stream);
     if (rc) return rc;
     return evaluate(*pl, ws.ptr, di, Z, X_concat, gamma, out_values, nullptr, out_grad, nullptr, 0.f, stream);
 }
@@ -356,7 +372,7 @@ int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat,
     rc = get_plan(di.dev, m, d, offsets, N, true, stream, &pl);
     if (rc) return rc;
     Workspace ws;
-    rc = ws.acquire(pl->L.total, stream);
+    rc = ws.acquire(pl->L.total, di.dev, stream);
     if (rc) return rc;
     for (int it = 0; it < iters; ++it) {
         float* vals = (it == iters - 1) ? out_values : nullptr;
@@ -447,6 +463,15 @@ int sdtw_set_workspace(void* dev_ptr, size_t bytes) {
     if (!dev_ptr && bytes) return SDTW_ERR_INVALID_ARG;
     g_user_ws = dev_ptr;
     g_user_ws_bytes = dev_ptr ? bytes : 0;
+    if (!dev_ptr) {                                 // also drop the library-owned buffer of the current device
+        int dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64 && g_ws_cache[dev].ptr) {
+            if (g_ws_cache[dev].last_use) cudaEventSynchronize(g_ws_cache[dev].last_use);
+            cudaFree(g_ws_cache[dev].ptr);
+            g_ws_cache[dev].ptr = nullptr;
+            g_ws_cache[dev].bytes = 0;
+        }
+    }
     return SDTW_OK;
 }
 

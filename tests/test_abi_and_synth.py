@@ -1,0 +1,90 @@
+"""CPU-side checks: libsdtw.so loads and exports every symbol include/sdtw.h declares (no compute calls), the
+host planner's argument handling, and the seeded input generator."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2404_12134_b200 import synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_2404_12134_b200 import build
+    build.build()
+    from paper_2404_12134_b200 import binding as b
+    return b
+
+
+def test_library_exports_every_declared_symbol(binding):
+    hdr = open(os.path.join(ROOT, "include", "sdtw.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(sdtw_[a-z_]+)\s*\(", hdr))
+    assert {"sdtw_value_grad", "sdtw_barycenter", "sdtw_workspace_bytes", "sdtw_set_workspace"} <= declared
+    lib = ctypes.CDLL(os.path.join(ROOT, "paper_2404_12134_b200", "libsdtw.so"))
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert declared == set(binding.SYMBOLS), declared ^ set(binding.SYMBOLS)
+
+
+def test_status_strings_and_tile_info(binding):
+    assert binding.status_string(0) == "ok"
+    for code in (-1, -2, -3, -4):
+        assert binding.status_string(code) not in ("ok", "unknown status")
+    assert binding.status_string(-99) == "unknown status"
+    ti = binding.sdtw_tile_info()
+    assert ti["strip_cols"] == 32 * ti["cols_per_thread"] and ti["chunk_steps"] % ti["ckpt_steps"] == 0
+
+
+def test_workspace_bytes_planner(binding):
+    off = np.array([0, 30000, 57000, 90000])
+    full = binding.sdtw_workspace_bytes(30000, 1, off, True)
+    fwd = binding.sdtw_workspace_bytes(30000, 1, off, False)
+    assert 0 < fwd < full
+    ti = binding.sdtw_tile_info()
+    # checkpoints dominate: (W+1) floats per thread per ckpt_steps => 4 (W+1) / (W ckpt_steps) bytes per cell
+    cells = 90000 * 30000
+    per_cell = 4 * (ti["cols_per_thread"] + 1) / (ti["cols_per_thread"] * ti["ckpt_steps"])
+    assert 0.9 * per_cell * cells < full < 1.3 * per_cell * cells
+    # invalid arguments -> 0
+    assert binding.sdtw_workspace_bytes(0, 1, off, True) == 0
+    assert binding.sdtw_workspace_bytes(10, 0, off, True) == 0
+    assert binding.sdtw_workspace_bytes(10, 1, np.array([0, 5, 5]), True) == 0       # empty cycle
+    assert binding.sdtw_workspace_bytes(10, 1, np.array([1, 5, 9]), True) == 0       # offsets[0] != 0
+    assert binding.sdtw_workspace_bytes(10, 5, off, True) == 0                        # d above compiled maximum
+    # size is monotone in the problem
+    assert binding.sdtw_workspace_bytes(30000, 1, off[:3], True) < full
+
+
+def test_synth_is_deterministic_and_shaped():
+    a, b = synth.make(2), synth.make(2)
+    assert np.array_equal(a["X"], b["X"]) and np.array_equal(a["Z0"], b["Z0"]) and np.array_equal(a["offsets"], b["offsets"])
+    cfg = a["cfg"]
+    assert a["X"].dtype == np.float32 and a["Z0"].dtype == np.float32 and a["offsets"].dtype == np.int64
+    assert a["Z0"].shape == (cfg.m, cfg.d) and len(a["lengths"]) == cfg.N
+    assert a["lengths"].min() >= cfg.n_lo and a["lengths"].max() <= cfg.n_hi
+    assert a["offsets"][0] == 0 and a["offsets"][-1] == a["X"].shape[0]
+    c = synth.make(2, seed=7)
+    assert not np.array_equal(a["lengths"], c["lengths"])
+
+
+def test_synth_configs_match_baseline_json():
+    c = synth.CONFIGS
+    assert (c[1].N, c[1].n_lo, c[1].n_hi, c[1].m, c[1].gamma, c[1].iters, c[1].step) == (8, 48, 64, 56, 1.0, 10, 0.01)
+    assert (c[2].N, c[2].m, c[2].gamma, c[2].iters) == (64, 1000, 0.1, 20)
+    assert (c[3].N, c[3].d, c[3].m, c[3].gamma, c[3].iters) == (32, 4, 10000, 0.1, 10)
+    assert (c[4].N, c[4].n_lo, c[4].n_hi, c[4].m, c[4].gamma, c[4].iters) == (100, 27000, 33000, 30000, 0.01, 5)
+    assert (c[5].N, c[5].n_lo, c[5].n_hi, c[5].m, c[5].iters, c[5].anomaly_frac) == (1000, 20000, 40000, 30000, 0, 0.05)
+
+
+def test_synth_scoring_sweep_small():
+    cfg = synth.scaled(synth.CONFIGS[5], 0.01, N=40)
+    d = synth.make(cfg)
+    assert d["anomalous"].sum() == 2 and d["Z0"].shape == (cfg.m, 1)
+    # multichannel cycles share one warp: plateaus (zero slope) coincide across channels up to the noise
+    d3 = synth.make(synth.scaled(synth.CONFIGS[3], 0.05, N=3))
+    assert d3["X"].shape[1] == 4

@@ -1,0 +1,294 @@
+"""Parity of the CUDA path (through the C ABI of include/sdtw.h) with the float64 oracle.
+
+Tolerances (BASELINE.json north_star):
+  per-pair values : |v - v*| <= 1e-4 * max(|v*|, gamma (n_k + m))      (reading C10; the strict |v*| ratio is printed)
+  summed gradient : ||G - G*||_2 <= 2e-3 ||G*||_2
+  barycenter      : ||Z - Z*||_2 <= 2e-3 ||Z*||_2  after the configured iterations
+"""
+import dataclasses
+import os
+
+import numpy as np
+import pytest
+
+from paper_2404_12134_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+VAL_TOL, GRAD_TOL, BARY_TOL = 1e-4, 2e-3, 2e-3
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2404_12134_b200 import binding
+    return binding
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(np.asarray(a, np.float64) - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def check_values(v, ov, lengths, cfg, tag=""):
+    v = np.asarray(v, np.float64)
+    den = np.maximum(np.abs(ov), cfg.gamma * (np.asarray(lengths) + cfg.m))
+    err = np.abs(v - ov) / den
+    strict = np.abs(v - ov) / np.maximum(np.abs(ov), 1e-300)
+    print(f"[{tag}] values: C10 rel max {err.max():.3e}, strict rel max {strict.max():.3e}")
+    assert err.max() <= VAL_TOL, (tag, err.max())
+
+
+def run_value_grad(B, oracle, data, tag, mode="checkpointed"):
+    import torch
+    cfg = data["cfg"]
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    vals, G = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+    vals_f, none = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
+    torch.cuda.synchronize()
+    ov, oG = oracle.value_grad(data["Z0"], data["X"], data["offsets"], cfg.gamma, mode=mode)
+    check_values(vals.cpu().numpy(), ov, data["lengths"], cfg, tag)
+    assert none is None and torch.equal(vals, vals_f)            # forward-only sweep computes the same values
+    e = rel_l2(G.cpu().numpy(), oG)
+    print(f"[{tag}] gradient rel L2 {e:.3e}")
+    assert e <= GRAD_TOL, (tag, e)
+    return vals, G
+
+
+# ------------------------------------------------------------------------------------------- the five configurations
+def test_cfg1_tiny_value_grad_and_barycenter(B, oracle):
+    data = synth.make(1)
+    cfg = data["cfg"]
+    run_value_grad(B, oracle, data, "cfg1", mode="full")
+    Z, vals, obj = B.sdtw_barycenter(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, cfg.iters, cfg.step)
+    Zo, vo, oo = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, cfg.iters, cfg.step)
+    assert rel_l2(Z.cpu().numpy(), Zo) <= BARY_TOL
+    moved = np.linalg.norm(Z.cpu().numpy() - Zo) / np.linalg.norm(Zo - data["Z0"])
+    print(f"[cfg1] barycenter rel L2 {rel_l2(Z.cpu().numpy(), Zo):.3e}, relative to distance moved {moved:.3e}")
+    assert moved <= 1e-2
+    check_values(vals.cpu().numpy(), vo, data["lengths"], cfg, "cfg1 bary values")
+    assert np.allclose(obj.cpu().numpy(), oo, rtol=1e-5)
+
+
+def test_cfg2_medium_value_grad_and_barycenter(B, oracle):
+    data = synth.make(2)
+    cfg = data["cfg"]
+    run_value_grad(B, oracle, data, "cfg2")
+    Z, vals, obj = B.sdtw_barycenter(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, cfg.iters, cfg.step)
+    Zo, vo, oo = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, cfg.iters, cfg.step, mode="checkpointed")
+    e = rel_l2(Z.cpu().numpy(), Zo)
+    moved = np.linalg.norm(Z.cpu().numpy() - Zo) / np.linalg.norm(Zo - data["Z0"])
+    print(f"[cfg2] barycenter rel L2 {e:.3e}, relative to distance moved {moved:.3e}; objective {oo[0]:.2f} -> {oo[-1]:.2f}")
+    assert e <= BARY_TOL
+    assert np.allclose(obj.cpu().numpy(), oo, rtol=1e-4)
+    check_values(vals.cpu().numpy(), vo, data["lengths"], cfg, "cfg2 bary values")
+
+
+@pytest.mark.parametrize("idx,scale,N,iters", [(3, 0.1, 6, 4), (4, 0.1, 10, 3), (4, 0.2, 3, 0)])
+def test_scaled_multichannel_and_full_length(B, oracle, idx, scale, N, iters):
+    """cfg 3 / cfg 4 generators at reduced length: several strips, ragged tails, d = 4, gamma = 0.01."""
+    cfg = synth.scaled(synth.CONFIGS[idx], scale, N=N)
+    data = synth.make(cfg)
+    run_value_grad(B, oracle, data, cfg.name)
+    if iters:
+        step = 0.08 / N * 0.25
+        Z, vals, obj = B.sdtw_barycenter(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, iters, step)
+        Zo, vo, oo = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, iters, step, mode="checkpointed")
+        e = rel_l2(Z.cpu().numpy(), Zo)
+        print(f"[{cfg.name}] barycenter rel L2 {e:.3e}; objective {oo}")
+        assert e <= BARY_TOL
+
+
+def test_scaled_scoring_sweep_forward_only(B, oracle):
+    import torch
+    cfg = synth.scaled(synth.CONFIGS[5], 0.05, N=60)
+    data = synth.make(cfg)
+    vals, G = B.sdtw_value_grad(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, want_grad=False)
+    assert G is None
+    ov, _ = oracle.value_grad(data["Z0"], data["X"], data["offsets"], cfg.gamma, want_grad=False)
+    check_values(vals.cpu().numpy(), ov, data["lengths"], cfg, cfg.name)
+    # anomalous cycles score higher than the median normal one (what Step 3 of the paper uses the value for)
+    v = vals.cpu().numpy()
+    assert np.median(v[data["anomalous"]]) > np.median(v[~data["anomalous"]])
+
+
+# ------------------------------------------------------------------------------------------- edge cases
+SHAPES = [(1, 1, 1, 1, 2), (1, 1, 1, 3, 1), (1, 3, 5, 2, 3), (7, 9, 3, 1, 2), (5, 6, 8, 1, 2), (3, 4, 9, 1, 1),
+          (300, 310, 257, 3, 2), (250, 260, 256, 1, 3), (40, 50, 513, 1, 2), (600, 700, 255, 2, 2), (31, 33, 40, 4, 5),
+          (1, 2, 300, 1, 2), (900, 901, 1, 1, 2), (64, 64, 7, 1, 1)]
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+@pytest.mark.parametrize("gamma", [1.0, 0.01])
+def test_edge_shapes(B, oracle, shape, gamma):
+    """n = 1, m = 1, m < one thread's columns, m = strip width +- 1, single-row strips, d = 1..4."""
+    n_lo, n_hi, m, d, N = shape
+    cfg = dataclasses.replace(synth.CONFIGS[2], N=N, n_lo=n_lo, n_hi=n_hi, m=m, d=d, gamma=gamma, name=f"edge{shape}")
+    data = synth.make(cfg, seed=hash(shape) % 10000)
+    rng = np.random.default_rng(1)
+    data["Z0"] = (data["Z0"] + 0.1 * rng.normal(size=data["Z0"].shape)).astype(np.float32)   # keep the gradient non-degenerate
+    run_value_grad(B, oracle, data, cfg.name, mode="full")
+
+
+def test_expected_alignment_mass_and_constant_inputs(B, oracle):
+    """D == 0 (x == z == const): value = -gamma ln Del(n-1, m-1) (closed form, any size) and zero gradient."""
+    import math
+    import torch
+    n, m, gamma = 700, 523, 0.5
+    X = np.full((n, 1), 0.25, np.float32)
+    Z = np.full((m, 1), 0.25, np.float32)
+    vals, G = B.sdtw_value_grad(_dev(Z), _dev(X), np.array([0, n]), gamma)
+    ov, oG = oracle.value_grad(Z, X, np.array([0, n]), gamma)
+    assert abs(vals.item() - ov[0]) <= 1e-4 * abs(ov[0])
+    assert float(G.abs().max()) <= 1e-6 and np.abs(oG).max() == 0.0
+
+
+# ------------------------------------------------------------------------------------------- API behaviour
+def test_determinism_bitwise_and_workspace_registration(B):
+    import torch
+    cfg = synth.scaled(synth.CONFIGS[4], 0.1, N=12)
+    data = synth.make(cfg)
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    v1, g1 = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+    v2, g2 = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+    assert torch.equal(v1, v2) and torch.equal(g1, g2)
+    need = B.sdtw_workspace_bytes(cfg.m, cfg.d, data["offsets"], True)
+    ws = torch.empty(need + 256, dtype=torch.uint8, device="cuda")
+    try:
+        B.sdtw_set_workspace(ws)
+        v3, g3 = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+        assert torch.equal(v1, v3) and torch.equal(g1, g3)
+        small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+        B.sdtw_set_workspace(small)
+        with pytest.raises(B.SdtwError) as ei:
+            B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+        assert ei.value.status == B.SDTW_ERR_WORKSPACE
+    finally:
+        B.sdtw_set_workspace(None)
+    # a side stream gives the same bits
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        v4, g4 = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, stream=s)
+    s.synchronize()
+    assert torch.equal(v1, v4) and torch.equal(g1, g4)
+
+
+def test_argument_errors_leave_outputs_untouched(B):
+    import torch
+    data = synth.make(1)
+    cfg = data["cfg"]
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    vals = torch.full((cfg.N,), 7.0, device="cuda")
+    G = torch.full_like(Z, 7.0)
+    for gamma in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(B.SdtwError) as ei:
+            B.sdtw_value_grad(Z, X, data["offsets"], gamma, out_values=vals, out_grad=G)
+        assert ei.value.status == B.SDTW_ERR_INVALID_ARG
+    bad = data["offsets"].copy()
+    bad[3] = bad[2]
+    with pytest.raises(B.SdtwError):
+        B.sdtw_value_grad(Z, X, bad, cfg.gamma, out_values=vals, out_grad=G)
+    with pytest.raises(B.SdtwError) as ei:
+        B.sdtw_barycenter(Z.clone(), X, data["offsets"], cfg.gamma, -1, 0.01)
+    assert ei.value.status == B.SDTW_ERR_INVALID_ARG
+    Z5 = torch.zeros(10, 5, device="cuda")
+    with pytest.raises(B.SdtwError) as ei:
+        B.sdtw_value_grad(Z5, torch.zeros(20, 5, device="cuda"), np.array([0, 20]), 1.0)
+    assert ei.value.status == B.SDTW_ERR_UNSUPPORTED
+    torch.cuda.synchronize()
+    assert float(vals.min()) == 7.0 and float(G.min()) == 7.0
+    # iters = 0 is a legal no-op
+    Zc = Z.clone()
+    B.sdtw_barycenter(Zc, X, data["offsets"], cfg.gamma, 0, 0.01)
+    assert torch.equal(Zc, Z)
+
+
+def test_host_buffer_entry_points_and_gd_update(B, oracle):
+    import torch
+    data = synth.make(1)
+    cfg = data["cfg"]
+    vals = np.zeros(cfg.N, np.float32)
+    G = np.zeros_like(data["Z0"])
+    B.sdtw_value_grad_host(data["Z0"], data["X"], data["offsets"], cfg.gamma, vals, G)
+    dv, dG = B.sdtw_value_grad(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma)
+    assert np.array_equal(vals, dv.cpu().numpy()) and np.array_equal(G, dG.cpu().numpy())
+    Zh = data["Z0"].copy()
+    obj = np.zeros(cfg.iters, np.float32)
+    B.sdtw_barycenter_host(Zh, data["X"], data["offsets"], cfg.gamma, cfg.iters, cfg.step, None, obj)
+    Zd, _, objd = B.sdtw_barycenter(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, cfg.iters, cfg.step)
+    assert np.array_equal(Zh, Zd.cpu().numpy()) and np.array_equal(obj, objd.cpu().numpy())
+    # value_grad + gd_update == one barycenter iteration (the multi-GPU loop's building blocks)
+    Z1 = _dev(data["Z0"])
+    B.sdtw_gd_update(Z1, dG, cfg.step)
+    Zb, _, _ = B.sdtw_barycenter(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, 1, cfg.step)
+    assert torch.equal(Z1, Zb)
+
+
+def test_additivity_and_pair_order(B):
+    """Summed result = sum of single-pair calls; values come back in the caller's pair order."""
+    import torch
+    cfg = synth.scaled(synth.CONFIGS[4], 0.05, N=5)
+    data = synth.make(cfg)
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    vals, G = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+    acc = torch.zeros_like(G, dtype=torch.float64)
+    for k in range(cfg.N):
+        a, b = data["offsets"][k], data["offsets"][k + 1]
+        vk, gk = B.sdtw_value_grad(Z, X[a:b].contiguous(), np.array([0, b - a]), cfg.gamma)
+        assert vk.item() == vals[k].item()
+        acc += gk.double()
+    assert rel_l2(G.cpu().numpy(), acc.cpu().numpy()) < 1e-6
+
+
+# ------------------------------------------------------------------------------------------- full sizes (sampled)
+@pytest.mark.timeout(1500)
+def test_full_size_cfg3_cfg4_cfg5_sampled_against_oracle(B, oracle):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (all pairs in one call).  The oracle
+    computes a sample of pairs one by one: their values must match the full call's values; the gradient of the
+    sampled pairs alone (separable per pair) is checked at full length; properties cover the rest."""
+    import torch
+    ncpu = os.cpu_count() or 1
+    for idx, nsample in ((3, 2), (4, 2), (5, 3)):
+        data = synth.make(idx)
+        cfg = data["cfg"]
+        Z, X = _dev(data["Z0"]), _dev(data["X"])
+        want_grad = cfg.iters > 0
+        vals, G = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=want_grad)
+        torch.cuda.synchronize()
+        assert torch.isfinite(vals).all()
+        rng = np.random.default_rng(idx)
+        ks = np.sort(rng.choice(cfg.N, size=nsample, replace=False))
+        if idx == 5:                                    # make sure an anomalous cycle is in the sample
+            ks[0] = int(np.flatnonzero(data["anomalous"])[0])
+            ks = np.unique(ks)
+        from paper_2404_12134_b200.dist import take_pairs
+        Xs, offs = take_pairs(data["X"], data["offsets"], ks)
+        ov, oG = oracle.value_grad(data["Z0"], Xs, offs, cfg.gamma, want_grad=want_grad, mode="checkpointed",
+                                   nthreads=min(ncpu, len(ks)))
+        sub = dataclasses.replace(cfg)
+        check_values(vals.cpu().numpy()[ks], ov, data["lengths"][ks], sub, f"cfg{idx} full size, pairs {ks.tolist()}")
+        if want_grad:
+            vs, Gs = B.sdtw_value_grad(Z, _dev(Xs), offs, cfg.gamma)
+            assert torch.equal(vs.cpu(), vals.cpu()[torch.from_numpy(ks)])       # same bits alone or inside the batch
+            e = rel_l2(Gs.cpu().numpy(), oG)
+            print(f"[cfg{idx} full size] gradient of pairs {ks.tolist()} rel L2 {e:.3e}")
+            assert e <= GRAD_TOL
+            assert torch.isfinite(G).all()
+            # the batch call (work queue, strip-major schedule, reduction over pairs) against the sum of single-pair
+            # calls over ALL pairs (pair independence)
+            acc = torch.zeros_like(G, dtype=torch.float64)
+            for k in range(cfg.N):
+                a, b = int(data["offsets"][k]), int(data["offsets"][k + 1])
+                vk, gk = B.sdtw_value_grad(Z, X[a:b], np.array([0, b - a]), cfg.gamma)
+                assert vk.item() == vals[k].item()
+                acc += gk.double()
+            e = rel_l2(G.cpu().numpy(), acc.cpu().numpy())
+            print(f"[cfg{idx} full size] batch gradient vs sum of {cfg.N} single-pair calls: rel L2 {e:.3e}")
+            assert e <= 1e-5
+        del Z, X, vals, G
+        torch.cuda.empty_cache()
