@@ -222,38 +222,49 @@ def run_ours(args):
     value = cells_job / (ms_step * 1e-3)
 
     # ---- end to end: HOST buffers in, HOST results out, every step (C-ABI host entry point at N = 1)
-    Xh = torch.from_numpy(data["X"]).pin_memory()
-    Zh = torch.from_numpy(data["Z0"].copy()).pin_memory()
-    objh = torch.zeros(1, dtype=torch.float32).pin_memory()
-    valh = torch.zeros(cfg.N, dtype=torch.float32).pin_memory()
-    e2e_steps = max(1, min(args.steps, 3))
+    e2e = None
+    if not args.skip_e2e:
+        Xh = torch.from_numpy(data["X"]).pin_memory()
+        Zh = torch.from_numpy(data["Z0"].copy()).pin_memory()
+        objh = torch.zeros(1, dtype=torch.float32).pin_memory()
+        valh = torch.zeros(cfg.N, dtype=torch.float32).pin_memory()
+        e2e_steps = max(1, min(args.steps, 3))
 
-    def e2e_step():
-        if world == 1 and not forward_only:
-            B.sdtw_barycenter_host(Zh, Xh, offsets, cfg.gamma, 1, cfg.step, valh, objh,
-                                   stream=torch.cuda.current_stream().cuda_stream)
-        elif world == 1:
-            B.sdtw_value_grad_host(Zh, Xh, offsets, cfg.gamma, valh, None, stream=torch.cuda.current_stream().cuda_stream)
-        else:
-            X.copy_(Xh, non_blocking=True)
-            Z.copy_(Zh, non_blocking=True)
-            step()
-            Zh.copy_(Z, non_blocking=True)
-            valh.copy_(vals, non_blocking=True)
-            torch.cuda.synchronize()
+        def e2e_step():
+            if world == 1 and not forward_only:
+                B.sdtw_barycenter_host(Zh, Xh, offsets, cfg.gamma, 1, cfg.step, valh, objh,
+                                       stream=torch.cuda.current_stream().cuda_stream)
+            elif world == 1:
+                B.sdtw_value_grad_host(Zh, Xh, offsets, cfg.gamma, valh, None, stream=torch.cuda.current_stream().cuda_stream)
+            else:
+                X.copy_(Xh, non_blocking=True)
+                Z.copy_(Zh, non_blocking=True)
+                step()
+                Zh.copy_(Z, non_blocking=True)
+                valh.copy_(vals, non_blocking=True)
+                torch.cuda.synchronize()
 
-    e2e_step()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
         e2e_step()
-    barrier()
-    t_e2e = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-    e2e_val = cells_job / float(t_e2e.item())
-    h2d = int(Xh.numel() * 4 + Zh.numel() * 4)
-    d2h = int(valh.numel() * 4 + (0 if forward_only else Zh.numel() * 4 + 4))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e2e_step()
+        barrier()
+        t_e2e = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
+        e2e_val = cells_job / float(t_e2e.item())
+        h2d = int(Xh.numel() * 4 + Zh.numel() * 4)
+        d2h = int(valh.numel() * 4 + (0 if forward_only else Zh.numel() * 4 + 4))
+        e2e = {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "steps": e2e_steps, "api": "sdtw_barycenter_host" if world == 1 and not forward_only else
+               ("sdtw_value_grad_host" if world == 1 else "pinned copies + sdtw_value_grad + all_reduce + sdtw_gd_update")}
+
+    # ---- measured special-function issue rate of this device (the roofline denominator)
+    mufu = {}
+    if rank == 0:
+        for kind, name in ((0, "ex2"), (1, "lg2"), (2, "rcp")):
+            mufu[name], _ = B.sdtw_measure_mufu_peak(kind)
 
     if rank == 0:
         sm_max_hz = (clocks.get("sm_max_mhz") or 1965.0) * 1e6
@@ -273,6 +284,7 @@ def run_ours(args):
             "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
             "peak_source": f"derived: {MUFU_PER_CLK_PER_SM} MUFU results/clk/SM x {sms} SMs x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm); "
                            "MEASURED_PEAKS.json holds no ALU figure (DESIGN.md section 8)",
+            "mufu_measured_gops": {k: v / 1e9 for k, v in mufu.items()},
             "algorithmic_per_cell": {"forward": ALGO_MUFU_FWD, "reverse": ALGO_MUFU_BWD},
             "kernel_ms": {"forward": t_fwd * 1e3, "reverse": t_bwd * 1e3, "other": prof["ms_other"] / n_eval},
             "forward_frac": (ALGO_MUFU_FWD * ncells_local / t_fwd) / mufu_peak if t_fwd > 0 else None,
@@ -280,7 +292,7 @@ def run_ours(args):
             "checkpoint_hbm_gbs": None if forward_only else
                 (2 * ws_bytes) / max(t_fwd + t_bwd, 1e-9) / 1e9,
         }
-        cpu = time_oracle(data)
+        cpu = None if args.skip_cpu else time_oracle(data)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
@@ -291,9 +303,7 @@ def run_ours(args):
                        "tile": B.sdtw_tile_info()},
             "barycenter_iter_s": ms_step * 1e-3,
             "roofline": roofline, "cpu_baseline": cpu,
-            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": e2e_steps, "api": "sdtw_barycenter_host" if world == 1 and not forward_only else
-                    ("sdtw_value_grad_host" if world == 1 else "pinned copies + sdtw_value_grad + all_reduce + sdtw_gd_update")},
+            "e2e": e2e,
             "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(out))
@@ -309,6 +319,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--skip-e2e", action="store_true", help="profiling runs only: leave out the host-buffer leg")
+    ap.add_argument("--skip-cpu", action="store_true", help="profiling runs only: leave out the timed oracle leg")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

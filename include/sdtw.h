@@ -115,6 +115,14 @@ uint64_t sdtw_launch_count(void);
 int sdtw_profile_enable(int on);
 int sdtw_profile_read(double* ms_forward, double* ms_backward, double* ms_other, int64_t* evaluations);
 
+/*
+ * sdtw_measure_mufu_peak -- measurement, not part of the numerical path: runs dependent chains of one special-function
+ * instruction (kind 0 = ex2.approx, 1 = lg2.approx, 2 = rcp.approx; the three the kernels use) on every SM of the
+ * current device on a private stream, BLOCKS until done, and returns results per second (best of 3) and the SM count.
+ * This is the denominator of the roofline bench.py reports.
+ */
+int sdtw_measure_mufu_peak(int32_t kind, double* ops_per_s, int32_t* sm_count);
+
 /* Compile-time tile constants, for DESIGN.md / bench.py reporting: columns per thread, steps between checkpoints. */
 int sdtw_tile_info(int32_t* cols_per_thread, int32_t* strip_cols, int32_t* ckpt_steps, int32_t* chunk_steps);
 

@@ -34,6 +34,7 @@ SYMBOLS = {
     "sdtw_profile_enable": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_profile_read": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double)] * 3 + [_i64p]),
     "sdtw_tile_info": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int32)] * 4),
+    "sdtw_measure_mufu_peak": (ctypes.c_int, [_i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int32)]),
 }
 for _name, (_res, _args) in SYMBOLS.items():
     _fn = getattr(_lib, _name)          # AttributeError here = the library does not export what sdtw.h declares
@@ -208,3 +209,10 @@ def sdtw_tile_info():
     v = [ctypes.c_int32(0) for _ in range(4)]
     _check(_lib.sdtw_tile_info(*[ctypes.byref(x) for x in v]))
     return dict(cols_per_thread=v[0].value, strip_cols=v[1].value, ckpt_steps=v[2].value, chunk_steps=v[3].value)
+
+
+def sdtw_measure_mufu_peak(kind: int = 0):
+    """Measured special-function results per second on the current device (0 = ex2, 1 = lg2, 2 = rcp) and SM count."""
+    r, n = ctypes.c_double(0), ctypes.c_int32(0)
+    _check(_lib.sdtw_measure_mufu_peak(int(kind), ctypes.byref(r), ctypes.byref(n)))
+    return r.value, n.value

@@ -15,7 +15,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libsdtw.so"
-SOURCES = [CSRC / "sdtw.cu"]
+SOURCES = [CSRC / "sdtw.cu", CSRC / "mufu_peak.cu"]
 DEPS = SOURCES + [CSRC / "sdtw_kernels.cuh", ROOT / "include" / "sdtw.h"]
 
 

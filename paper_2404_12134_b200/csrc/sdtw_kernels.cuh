@@ -109,27 +109,44 @@ __device__ __forceinline__ void stage_x(float* xs, const float* __restrict__ X, 
 
 // ------------------------------------------------------------------------------------------------------------------
 // one cell of the difference-form recurrence.  v is v_in on entry and v_out on return; h is h_in / h_out.
+// t2 is the SQUARED cost input: the cell cost is D = sum_c t_c^2, passed as (t_last, acc) with D = t_last^2 + acc so
+// that the last square fuses with the subtraction of the log (one FFMA).
+// With a = mn - h_in, b = mn - v_in (mn = min(0, h_in, v_in); one of 0, a, b is exactly 0) the three soft-min terms are
+// 2^mn (diagonal), 2^a ("up"), 2^b ("left"); sorted, they are 1, e1 = 2^-|min(h,v)| and e2 = 2^min(a,b).
 // STASH: also emit the weights (w_up, w_left) of this cell's "up" and "left" predecessors.
-template <bool STASH>
-__device__ __forceinline__ void cell(float Dc, float& h, float& v, float& wu, float& wl) {
+__device__ __forceinline__ float min3(float a, float b, float c) {
+    float r; asm("min.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c)); return r;
+}
+template <bool STASH, bool HASACC>
+__device__ __forceinline__ void cell(float t_last, float acc, float& h, float& v, float& wu, float& wl) {
     const float hin = h, vin = v;
-    const float p = fminf(hin, vin), q = fmaxf(hin, vin);
-    const float mn = fminf(p, 0.f);
-    const float e1 = ex2_approx(-fabsf(p));     // p >= 0: the p term;    p < 0: the diagonal term
-    const float e2 = ex2_approx(mn - q);        // the q term
+    const float mn = min3(hin, vin, 0.f);
+    const float p = fminf(hin, vin);
+    const float a = mn - hin, b = mn - vin;
+    const float e1 = ex2_approx(-fabsf(p));     // p >= 0: the min(h,v) term;  p < 0: the diagonal term
+    const float e2 = ex2_approx(fminf(a, b));   // the max(h,v) term
     const float S = (1.f + e1) + e2;
     const float l = lg2_approx(S);
-    const float c = Dc - l;
-    h = c + (mn - vin);
-    v = c + (mn - hin);
+    const float c = HASACC ? fmaf(t_last, t_last, acc - l) : fmaf(t_last, t_last, -l);
+    h = c + b;
+    v = c + a;
     if constexpr (STASH) {
         const float rS = rcp_approx(S);
         const float wp = (p < 0.f) ? rS : e1 * rS;
         const float wq = e2 * rS;
-        const bool h_is_p = hin <= vin;
+        const bool h_is_p = a >= b;             // h_in <= v_in
         wu = h_is_p ? wp : wq;
         wl = h_is_p ? wq : wp;
     }
+}
+
+// cost of one cell as (t_last, acc): D = t_last^2 + acc
+template <int D>
+__device__ __forceinline__ void sqdist2(const XRow<D>& x, const float (&z)[D], float& t_last, float& acc) {
+    acc = 0.f;
+#pragma unroll
+    for (int c = 0; c + 1 < D; ++c) { const float t = x.c[c] - z[c]; acc = fmaf(t, t, acc); }
+    t_last = x.c[D - 1] - z[D - 1];
 }
 
 template <int D>
@@ -141,8 +158,17 @@ __device__ __forceinline__ float sqdist(const XRow<D>& x, const float (&z)[D]) {
     return acc;
 }
 
+struct FastTag { static constexpr bool slow = false; };
+struct SlowTag { static constexpr bool slow = true; };
+
+// chunk c (steps 32c .. 32c+31, rows 32c-31 .. 32c+31 over the 32 lanes) touches only valid rows
+__device__ __forceinline__ bool interior_chunk(int c, int n) { return c >= 1 && c * CH + CH <= n; }
+
 // ------------------------------------------------------------------------------------------------------------------
-// forward: eq. 5 in difference form, value by a staircase sum, strip-boundary column to VS, checkpoints to CK
+// forward: eq. 5 in difference form, value by a staircase sum, strip-boundary column to VS, checkpoints to CK.
+// Chunks whose 32 x 32 (step, lane) block lies inside the matrix and off this warp's value staircase run the FAST
+// step (no bounds or staircase tests, 8 steps unrolled between checkpoints); the others run the general step.  Both
+// evaluate every cell with the same expressions.
 template <int D, bool CKPT>
 __global__ void __launch_bounds__(WARPS * 32) forward_kernel(const Params p) {
     extern __shared__ __align__(16) float smem[];
@@ -150,6 +176,7 @@ __global__ void __launch_bounds__(WARPS * 32) forward_kernel(const Params p) {
     float* xs = smem + warp * fwd_smem_floats<D>();
     float* vin_s = xs + 64 * D;
     float* vout_s = vin_s + 32;
+    const float* xs_lane = xs + (32 - lane) * D;           // row (c*CH + t - lane) of the staged window is xs_lane[t*D ..]
     const int m = p.m;
 
     for (;;) {
@@ -189,32 +216,27 @@ __global__ void __launch_bounds__(WARPS * 32) forward_kernel(const Params p) {
             r_h = rho_prev; jlo = max(1, j0); jhi = j0 + W - 1; r_v0 = rho_prev; r_v1 = rho_cur;
         } else { r_h = n - 1; jlo = j0; jhi = m - 1; r_v0 = r_v1 = n - 1; }
         float vacc = 0.f, hsum = 0.f;
+        // chunks that hold a staircase row of some lane of this warp (row i of lane l is visited at step i + l)
+        const int c_v0 = __reduce_min_sync(FULL, min(r_h, r_v0)) / CH;
+        const int c_v1 = (__reduce_max_sync(FULL, max(r_h, r_v1)) + 31) / CH;
 
-        unsigned seen = 0;
-        for (int c = 0; c < C; ++c) {
-            if (J > 0) {                                   // wait until the left strip has published what this chunk reads
-                const unsigned need = (unsigned)min(c + 2, C);
-                while (seen < need) { seen = ld_acquire(p.prog_f + item - 1); if (seen < need) __nanosleep(256); }
-            }
-            {
-                const int s = c * CH + lane;               // lane 0 works on row s at step s
-                vin_s[lane] = (J > 0) ? VSprev[s + 31] : ((s == 0) ? BIG : 0.f);
-                stage_x<D>(xs, p.X, pm.x_off, n, c, lane, p.sqrtk);
-            }
-            __syncwarp();
-            for (int t = 0; t < CH; ++t) {
-                const int s = c * CH + t, i = s - lane;
-                float v = __shfl_up_sync(FULL, vprev, 1);
-                if (lane == 0) v = vin_s[t];
-                if ((unsigned)i < (unsigned)n) {
-                    const XRow<D> x = load_x<D>(xs, 32 + t - lane);
-                    float vfirst = 0.f, dummy0, dummy1;
+        auto step = [&](const int c, const int t, auto tag) {
+            constexpr bool slow = decltype(tag)::slow;
+            float v = __shfl_up_sync(FULL, vprev, 1);
+            if (lane == 0) v = vin_s[t];
+            const int i = c * CH + t - lane;
+            if (!slow || (unsigned)i < (unsigned)n) {
+                const XRow<D> x = load_x<D>(xs_lane, t);
+                float vfirst = 0.f, dummy0, dummy1;
 #pragma unroll
-                    for (int w = 0; w < W; ++w) {
-                        cell<false>(sqdist<D>(x, z[w]), h[w], v, dummy0, dummy1);
-                        if (w == 0) vfirst = v;
-                    }
-                    vprev = v;
+                for (int w = 0; w < W; ++w) {
+                    float tl, acc;
+                    sqdist2<D>(x, z[w], tl, acc);
+                    cell<false, (D > 1)>(tl, acc, h[w], v, dummy0, dummy1);
+                    if (slow && w == 0) vfirst = v;
+                }
+                vprev = v;
+                if constexpr (slow) {
                     if ((unsigned)(i - r_v0 - 1) < (unsigned)(r_v1 - r_v0)) vacc += vfirst_sel ? vfirst : v;
                     if (i == r_h) {
 #pragma unroll
@@ -222,19 +244,46 @@ __global__ void __launch_bounds__(WARPS * 32) forward_kernel(const Params p) {
                     }
                     if (T == 0 && i == 0) hsum += sqdist<D>(x, z[0]);   // r_11 = D_11
                 }
-                if (lane == 31) vout_s[t] = vprev;
-                if (CKPT && ((t + 1) & (TR - 1)) == 0) {   // state after step s = checkpoint (s+1)/TR
-                    float* ck = CKme + (long long)((s + 1) / TR) * CK_FLOATS;
+            }
+            if (lane == 31) vout_s[t] = vprev;
+        };
+        auto checkpoint = [&](const int idx) {             // state after step idx*TR - 1
+            float* ck = CKme + (long long)idx * CK_FLOATS;
 #pragma unroll
-                    for (int g = 0; g < W / 4; ++g)
-                        reinterpret_cast<float4*>(ck)[g * 32 + lane] = make_float4(h[4 * g], h[4 * g + 1], h[4 * g + 2], h[4 * g + 3]);
-                    ck[W * 32 + lane] = vprev;
+            for (int g = 0; g < W / 4; ++g)
+                reinterpret_cast<float4*>(ck)[g * 32 + lane] = make_float4(h[4 * g], h[4 * g + 1], h[4 * g + 2], h[4 * g + 3]);
+            ck[W * 32 + lane] = vprev;
+        };
+
+        unsigned seen = 0;
+        for (int c = 0; c < C; ++c) {
+            if (J > 0) {                                   // wait until the left strip has published what this chunk reads
+                const unsigned need = (unsigned)min(c + 2, C);
+                while (seen < need) { seen = ld_acquire(p.prog_f + item - 1); if (seen < need) __nanosleep(128); }
+            }
+            {
+                const int s = c * CH + lane;               // lane 0 works on row s at step s
+                vin_s[lane] = (J > 0) ? VSprev[s + 31] : ((s == 0) ? BIG : 0.f);
+                stage_x<D>(xs, p.X, pm.x_off, n, c, lane, p.sqrtk);
+            }
+            __syncwarp();
+            if (interior_chunk(c, n) && (c < c_v0 || c > c_v1)) {
+#pragma unroll 1
+                for (int b = 0; b < CH / TR; ++b) {
+#pragma unroll
+                    for (int u = 0; u < TR; ++u) step(c, b * TR + u, FastTag{});
+                    if (CKPT) checkpoint(c * (CH / TR) + b + 1);
+                }
+            } else {
+#pragma unroll 1
+                for (int t = 0; t < CH; ++t) {
+                    step(c, t, SlowTag{});
+                    if (CKPT && ((t + 1) & (TR - 1)) == 0) checkpoint((c * CH + t + 1) / TR);
                 }
             }
             __syncwarp();
             VSme[c * CH + lane] = vout_s[lane];
-            __threadfence();
-            __syncwarp();
+            __syncwarp();                                  // orders every lane's VS store before lane 0's release
             if (lane == 0) st_release(p.prog_f + item, (unsigned)(c + 1));
         }
         // value partial of this item
@@ -246,17 +295,20 @@ __global__ void __launch_bounds__(WARPS * 32) forward_kernel(const Params p) {
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// reverse: restore checkpoint, recompute TR steps (weights -> smem), E recurrence backwards, gradient contraction
+// reverse: restore checkpoint, recompute TR steps (weights -> smem), E recurrence backwards, gradient contraction.
+// The flow of E out of a cell is split with fused multiply-adds: with (wu, wl) the cell's "up" / "left" weights,
+//   into (i-1, j): E wu      into (i, j-1): E wl      into (i-1, j-1): E - E wu - E wl   (mass conserving)
 template <int D>
 __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
     extern __shared__ __align__(16) float smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float* base = smem + warp * bwd_smem_floats<D>();
-    float2* stash = reinterpret_cast<float2*>(base);            // [TR][W][32]
+    float2* stash = reinterpret_cast<float2*>(base) + lane;     // [TR][W][32] (+ lane)
     float* xs = base + TR * W * 32 * 2;
     float* vin_s = xs + 64 * D;
     float* ein_s = vin_s + 32;
     float* eout_s = ein_s + 32;
+    const float* xs_lane = xs + (32 - lane) * D;
     const int m = p.m;
     constexpr int BPC = CH / TR;
 
@@ -299,11 +351,55 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
         };
         prefetch(C * BPC - 1);
 
+        // recompute step t of the chunk (u = t - t0 within the block), keeping the transition weights
+        auto recompute = [&](const int c, const int t, const int u, auto tag) {
+            constexpr bool slow = decltype(tag)::slow;
+            float v = __shfl_up_sync(FULL, vprev, 1);
+            if (lane == 0) v = vin_s[t];
+            const int i = c * CH + t - lane;
+            if (!slow || (unsigned)i < (unsigned)n) {
+                const XRow<D> x = load_x<D>(xs_lane, t);
+#pragma unroll
+                for (int w = 0; w < W; ++w) {
+                    float tl, acc, wu, wl;
+                    sqdist2<D>(x, z[w], tl, acc);
+                    cell<true, (D > 1)>(tl, acc, h[w], v, wu, wl);
+                    stash[(u * W + w) * 32] = make_float2(wu, wl);
+                }
+                vprev = v;
+            }
+        };
+        // E recurrence for the same step, backwards (probability flow, mass conserving)
+        auto eflow = [&](const int c, const int t, const int u, auto tag) {
+            constexpr bool slow = decltype(tag)::slow;
+            float msg_in = __shfl_down_sync(FULL, msg_prev, 1);
+            if (lane == 31) msg_in = ein_s[t];
+            const int i = c * CH + t - lane;
+            if (!slow || (unsigned)i < (unsigned)n) {
+                const XRow<D> x = load_x<D>(xs_lane, t);
+                float E = A[W - 1] + msg_in;
+                float cd_right = 0.f, cl_out = 0.f;
+#pragma unroll
+                for (int w = W - 1; w >= 0; --w) {
+                    const float2 wt = stash[(u * W + w) * 32];
+#pragma unroll
+                    for (int ch = 0; ch < D; ++ch) g[w][ch] = fmaf(E, z[w][ch] - x.c[ch], g[w][ch]);
+                    const float Anew = fmaf(E, wt.x, cd_right);       // into (i-1, j): from (i, j) and, diagonally, (i, j+1)
+                    cd_right = fmaf(-E, wt.y, fmaf(-E, wt.x, E));     // diagonal share of this cell
+                    if (w > 0) E = fmaf(E, wt.y, A[w - 1]); else cl_out = E * wt.y;
+                    A[w] = Anew;
+                }
+                msg_prev = cl_out + cdf_prev;                // flow into the left neighbour's cell (i, j0-1)
+                cdf_prev = cd_right;
+            }
+            if (lane == 0) eout_s[t] = msg_prev;
+        };
+
         unsigned seen = 0;
         for (int c = C - 1; c >= 0; --c) {
             if (has_right) {                                   // right strip must have finished chunks >= max(c-1, 0)
                 const unsigned need = (unsigned)(C - max(c - 1, 0));
-                while (seen < need) { seen = ld_acquire(p.prog_b + item + 1); if (seen < need) __nanosleep(256); }
+                while (seen < need) { seen = ld_acquire(p.prog_b + item + 1); if (seen < need) __nanosleep(128); }
             }
             {
                 const int s = c * CH + lane;
@@ -312,8 +408,10 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
                 stage_x<D>(xs, p.X, pm.x_off, n, c, lane, p.sqrtk);
             }
             __syncwarp();
+            const bool fast = interior_chunk(c, n);
+#pragma unroll 1
             for (int b = BPC - 1; b >= 0; --b) {
-                const int bidx = c * BPC + b, s0 = bidx * TR, t0 = b * TR;
+                const int bidx = c * BPC + b, t0 = b * TR;
                 if (bidx == 0) {
 #pragma unroll
                     for (int w = 0; w < W; ++w) h[w] = (j0 + w == 0) ? BIG : 0.f;
@@ -324,53 +422,21 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
                     vprev = pv;
                 }
                 prefetch(bidx - 1);
-                // ---- recompute steps s0 .. s0+TR-1, keeping the transition weights
-                for (int u = 0; u < TR; ++u) {
-                    const int i = s0 + u - lane;
-                    float v = __shfl_up_sync(FULL, vprev, 1);
-                    if (lane == 0) v = vin_s[t0 + u];
-                    if ((unsigned)i < (unsigned)n) {
-                        const XRow<D> x = load_x<D>(xs, 32 + t0 + u - lane);
+                if (fast) {
 #pragma unroll
-                        for (int w = 0; w < W; ++w) {
-                            float wu, wl;
-                            cell<true>(sqdist<D>(x, z[w]), h[w], v, wu, wl);
-                            stash[(u * W + w) * 32 + lane] = make_float2(wu, wl);
-                        }
-                        vprev = v;
-                    }
-                }
-                // ---- E recurrence over the same steps, backwards (probability flow, mass conserving)
-                for (int u = TR - 1; u >= 0; --u) {
-                    const int i = s0 + u - lane;
-                    float msg_in = __shfl_down_sync(FULL, msg_prev, 1);
-                    if (lane == 31) msg_in = ein_s[t0 + u];
-                    if ((unsigned)i < (unsigned)n) {
-                        const XRow<D> x = load_x<D>(xs, 32 + t0 + u - lane);
-                        float E = A[W - 1] + msg_in;
-                        float cd_right = 0.f, cl_out = 0.f;
+                    for (int u = 0; u < TR; ++u) recompute(c, t0 + u, u, FastTag{});
 #pragma unroll
-                        for (int w = W - 1; w >= 0; --w) {
-                            const float2 wt = stash[(u * W + w) * 32 + lane];
-                            const float cu = E * wt.x, cl = E * wt.y;
-                            const float cd = (E - cu) - cl;
-#pragma unroll
-                            for (int ch = 0; ch < D; ++ch) g[w][ch] = fmaf(E, z[w][ch] - x.c[ch], g[w][ch]);
-                            const float Anew = cu + cd_right;      // flow into (i-1, j) from (i, j) and (i, j+1)
-                            cd_right = cd;
-                            if (w > 0) { E = A[w - 1] + cl; } else { cl_out = cl; }
-                            A[w] = Anew;
-                        }
-                        msg_prev = cl_out + cdf_prev;            // flow into the left neighbour's cell (i, j0-1)
-                        cdf_prev = cd_right;
-                    }
-                    if (lane == 0) eout_s[t0 + u] = msg_prev;
+                    for (int u = TR - 1; u >= 0; --u) eflow(c, t0 + u, u, FastTag{});
+                } else {
+#pragma unroll 1
+                    for (int u = 0; u < TR; ++u) recompute(c, t0 + u, u, SlowTag{});
+#pragma unroll 1
+                    for (int u = TR - 1; u >= 0; --u) eflow(c, t0 + u, u, SlowTag{});
                 }
             }
             __syncwarp();
             if (J > 0) ESme[c * CH + lane] = eout_s[lane];
-            __threadfence();
-            __syncwarp();
+            __syncwarp();                                      // orders every lane's ES store before lane 0's release
             if (lane == 0) st_release(p.prog_b + item, (unsigned)(C - c));
         }
         // eq. 6 partial of this pair for this strip's columns, back in natural units
