@@ -123,6 +123,18 @@ int sdtw_profile_read(double* ms_forward, double* ms_backward, double* ms_other,
  */
 int sdtw_measure_mufu_peak(int32_t kind, double* ops_per_s, int32_t* sm_count);
 
+/*
+ * Reverse-pass mode.  The expected-alignment matrix E of eq. 6 underflows to exactly +0 in float32 away from the
+ * alignment band, and every quantity the reverse recurrence derives from zero flows is +0 as well; by default the
+ * reverse kernel therefore SKIPS a 32-step chunk of a column strip when every flow entering it is +0.  The result is
+ * bitwise identical to visiting every cell.  sdtw_set_reverse_mode(1) disables the skip (every cell is visited: the
+ * "dense" mode used for measurement and for the bitwise-equality test); 0 restores the default.
+ * sdtw_reverse_stats() BLOCKS (device synchronise) and returns, for the last evaluation that ran a reverse pass, the
+ * number of (strip, chunk) units and how many of them were skipped.  Either pointer may be NULL.
+ */
+int sdtw_set_reverse_mode(int dense);
+int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped);
+
 /* Compile-time tile constants, for DESIGN.md / bench.py reporting: columns per thread, steps between checkpoints. */
 int sdtw_tile_info(int32_t* cols_per_thread, int32_t* strip_cols, int32_t* ckpt_steps, int32_t* chunk_steps);
 

@@ -34,6 +34,8 @@ SYMBOLS = {
     "sdtw_profile_enable": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_profile_read": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double)] * 3 + [_i64p]),
     "sdtw_tile_info": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int32)] * 4),
+    "sdtw_set_reverse_mode": (ctypes.c_int, [ctypes.c_int]),
+    "sdtw_reverse_stats": (ctypes.c_int, [ctypes.POINTER(ctypes.c_uint64)] * 2),
     "sdtw_measure_mufu_peak": (ctypes.c_int, [_i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int32)]),
 }
 for _name, (_res, _args) in SYMBOLS.items():
@@ -216,3 +218,15 @@ def sdtw_measure_mufu_peak(kind: int = 0):
     r, n = ctypes.c_double(0), ctypes.c_int32(0)
     _check(_lib.sdtw_measure_mufu_peak(int(kind), ctypes.byref(r), ctypes.byref(n)))
     return r.value, n.value
+
+
+def sdtw_set_reverse_mode(dense: bool):
+    """dense=True visits every cell in the reverse pass; False (default) skips chunks whose incoming flow is +0."""
+    _check(_lib.sdtw_set_reverse_mode(1 if dense else 0))
+
+
+def sdtw_reverse_stats():
+    """(strip-chunk units, units skipped) of the last reverse pass; synchronises the device."""
+    a, b = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    _check(_lib.sdtw_reverse_stats(ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value

@@ -21,6 +21,8 @@ uint64_t g_launches = 0;
 void* g_user_ws = nullptr;
 size_t g_user_ws_bytes = 0;
 bool g_profile = false;
+int g_dense_reverse = 0;
+const unsigned long long* g_last_stats = nullptr;   // device address of the last evaluation's reverse statistics
 
 struct ProfRec { cudaEvent_t e[4]; };
 std::vector<ProfRec> g_prof;
@@ -40,6 +42,7 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 struct Layout {
     int NS = 0;                 // strips per pair
     long long items = 0;
+    size_t off_stats = 0;
     size_t off_counters = 0, off_prog_f = 0, off_prog_b = 0, off_VP = 0, off_VS = 0, off_ES = 0, off_CK = 0, off_Gk = 0,
            off_G = 0, off_vals = 0;
     size_t sync_bytes = 0;      // counters + prog_f + prog_b: cleared before every evaluation
@@ -81,7 +84,8 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
         if (want_grad) ck_floats += pm.ck_stride * L.NS;
     }
     size_t o = 0;
-    L.off_counters = o; o += 256;
+    L.off_counters = o; o += 128;
+    L.off_stats = o;    o += 128;
     L.off_prog_f = o;   o += align_up((size_t)L.items * 4, 256);
     L.off_prog_b = o;   o += align_up((size_t)L.items * 4, 256);
     L.sync_bytes = o;
@@ -250,6 +254,9 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     P.ES = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_ES) : nullptr;
     P.CK = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_CK) : nullptr;
     P.Gk = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_Gk) : nullptr;
+    P.stats = reinterpret_cast<unsigned long long*>(ws + L.off_stats);
+    P.dense_reverse = g_dense_reverse;
+    g_last_stats = P.stats;
     P.m = (int)pl.m; P.N = pl.N; P.NS = L.NS;
     P.num_items = (unsigned)L.items;
     const double kappa = 1.0 / ((double)gamma * std::log(2.0));
@@ -321,6 +328,7 @@ struct Workspace {
             if (cache->ptr) {                       // rare: the problem grew; wait for earlier users, then regrow
                 CUDA_TRY(cudaEventSynchronize(cache->last_use));
                 CUDA_TRY(cudaFree(cache->ptr));
+                g_last_stats = nullptr;
                 cache->ptr = nullptr; cache->bytes = 0;
             }
             void* q = nullptr;
@@ -462,12 +470,14 @@ int sdtw_set_workspace(void* dev_ptr, size_t bytes) {
     if (dev_ptr && (reinterpret_cast<uintptr_t>(dev_ptr) & 255u)) return SDTW_ERR_INVALID_ARG;
     if (!dev_ptr && bytes) return SDTW_ERR_INVALID_ARG;
     g_user_ws = dev_ptr;
+    g_last_stats = nullptr;
     g_user_ws_bytes = dev_ptr ? bytes : 0;
     if (!dev_ptr) {                                 // also drop the library-owned buffer of the current device
         int dev = 0;
         if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64 && g_ws_cache[dev].ptr) {
             if (g_ws_cache[dev].last_use) cudaEventSynchronize(g_ws_cache[dev].last_use);
             cudaFree(g_ws_cache[dev].ptr);
+            g_last_stats = nullptr;
             g_ws_cache[dev].ptr = nullptr;
             g_ws_cache[dev].bytes = 0;
         }
@@ -515,6 +525,24 @@ int sdtw_profile_read(double* ms_forward, double* ms_backward, double* ms_other,
     if (ms_other) *ms_other = o;
     if (evaluations) *evaluations = (int64_t)g_prof.size();
     g_prof.clear();
+    return SDTW_OK;
+}
+
+int sdtw_set_reverse_mode(int dense) {
+    std::lock_guard<std::mutex> lock(g_mutex);
+    g_dense_reverse = dense ? 1 : 0;
+    return SDTW_OK;
+}
+
+int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped) {
+    std::lock_guard<std::mutex> lock(g_mutex);
+    unsigned long long h[2] = {0, 0};
+    if (g_last_stats) {
+        CUDA_TRY(cudaDeviceSynchronize());
+        CUDA_TRY(cudaMemcpy(h, g_last_stats, sizeof(h), cudaMemcpyDeviceToHost));
+    }
+    if (chunks) *chunks = h[0];
+    if (skipped) *skipped = h[1];
     return SDTW_OK;
 }
 

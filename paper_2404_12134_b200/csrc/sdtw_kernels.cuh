@@ -23,7 +23,7 @@
 
 namespace sdtw {
 
-constexpr int W = 8;            // columns per thread
+constexpr int W = 4;            // columns per thread
 constexpr int SW = 32 * W;      // columns per strip (work item)
 constexpr int CH = 32;          // steps per chunk (granularity of the strip-boundary exchange)
 constexpr int TR = 8;           // steps between checkpoints (= rows recomputed per reverse block)
@@ -57,6 +57,8 @@ struct Params {
     float* Gk;            // [N][m][D] per-pair gradient partials
     int m, N, NS;
     unsigned num_items;
+    unsigned long long* stats;  // [0] reverse chunks visited, [1] reverse chunks skipped (instrumentation; may be null)
+    int dense_reverse;    // 1: never skip a reverse chunk (for measurement / validation of the exact skip)
     float sqrtk;          // sqrt(1 / (gamma ln 2))
     float gscale;         // 2 / sqrtk
 };
@@ -396,17 +398,32 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
         };
 
         unsigned seen = 0;
+        int pf = C * BPC - 1;                                  // block whose checkpoint (ph, pv) currently holds
+        unsigned long long skipped = 0;
         for (int c = C - 1; c >= 0; --c) {
             if (has_right) {                                   // right strip must have finished chunks >= max(c-1, 0)
                 const unsigned need = (unsigned)(C - max(c - 1, 0));
-                while (seen < need) { seen = ld_acquire(p.prog_b + item + 1); if (seen < need) __nanosleep(128); }
+                while (seen < need) { seen = ld_acquire(p.prog_b + item + 1); if (seen < need) __nanosleep(64); }
             }
-            {
-                const int s = c * CH + lane;
-                vin_s[lane] = (J > 0) ? __ldcs(VSprev + s + 31) : ((s == 0) ? BIG : 0.f);
-                ein_s[lane] = has_right ? ESnext[s - 31] : 0.f;   // lane 31 works on row s - 31 at step s
-                stage_x<D>(xs, p.X, pm.x_off, n, c, lane, p.sqrtk);
+            const int s = c * CH + lane;
+            const float ein = has_right ? ESnext[s - 31] : 0.f;   // lane 31 works on row s - 31 at step s
+            // Exact skip: every flow that could enter this chunk's cells is +0 (E underflows to zero off the
+            // alignment band), so every product and sum below would be +0 and g would not change.
+            if (!p.dense_reverse) {
+                unsigned bits = __float_as_uint(ein) | __float_as_uint(msg_prev) | __float_as_uint(cdf_prev);
+#pragma unroll
+                for (int w = 0; w < W; ++w) bits |= __float_as_uint(A[w]);
+                if (!__any_sync(FULL, bits != 0u)) {
+                    if (J > 0) ESme[c * CH + lane] = 0.f;
+                    __syncwarp();
+                    if (lane == 0) st_release(p.prog_b + item, (unsigned)(C - c));
+                    ++skipped;
+                    continue;
+                }
             }
+            vin_s[lane] = (J > 0) ? __ldcs(VSprev + s + 31) : ((s == 0) ? BIG : 0.f);
+            ein_s[lane] = ein;
+            stage_x<D>(xs, p.X, pm.x_off, n, c, lane, p.sqrtk);
             __syncwarp();
             const bool fast = interior_chunk(c, n);
 #pragma unroll 1
@@ -417,11 +434,13 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
                     for (int w = 0; w < W; ++w) h[w] = (j0 + w == 0) ? BIG : 0.f;
                     vprev = 0.f;
                 } else {
+                    if (pf != bidx) prefetch(bidx);            // the chunk below was skipped: nothing was prefetched
 #pragma unroll
                     for (int gq = 0; gq < W / 4; ++gq) { h[4 * gq] = ph[gq].x; h[4 * gq + 1] = ph[gq].y; h[4 * gq + 2] = ph[gq].z; h[4 * gq + 3] = ph[gq].w; }
                     vprev = pv;
                 }
                 prefetch(bidx - 1);
+                pf = bidx - 1;
                 if (fast) {
 #pragma unroll
                     for (int u = 0; u < TR; ++u) recompute(c, t0 + u, u, FastTag{});
@@ -439,6 +458,7 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
             __syncwarp();                                      // orders every lane's ES store before lane 0's release
             if (lane == 0) st_release(p.prog_b + item, (unsigned)(C - c));
         }
+        if (lane == 0 && p.stats) { atomicAdd(p.stats + 0, (unsigned long long)C); atomicAdd(p.stats + 1, skipped); }
         // eq. 6 partial of this pair for this strip's columns, back in natural units
 #pragma unroll
         for (int w = 0; w < W; ++w) {

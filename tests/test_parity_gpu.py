@@ -148,6 +148,30 @@ def test_expected_alignment_mass_and_constant_inputs(B, oracle):
     assert float(G.abs().max()) <= 1e-6 and np.abs(oG).max() == 0.0
 
 
+def test_reverse_zero_skip_is_bitwise_exact(B):
+    """The reverse kernel skips chunks whose incoming E flow is +0 (include/sdtw.h: sdtw_set_reverse_mode).  The
+    result must be bit-for-bit the one obtained by visiting every cell, and the skip must actually fire on sharp
+    (small gamma) problems and never on a problem whose E is nowhere zero."""
+    import torch
+    for idx, scale, N, d_expect_skip in ((4, 0.1, 6, True), (3, 0.1, 3, True), (2, 1.0, 8, True), (1, 1.0, 8, False)):
+        cfg = synth.scaled(synth.CONFIGS[idx], scale, N=N)
+        data = synth.make(cfg)
+        Z, X = _dev(data["Z0"]), _dev(data["X"])
+        try:
+            B.sdtw_set_reverse_mode(True)
+            vd, gd = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+            chunks_d, skipped_d = B.sdtw_reverse_stats()
+            B.sdtw_set_reverse_mode(False)
+            vs, gs = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+            chunks_s, skipped_s = B.sdtw_reverse_stats()
+        finally:
+            B.sdtw_set_reverse_mode(False)
+        assert torch.equal(vd, vs) and torch.equal(gd, gs), cfg.name
+        assert skipped_d == 0 and chunks_d == chunks_s > 0
+        print(f"[{cfg.name}] reverse chunks {chunks_s}, skipped {skipped_s} ({100.0 * skipped_s / chunks_s:.1f} %)")
+        assert (skipped_s > 0) == d_expect_skip, (cfg.name, skipped_s)
+
+
 # ------------------------------------------------------------------------------------------- API behaviour
 def test_determinism_bitwise_and_workspace_registration(B):
     import torch
