@@ -272,7 +272,9 @@ def run_ours(args):
         mufu_peak = MUFU_PER_CLK_PER_SM * sms * sm_max_hz
         n_eval = max(prof["evaluations"], 1)
         t_fwd, t_bwd = prof["ms_forward"] / n_eval * 1e-3, prof["ms_backward"] / n_eval * 1e-3
-        if forward_only or t_bwd <= 0:
+        # the dominant kernel is the one with the longest measured duration (the reverse kernel skips chunks whose
+        # incoming E flow is +0, so it usually is the forward kernel)
+        if forward_only or t_bwd <= t_fwd:
             dom, t_dom, algo = "forward_kernel", t_fwd, ALGO_MUFU_FWD
         else:
             dom, t_dom, algo = "backward_kernel", t_bwd, ALGO_MUFU_BWD

@@ -17,7 +17,8 @@ __device__ __forceinline__ float mufu_step(float x) {
     float y;
     if constexpr (KIND == 0) asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(-x));          // stays in (0.5, 1]
     else if constexpr (KIND == 1) asm volatile("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x + 3.f)); // -> ~2.2
-    else asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));                                 // toggles x <-> 1/x
+    else asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x + 0.5f));                          // -> ~0.78 (a bare
+                                                                 // rcp(rcp(x)) chain is folded away by ptxas)
     return y;
 }
 
