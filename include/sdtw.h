@@ -135,8 +135,11 @@ int sdtw_measure_mufu_peak(int32_t kind, double* ops_per_s, int32_t* sm_count);
 int sdtw_set_reverse_mode(int dense);
 int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped);
 
-/* Compile-time tile constants, for DESIGN.md / bench.py reporting: columns per thread, steps between checkpoints. */
-int sdtw_tile_info(int32_t* cols_per_thread, int32_t* strip_cols, int32_t* ckpt_steps, int32_t* chunk_steps);
+/* Compile-time tile constants, for DESIGN.md / bench.py reporting: columns per thread, columns per strip (work item),
+ * wavefront steps between checkpoints, steps per strip-boundary exchange, rows a lane works on per step.  Any pointer
+ * may be NULL. */
+int sdtw_tile_info(int32_t* cols_per_thread, int32_t* strip_cols, int32_t* ckpt_steps, int32_t* chunk_steps,
+                   int32_t* rows_per_step);
 
 #ifdef __cplusplus
 }

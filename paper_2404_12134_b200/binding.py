@@ -33,7 +33,7 @@ SYMBOLS = {
     "sdtw_launch_count": (ctypes.c_uint64, []),
     "sdtw_profile_enable": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_profile_read": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double)] * 3 + [_i64p]),
-    "sdtw_tile_info": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int32)] * 4),
+    "sdtw_tile_info": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int32)] * 5),
     "sdtw_set_reverse_mode": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_reverse_stats": (ctypes.c_int, [ctypes.POINTER(ctypes.c_uint64)] * 2),
     "sdtw_measure_mufu_peak": (ctypes.c_int, [_i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int32)]),
@@ -208,9 +208,10 @@ def sdtw_profile_read():
 
 
 def sdtw_tile_info():
-    v = [ctypes.c_int32(0) for _ in range(4)]
+    v = [ctypes.c_int32(0) for _ in range(5)]
     _check(_lib.sdtw_tile_info(*[ctypes.byref(x) for x in v]))
-    return dict(cols_per_thread=v[0].value, strip_cols=v[1].value, ckpt_steps=v[2].value, chunk_steps=v[3].value)
+    return dict(cols_per_thread=v[0].value, strip_cols=v[1].value, ckpt_steps=v[2].value, chunk_steps=v[3].value,
+                rows_per_step=v[4].value)
 
 
 def sdtw_measure_mufu_peak(kind: int = 0):

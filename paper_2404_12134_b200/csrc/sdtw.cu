@@ -24,7 +24,7 @@ bool g_profile = false;
 int g_dense_reverse = 0;
 const unsigned long long* g_last_stats = nullptr;   // device address of the last evaluation's reverse statistics
 
-struct ProfRec { cudaEvent_t e[4]; };
+struct ProfRec { cudaEvent_t e[5]; };   // start | prologue | forward | reverse | small kernels
 std::vector<ProfRec> g_prof;
 
 #define CUDA_TRY(expr)                                   \
@@ -43,9 +43,10 @@ struct Layout {
     int NS = 0;                 // strips per pair
     long long items = 0;
     size_t off_stats = 0;
-    size_t off_counters = 0, off_prog_f = 0, off_prog_b = 0, off_VP = 0, off_VS = 0, off_ES = 0, off_CK = 0, off_Gk = 0,
-           off_G = 0, off_vals = 0;
-    size_t sync_bytes = 0;      // counters + prog_f + prog_b: cleared before every evaluation
+    size_t off_counters = 0, off_prog_b = 0, off_VP = 0, off_Xs = 0, off_Zs = 0, off_VS = 0, off_ES = 0, off_CK = 0,
+           off_Gk = 0;
+    size_t sync_bytes = 0;      // counters + stats + prog_b: cleared before every evaluation
+    size_t vs_bytes = 0;        // VS: preset to the sentinel pattern before every evaluation
     size_t total = 0;
     std::vector<PairMeta> pm;   // schedule order
 };
@@ -75,8 +76,8 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
         pm.k = k;
         pm.x_off = offsets[k];
         pm.n = (int)(offsets[k + 1] - offsets[k]);
-        pm.C = (pm.n + 31 + CH - 1) / CH;
-        pm.vs_stride = pm.C * CH + 64;
+        pm.C = ((pm.n + RP - 1) / RP + 31 + CH - 1) / CH;
+        pm.vs_stride = VS_PAD + pm.C * CROWS;
         pm.vs_off = vs_floats;
         vs_floats += (long long)pm.vs_stride * L.NS;
         pm.ck_stride = (long long)(pm.C * (CH / TR) + 1) * CK_FLOATS;
@@ -86,17 +87,17 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
     size_t o = 0;
     L.off_counters = o; o += 128;
     L.off_stats = o;    o += 128;
-    L.off_prog_f = o;   o += align_up((size_t)L.items * 4, 256);
     L.off_prog_b = o;   o += align_up((size_t)L.items * 4, 256);
     L.sync_bytes = o;
     L.off_VP = o;       o += align_up((size_t)L.items * 8, 256);
-    L.off_vals = o;     o += align_up((size_t)N * 4, 256);
-    L.off_VS = o;       o += align_up((size_t)vs_floats * 4, 256);
+    L.off_Xs = o;       o += align_up((size_t)offsets[N] * (size_t)d * 4, 256);
+    L.off_Zs = o;       o += align_up((size_t)m * (size_t)d * 4, 256);
+    L.vs_bytes = align_up((size_t)vs_floats * 4, 256);
+    L.off_VS = o;       o += L.vs_bytes;
     if (want_grad) {
-        L.off_ES = o;   o += align_up((size_t)vs_floats * 4, 256);
+        L.off_ES = o;   o += L.vs_bytes;
         L.off_CK = o;   o += align_up((size_t)ck_floats * 4, 256);
         L.off_Gk = o;   o += align_up((size_t)N * (size_t)m * (size_t)d * 4, 256);
-        L.off_G = o;    o += align_up((size_t)m * (size_t)d * 4, 256);
     }
     L.total = o;
     return SDTW_OK;
@@ -189,22 +190,28 @@ int persistent_grid(K kernel, int smem_bytes, int sms, long long items, int* gri
     return SDTW_OK;
 }
 
-template <int D>
-int launch_forward(const Params& P, bool ckpt, int sms, cudaStream_t stream) {
-    const int smem = WARPS * fwd_smem_floats<D>() * 4;
-    int grid = 1, rc;
-    if (ckpt) {
-        rc = persistent_grid(forward_kernel<D, true>, smem, sms, P.num_items, &grid);
-        if (rc) return rc;
-        forward_kernel<D, true><<<grid, WARPS * 32, smem, stream>>>(P);
-    } else {
-        rc = persistent_grid(forward_kernel<D, false>, smem, sms, P.num_items, &grid);
-        if (rc) return rc;
-        forward_kernel<D, false><<<grid, WARPS * 32, smem, stream>>>(P);
-    }
+template <int D> constexpr int fwd_warps() { return D <= 2 ? 32 : 16; }   // warps per CTA = strips per unit
+
+template <int D, bool CKPT>
+int launch_forward_t(const Params& P, int sms, cudaStream_t stream) {
+    constexpr int FW = fwd_warps<D>();
+    const int smem = FW * fwd_smem_floats<D>() * 4;
+    auto kernel = forward_kernel<D, CKPT, FW>;
+    CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    int occ = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, FW * 32, smem));
+    if (occ < 1) return SDTW_ERR_UNSUPPORTED;
+    const long long units = (long long)((P.NS + FW - 1) / FW) * P.N;
+    const int grid = (int)std::max(1LL, std::min(units, (long long)sms * occ));
+    kernel<<<grid, FW * 32, smem, stream>>>(P);
     ++g_launches;
     CUDA_TRY(cudaGetLastError());
     return SDTW_OK;
+}
+
+template <int D>
+int launch_forward(const Params& P, bool ckpt, int sms, cudaStream_t stream) {
+    return ckpt ? launch_forward_t<D, true>(P, sms, stream) : launch_forward_t<D, false>(P, sms, stream);
 }
 
 template <int D>
@@ -245,9 +252,10 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
              float* out_values, float* out_objective, float* out_grad, float* Z_update, float step, cudaStream_t stream) {
     const Layout& L = pl.L;
     Params P{};
-    P.Z = Z; P.X = X; P.pm = pl.d_pm;
+    float* Xs = reinterpret_cast<float*>(ws + L.off_Xs);
+    float* Zs = reinterpret_cast<float*>(ws + L.off_Zs);
+    P.Zs = Zs; P.Xs = Xs; P.pm = pl.d_pm;
     P.counters = reinterpret_cast<unsigned*>(ws + L.off_counters);
-    P.prog_f = reinterpret_cast<unsigned*>(ws + L.off_prog_f);
     P.prog_b = reinterpret_cast<unsigned*>(ws + L.off_prog_b);
     P.VP = reinterpret_cast<double*>(ws + L.off_VP);
     P.VS = reinterpret_cast<float*>(ws + L.off_VS);
@@ -260,23 +268,33 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     P.m = (int)pl.m; P.N = pl.N; P.NS = L.NS;
     P.num_items = (unsigned)L.items;
     const double kappa = 1.0 / ((double)gamma * std::log(2.0));
-    P.sqrtk = (float)std::sqrt(kappa);
-    P.gscale = (float)(2.0 / (double)P.sqrtk);
+    const float sqrtk = (float)std::sqrt(kappa);
+    P.gscale = (float)(2.0 / (double)sqrtk);
     // the kernels see gamma only through the rounded sqrtk; undo exactly that scale on the way out
-    const double inv_kappa = 1.0 / ((double)P.sqrtk * (double)P.sqrtk);
+    const double inv_kappa = 1.0 / ((double)sqrtk * (double)sqrtk);
 
     ProfRec pr{};
     if (g_profile) for (auto& e : pr.e) CUDA_TRY(cudaEventCreate(&e));
-    CUDA_TRY(cudaMemsetAsync(ws + L.off_counters, 0, L.sync_bytes, stream));
     if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[0], stream));
+    CUDA_TRY(cudaMemsetAsync(ws + L.off_counters, 0, L.sync_bytes, stream));
+    // every word of the strip-boundary columns starts as the sentinel the consumers poll for (sdtw_kernels.cuh)
+    CUDA_TRY(cudaMemsetAsync(ws + L.off_VS, 0xFF, L.vs_bytes, stream));
+    {
+        const long long nx = (long long)pl.offsets[pl.N] * pl.d, nz = (long long)pl.m * pl.d;
+        const int blocks = (int)std::min<long long>((nx + nz + 255) / 256, (long long)di.sms * 8);
+        scale_inputs_kernel<<<blocks, 256, 0, stream>>>(X, nx, Z, nz, sqrtk, Xs, Zs);
+        ++g_launches;
+        CUDA_TRY(cudaGetLastError());
+    }
+    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[1], stream));
     int rc = dispatch_forward(pl.d, P, pl.want_grad, di.sms, stream);
     if (rc) return rc;
-    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[1], stream));
+    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[2], stream));
     if (pl.want_grad) {
         rc = dispatch_backward(pl.d, P, di.sms, stream);
         if (rc) return rc;
     }
-    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[2], stream));
+    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[3], stream));
     if (out_values || out_objective) {
         finalize_values_kernel<<<1, 256, 0, stream>>>(P.VP, pl.d_pm, pl.N, L.NS, inv_kappa, out_values, out_objective);
         ++g_launches;
@@ -290,7 +308,7 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
         CUDA_TRY(cudaGetLastError());
     }
     if (g_profile) {
-        CUDA_TRY(cudaEventRecord(pr.e[3], stream));
+        CUDA_TRY(cudaEventRecord(pr.e[4], stream));
         g_prof.push_back(pr);
     }
     return SDTW_OK;
@@ -513,11 +531,12 @@ int sdtw_profile_read(double* ms_forward, double* ms_backward, double* ms_other,
     std::lock_guard<std::mutex> lock(g_mutex);
     double f = 0, b = 0, o = 0;
     for (auto& pr : g_prof) {
-        CUDA_TRY(cudaEventSynchronize(pr.e[3]));
+        CUDA_TRY(cudaEventSynchronize(pr.e[4]));
         float t = 0;
-        CUDA_TRY(cudaEventElapsedTime(&t, pr.e[0], pr.e[1])); f += t;
-        CUDA_TRY(cudaEventElapsedTime(&t, pr.e[1], pr.e[2])); b += t;
-        CUDA_TRY(cudaEventElapsedTime(&t, pr.e[2], pr.e[3])); o += t;
+        CUDA_TRY(cudaEventElapsedTime(&t, pr.e[1], pr.e[2])); f += t;
+        CUDA_TRY(cudaEventElapsedTime(&t, pr.e[2], pr.e[3])); b += t;
+        CUDA_TRY(cudaEventElapsedTime(&t, pr.e[0], pr.e[1])); o += t;   // prologue: clears, sentinel preset, input scaling
+        CUDA_TRY(cudaEventElapsedTime(&t, pr.e[3], pr.e[4])); o += t;   // values, reduction over pairs, descent step
         for (auto& e : pr.e) cudaEventDestroy(e);
     }
     if (ms_forward) *ms_forward = f;
@@ -546,7 +565,9 @@ int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped) {
     return SDTW_OK;
 }
 
-int sdtw_tile_info(int32_t* cols_per_thread, int32_t* strip_cols, int32_t* ckpt_steps, int32_t* chunk_steps) {
+int sdtw_tile_info(int32_t* cols_per_thread, int32_t* strip_cols, int32_t* ckpt_steps, int32_t* chunk_steps,
+                   int32_t* rows_per_step) {
+    if (rows_per_step) *rows_per_step = RP;
     if (cols_per_thread) *cols_per_thread = W;
     if (strip_cols) *strip_cols = SW;
     if (ckpt_steps) *ckpt_steps = TR;

@@ -11,26 +11,60 @@
 //   and E is pushed backwards as a probability flow:  E[pred] += E[cell] * w_pred  (mass conserving in fp32).
 //
 // Work decomposition: a WORK ITEM is one column strip (32 lanes x W columns) of one pair, swept over all rows by ONE
-// warp.  Lane l works on row (step - l): the anti-diagonal wavefront.  Neighbouring lanes exchange one value per step
-// by warp shuffle; neighbouring strips exchange the strip-boundary column through global memory (VS forward, ES
-// reverse) with a release/acquire progress counter per item.  Every TR steps the forward kernel checkpoints the warp
-// state (h[W] + the value in flight) to HBM; the reverse kernel restores a checkpoint, recomputes TR steps keeping the
-// transition weights in shared memory, then runs the E recurrence over those TR steps backwards, accumulating the
-// gradient contraction of eq. 6 in registers.
+// warp.  At step s lane l works on the RP = 2 rows 2(s - l), 2(s - l) + 1 of its W columns: a skewed anti-diagonal
+// wavefront whose 2 x W register tile gives every thread two independent dependency chains (the cells (A, w+1) and
+// (A+1, w) do not depend on each other), which is what keeps the MUFU pipe fed.  Neighbouring lanes exchange two values
+// per step by warp shuffle; neighbouring strips exchange the strip-boundary column through global memory:
+//   forward  VS[row]: written by lane 31 of the left strip, read by lane 0 of the right strip.  No flag: the buffer is
+//            preset to a sentinel bit pattern no arithmetic result can have and the consumer polls the DATA words with
+//            relaxed gpu-scope loads, one 64-row chunk ahead of use, so the wait is normally hidden;
+//   reverse  ES[row]: E messages from the right strip to the left one, ordered by a release/acquire progress counter.
+// Every TR steps the forward kernel checkpoints the warp state (h[W] + the two values in flight) to HBM; the reverse
+// kernel restores a checkpoint, recomputes TR steps keeping the transition weights in shared memory, then runs the E
+// recurrence over those TR steps backwards, accumulating the gradient contraction of eq. 6 in registers.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace sdtw {
 
-constexpr int W = 4;            // columns per thread
+#ifndef SDTW_W
+#define SDTW_W 4
+#endif
+#ifndef SDTW_TR
+#define SDTW_TR 8
+#endif
+#ifndef SDTW_WARPS
+#define SDTW_WARPS 4
+#endif
+#ifndef SDTW_CH
+#define SDTW_CH 32
+#endif
+#ifndef SDTW_SLACK
+#define SDTW_SLACK 2
+#endif
+
+constexpr int W = SDTW_W;       // columns per thread
+constexpr int RP = 2;           // rows per lane per step
 constexpr int SW = 32 * W;      // columns per strip (work item)
-constexpr int CH = 32;          // steps per chunk (granularity of the strip-boundary exchange)
-constexpr int TR = 8;           // steps between checkpoints (= rows recomputed per reverse block)
-constexpr int WARPS = 4;        // warps per CTA (each warp is an independent agent)
-constexpr int CK_FLOATS = 32 * (W + 1);  // floats per checkpoint record
+constexpr int CH = SDTW_CH;     // steps per chunk (granularity of the strip-boundary exchange), <= 32
+constexpr int CROWS = CH * RP;  // rows a lane sweeps per chunk
+constexpr int SKEW = 31 * RP;   // lane 31 is this many rows behind lane 0
+constexpr int XPAD = 64;        // >= SKEW, keeps the staged window aligned
+constexpr int XWIN = XPAD + CROWS;  // rows of the cycle staged per chunk: [c*CROWS - XPAD, c*CROWS + CROWS)
+constexpr int SLACK = SDTW_SLACK;   // chunks a forward consumer lets its producer get ahead once it has caught up
+constexpr int LAGC = (SKEW + CROWS - 1) / CROWS;  // chunks of the neighbouring strip one chunk reaches back into
+constexpr int TR = SDTW_TR;     // steps between checkpoints (= steps recomputed per reverse block)
+constexpr int WARPS = SDTW_WARPS;  // warps per CTA (each warp is an independent agent)
+constexpr int CK_FLOATS = 32 * (W + RP);  // floats per checkpoint record
+constexpr int VS_PAD = 64;      // floats of front padding of every VS / ES strip (rows -62 .. -1 are addressed)
 constexpr float BIG = 1.0e30f;  // stands for the +inf border of eq. 5
 constexpr unsigned FULL = 0xffffffffu;
+constexpr unsigned SENTINEL = 0xffffffffu;  // a NaN pattern no arithmetic instruction returns (results are 0x7fffffff)
+
+static_assert(W % 4 == 0, "checkpoints store h as float4");
+static_assert(CH % TR == 0 && CH <= 32, "a chunk holds a whole number of checkpoint blocks; one lane per step");
+static_assert(VS_PAD >= SKEW && XPAD >= SKEW && (XWIN * 1) % 32 == 0, "padding covers the lane skew");
 
 struct PairMeta {   // one per pair, in schedule order (longest first)
     long long x_off;      // first row of this cycle in X_concat
@@ -40,18 +74,17 @@ struct PairMeta {   // one per pair, in schedule order (longest first)
     int vs_stride;
     int n;                // rows of this cycle
     int k;                // caller's pair index
-    int C;                // chunks = ceil((n + 31) / CH)
+    int C;                // chunks = ceil((ceil(n / RP) + 31) / CH)
 };
 
 struct Params {
-    const float* Z;
-    const float* X;
+    const float* Zs;      // sqrt(kappa) * Z
+    const float* Xs;      // sqrt(kappa) * X_concat
     const PairMeta* pm;
     unsigned* counters;   // [0] forward work queue, [1] reverse work queue
-    unsigned* prog_f;     // [N * NS] chunks completed by each forward item
     unsigned* prog_b;     // [N * NS] chunks completed by each reverse item
-    float* VS;            // strip-boundary v columns, indexed by producer step
-    float* ES;            // strip-boundary E messages, indexed by row (32 floats of front padding per strip)
+    float* VS;            // strip-boundary v columns, indexed by row
+    float* ES;            // strip-boundary E messages, indexed by row
     float* CK;            // checkpoints
     double* VP;           // [N * NS] per-item partial of the value (staircase sum), scaled units
     float* Gk;            // [N][m][D] per-pair gradient partials
@@ -59,8 +92,7 @@ struct Params {
     unsigned num_items;
     unsigned long long* stats;  // [0] reverse chunks visited, [1] reverse chunks skipped (instrumentation; may be null)
     int dense_reverse;    // 1: never skip a reverse chunk (for measurement / validation of the exact skip)
-    float sqrtk;          // sqrt(1 / (gamma ln 2))
-    float gscale;         // 2 / sqrtk
+    float gscale;         // 2 / sqrt(kappa)
 };
 
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
@@ -72,47 +104,70 @@ __device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
 __device__ __forceinline__ void st_release(unsigned* p, unsigned v) {
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
+// relaxed gpu-scope accesses of the forward strip-boundary column (each 32-bit word is valid or the sentinel)
+__device__ __forceinline__ float2 ld_relaxed_f2(const float* p) {
+    float2 v; asm volatile("ld.relaxed.gpu.global.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p) : "memory"); return v;
+}
+__device__ __forceinline__ void st_relaxed_f2(float* p, float2 v) {
+    asm volatile("st.relaxed.gpu.global.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.x), "f"(v.y) : "memory");
+}
+__device__ __forceinline__ bool is_sentinel(float x) { return __float_as_uint(x) == SENTINEL; }
+
+template <int BYTES>
+__device__ __forceinline__ void cp_async(float* smem_dst, const float* gsrc, bool ok) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    const int sz = ok ? BYTES : 0;                           // src-size 0: the destination is zero-filled
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2, %3;" ::"r"(s), "l"(gsrc), "n"(BYTES), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // shared memory per warp (floats)
-template <int D> __host__ __device__ constexpr int fwd_smem_floats() { return 64 * D + 64; }
-template <int D> __host__ __device__ constexpr int bwd_smem_floats() { return TR * W * 32 * 2 + 64 * D + 96; }
+template <int D> __host__ __device__ constexpr int fwd_smem_floats() { return 2 * XWIN * D + 4 * 32; }
+template <int D> __host__ __device__ constexpr int bwd_smem_floats() { return TR * RP * W * 32 * 2 + XWIN * D + 6 * 32; }
 
 template <int D> struct XRow { float c[D]; };
 
+// rows e and e + 1 (e even) of a staged window
 template <int D>
-__device__ __forceinline__ XRow<D> load_x(const float* xs, int e) {
-    XRow<D> r;
-    if constexpr (D == 4) {
-        float4 t = *reinterpret_cast<const float4*>(xs + e * 4);
-        r.c[0] = t.x; r.c[1] = t.y; r.c[2] = t.z; r.c[3] = t.w;
+__device__ __forceinline__ void load_x2(const float* xs, int e, XRow<D>& a, XRow<D>& b) {
+    if constexpr (D == 1) {
+        const float2 t = *reinterpret_cast<const float2*>(xs + e);
+        a.c[0] = t.x; b.c[0] = t.y;
     } else if constexpr (D == 2) {
-        float2 t = *reinterpret_cast<const float2*>(xs + e * 2);
-        r.c[0] = t.x; r.c[1] = t.y;
+        const float4 t = *reinterpret_cast<const float4*>(xs + e * 2);
+        a.c[0] = t.x; a.c[1] = t.y; b.c[0] = t.z; b.c[1] = t.w;
+    } else if constexpr (D == 4) {
+        const float4 t = *reinterpret_cast<const float4*>(xs + e * 4);
+        const float4 u = *reinterpret_cast<const float4*>(xs + e * 4 + 4);
+        a.c[0] = t.x; a.c[1] = t.y; a.c[2] = t.z; a.c[3] = t.w;
+        b.c[0] = u.x; b.c[1] = u.y; b.c[2] = u.z; b.c[3] = u.w;
     } else {
 #pragma unroll
-        for (int c = 0; c < D; ++c) r.c[c] = xs[e * D + c];
+        for (int c = 0; c < D; ++c) { a.c[c] = xs[e * D + c]; b.c[c] = xs[(e + 1) * D + c]; }
     }
-    return r;
 }
 
-// stage rows [c*CH - 32, c*CH + 32) of the (scaled) cycle into xs[64][D]; rows outside [0, n) read as 0
+// asynchronously stage rows [c*CROWS - XPAD, c*CROWS + CROWS) of the scaled cycle into xs[XWIN][D]; rows outside
+// [0, n) read as 0.  Completed by cp_async_wait_all() + __syncwarp().
 template <int D>
-__device__ __forceinline__ void stage_x(float* xs, const float* __restrict__ X, long long x_off, int n, int c, int lane,
-                                        float sqrtk) {
+__device__ __forceinline__ void stage_x_async(float* xs, const float* __restrict__ Xs, long long x_off, int n, int c, int lane) {
+    constexpr int VE = (D % 4 == 0) ? 4 : (D % 2 == 0) ? 2 : 1;       // floats per copy (a copy never straddles a row)
+    constexpr int PER_LANE = XWIN * D / VE / 32;
+    static_assert(XWIN * D % (VE * 32) == 0, "whole copies per lane");
+    const int wb = c * CROWS - XPAD;
 #pragma unroll
-    for (int half = 0; half < 2; ++half) {
-        const int e = lane + 32 * half;
-        const int r = c * CH - 32 + e;
+    for (int q = 0; q < PER_LANE; ++q) {
+        const int f = (lane + 32 * q) * VE;                           // float index in the window
+        const int r = wb + f / D;
         const bool ok = (unsigned)r < (unsigned)n;
-#pragma unroll
-        for (int ch = 0; ch < D; ++ch) xs[e * D + ch] = ok ? __ldg(X + (x_off + r) * D + ch) * sqrtk : 0.f;
+        const float* src = ok ? Xs + (x_off + wb) * D + f : Xs;
+        cp_async<VE * 4>(xs + f, src, ok);
     }
 }
 
 // ------------------------------------------------------------------------------------------------------------------
 // one cell of the difference-form recurrence.  v is v_in on entry and v_out on return; h is h_in / h_out.
-// t2 is the SQUARED cost input: the cell cost is D = sum_c t_c^2, passed as (t_last, acc) with D = t_last^2 + acc so
-// that the last square fuses with the subtraction of the log (one FFMA).
+// The cell cost is D = t_last^2 + acc, so that the last square fuses with the subtraction of the log (one FFMA).
 // With a = mn - h_in, b = mn - v_in (mn = min(0, h_in, v_in); one of 0, a, b is exactly 0) the three soft-min terms are
 // 2^mn (diagonal), 2^a ("up"), 2^b ("left"); sorted, they are 1, e1 = 2^-|min(h,v)| and e2 = 2^min(a,b).
 // STASH: also emit the weights (w_up, w_left) of this cell's "up" and "left" predecessors.
@@ -163,36 +218,92 @@ __device__ __forceinline__ float sqdist(const XRow<D>& x, const float (&z)[D]) {
 struct FastTag { static constexpr bool slow = false; };
 struct SlowTag { static constexpr bool slow = true; };
 
-// chunk c (steps 32c .. 32c+31, rows 32c-31 .. 32c+31 over the 32 lanes) touches only valid rows
-__device__ __forceinline__ bool interior_chunk(int c, int n) { return c >= 1 && c * CH + CH <= n; }
+// chunk c (steps c CH .. c CH + CH-1, rows c CROWS - SKEW .. c CROWS + CROWS-1 over the 32 lanes) touches only valid rows
+__device__ __forceinline__ bool interior_chunk(int c, int n) { return c * CROWS >= SKEW && c * CROWS + CROWS <= n; }
+
+// ------------------------------------------------------------------------------------------------------------------
+// prologue: the scaled copies of the inputs the two wavefront kernels read
+__global__ void scale_inputs_kernel(const float* __restrict__ X, long long nx, const float* __restrict__ Z, long long nz,
+                                    float s, float* __restrict__ Xs, float* __restrict__ Zs) {
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < nx + nz; e += stride) {
+        if (e < nx) Xs[e] = X[e] * s; else Zs[e - nx] = Z[e - nx] * s;
+    }
+}
 
 // ------------------------------------------------------------------------------------------------------------------
 // forward: eq. 5 in difference form, value by a staircase sum, strip-boundary column to VS, checkpoints to CK.
 // Chunks whose 32 x 32 (step, lane) block lies inside the matrix and off this warp's value staircase run the FAST
-// step (no bounds or staircase tests, 8 steps unrolled between checkpoints); the others run the general step.  Both
-// evaluate every cell with the same expressions.
-template <int D, bool CKPT>
-__global__ void __launch_bounds__(WARPS * 32) forward_kernel(const Params p) {
-    extern __shared__ __align__(16) float smem[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float* xs = smem + warp * fwd_smem_floats<D>();
-    float* vin_s = xs + 64 * D;
-    float* vout_s = vin_s + 32;
-    const float* xs_lane = xs + (32 - lane) * D;           // row (c*CH + t - lane) of the staged window is xs_lane[t*D ..]
-    const int m = p.m;
+// step (no bounds or staircase tests, TR steps unrolled between checkpoints, the two rows of a step interleaved); the
+// others run the general step.  Both evaluate every cell with the same expressions.
+//
+// Schedule: a UNIT is FW adjacent strips of one pair (unit u = g N + ps: group-major, so group g+1 of a pair is taken
+// long after its group g).  A CTA of FW warps pops units from a global counter and its warps serve a rolling stream of
+// strips: strip s of the CTA's k-th unit goes to the warp whose position is (base_k + s) mod FW, base_k = strips of the
+// earlier units.  So a strip and the strip it waits on run on the SAME SM (8 consecutive ones on the same scheduler): a
+// warp that has caught up with its producer stops competing with it for the MUFU pipe, which is what balances the
+// chain; chains that span SMs leave every SM partly idle.
+constexpr int UNIT_RING = 8;
+struct RollCtl { int popped; int lock; int uid[UNIT_RING]; int seen[32]; };
 
-    for (;;) {
-        unsigned q = 0;
-        if (lane == 0) q = atomicAdd(p.counters + 0, 1u);
-        q = __shfl_sync(FULL, q, 0);
-        if (q >= p.num_items) break;
-        const int J = q / p.N, ps = q - J * p.N;          // strip-major order: all pairs' strip 0 first
+template <int D, bool CKPT, int FW>
+__global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params p) {
+    extern __shared__ __align__(16) float smem[];
+    __shared__ RollCtl ctl;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float* xs0 = smem + warp * fwd_smem_floats<D>();                 // [2][XWIN][D]
+    float2* vin_s = reinterpret_cast<float2*>(xs0 + 2 * XWIN * D);   // [CH] (v_in of lane 0 for the step's two rows)
+    float2* vout_s = vin_s + 32;                                     // [CH] (v_out of lane 31)
+    const int m = p.m;
+    const int NG = (p.NS + FW - 1) / FW, NU = NG * p.N;              // groups per pair, units
+    // position of this warp in the rolling stream: consecutive positions share a scheduler (warp id mod 4)
+    const int mypos = (warp & 3) * (FW / 4) + (warp >> 2);
+    if (threadIdx.x < 32) { ctl.seen[threadIdx.x] = 0; if (threadIdx.x == 0) { ctl.popped = 0; ctl.lock = 0; } }
+    __syncthreads();
+
+    int base = 0;                                          // strips of the units before unit k, mod FW
+    for (int k = 0;; ++k) {
+        int u = 0;
+        if (lane == 0) {                                   // the CTA's k-th unit: popped by whichever warp needs it first
+            volatile RollCtl* vc = &ctl;
+            while (vc->popped <= k) {
+                if (atomicCAS(&ctl.lock, 0, 1) == 0) {
+                    const int pc = vc->popped;
+                    if (pc <= k) {
+                        for (;;) {                         // ring slot free: every warp has read unit pc - UNIT_RING
+                            int mn = vc->seen[0];
+                            for (int w2 = 1; w2 < FW; ++w2) mn = min(mn, vc->seen[w2]);
+                            if (mn > pc - UNIT_RING) break;
+                            __nanosleep(100);
+                        }
+                        vc->uid[pc % UNIT_RING] = (int)min(atomicAdd(p.counters + 0, 1u), (unsigned)NU);
+                        __threadfence_block();
+                        vc->popped = pc + 1;
+                    }
+                    __threadfence_block();
+                    atomicExch(&ctl.lock, 0);
+                } else {
+                    __nanosleep(50);
+                }
+            }
+            __threadfence_block();
+            u = vc->uid[k % UNIT_RING];
+            vc->seen[warp] = k + 1;
+        }
+        u = __shfl_sync(FULL, u, 0);
+        if (u >= NU) break;
+        const int g = u / p.N, ps = u - g * p.N;
+        const int S = min(FW, p.NS - g * FW);              // strips of this unit
+        const int sidx = (mypos - base + FW) % FW;
+        base = (base + S) % FW;
+        if (sidx >= S) continue;
+        const int J = g * FW + sidx;
         const PairMeta pm = p.pm[ps];
         const int n = pm.n, C = pm.C;
         const int item = ps * p.NS + J;
         const int T = J * 32 + lane;                       // global thread (column group) index
         const int j0 = T * W;
-        float* VSme = p.VS + pm.vs_off + (long long)J * pm.vs_stride;
+        float* VSme = p.VS + pm.vs_off + (long long)J * pm.vs_stride + VS_PAD;      // indexed by row
         const float* VSprev = VSme - pm.vs_stride;
         float* CKme = p.CK + pm.ck_off + (long long)J * pm.ck_stride;
 
@@ -201,10 +312,10 @@ __global__ void __launch_bounds__(WARPS * 32) forward_kernel(const Params p) {
         for (int w = 0; w < W; ++w) {
             const int j = j0 + w;
 #pragma unroll
-            for (int c = 0; c < D; ++c) z[w][c] = (j < m) ? __ldg(p.Z + (long long)j * D + c) * p.sqrtk : 0.f;
+            for (int c = 0; c < D; ++c) z[w][c] = (j < m) ? __ldg(p.Zs + (long long)j * D + c) : 0.f;
             h[w] = (j == 0) ? BIG : 0.f;                   // virtual row 0: r_00 = 0, r_0j = inf
         }
-        float vprev = 0.f;
+        float vp0 = 0.f, vp1 = 0.f;                        // v_out of this lane's last column, rows 2(s-l) and 2(s-l)+1
 
         // staircase for the value: r_{n,m} = sum of h along row r_h (columns jlo..jhi) + sum of v down one column
         // (rows r_v0+1 .. r_v1) over all threads; see DESIGN.md section 5.4
@@ -218,57 +329,104 @@ __global__ void __launch_bounds__(WARPS * 32) forward_kernel(const Params p) {
             r_h = rho_prev; jlo = max(1, j0); jhi = j0 + W - 1; r_v0 = rho_prev; r_v1 = rho_cur;
         } else { r_h = n - 1; jlo = j0; jhi = m - 1; r_v0 = r_v1 = n - 1; }
         float vacc = 0.f, hsum = 0.f;
-        // chunks that hold a staircase row of some lane of this warp (row i of lane l is visited at step i + l)
-        const int c_v0 = __reduce_min_sync(FULL, min(r_h, r_v0)) / CH;
-        const int c_v1 = (__reduce_max_sync(FULL, max(r_h, r_v1)) + 31) / CH;
+        // chunks that hold a staircase row of some lane of this warp (row i of lane l is visited at step i/2 + l)
+        const int c_v0 = (__reduce_min_sync(FULL, min(r_h, r_v0)) / RP) / CH;
+        const int c_v1 = (__reduce_max_sync(FULL, max(r_h, r_v1)) / RP + 31) / CH;
 
+        const float* xs_lane = xs0;                        // set per chunk
+        // general row: all W cells of row i, plus this thread's piece of the value staircase
+        auto slow_row = [&](const int i, const XRow<D>& x, float& v) {
+            float vfirst = 0.f, dummy0, dummy1;
+#pragma unroll
+            for (int w = 0; w < W; ++w) {
+                float tl, acc;
+                sqdist2<D>(x, z[w], tl, acc);
+                cell<false, (D > 1)>(tl, acc, h[w], v, dummy0, dummy1);
+                if (w == 0) vfirst = v;
+            }
+            if ((unsigned)(i - r_v0 - 1) < (unsigned)(r_v1 - r_v0)) vacc += vfirst_sel ? vfirst : v;
+            if (i == r_h) {
+#pragma unroll
+                for (int w = 0; w < W; ++w) if (j0 + w >= jlo && j0 + w <= jhi) hsum += h[w];
+            }
+            if (T == 0 && i == 0) hsum += sqdist<D>(x, z[0]);   // r_11 = D_11
+        };
         auto step = [&](const int c, const int t, auto tag) {
             constexpr bool slow = decltype(tag)::slow;
-            float v = __shfl_up_sync(FULL, vprev, 1);
-            if (lane == 0) v = vin_s[t];
-            const int i = c * CH + t - lane;
-            if (!slow || (unsigned)i < (unsigned)n) {
-                const XRow<D> x = load_x<D>(xs_lane, t);
-                float vfirst = 0.f, dummy0, dummy1;
+            float va = __shfl_up_sync(FULL, vp0, 1), vb = __shfl_up_sync(FULL, vp1, 1);
+            if (lane == 0) { const float2 qv = vin_s[t]; va = qv.x; vb = qv.y; }
+            XRow<D> xa, xb;
+            load_x2<D>(xs_lane, 2 * t, xa, xb);
+            if constexpr (!slow) {
+                float dummy0, dummy1;
 #pragma unroll
-                for (int w = 0; w < W; ++w) {
+                for (int w = 0; w < W; ++w) {              // cell (A, w+1) and cell (A+1, w) are independent
                     float tl, acc;
-                    sqdist2<D>(x, z[w], tl, acc);
-                    cell<false, (D > 1)>(tl, acc, h[w], v, dummy0, dummy1);
-                    if (slow && w == 0) vfirst = v;
+                    sqdist2<D>(xa, z[w], tl, acc);
+                    cell<false, (D > 1)>(tl, acc, h[w], va, dummy0, dummy1);
+                    sqdist2<D>(xb, z[w], tl, acc);
+                    cell<false, (D > 1)>(tl, acc, h[w], vb, dummy0, dummy1);
                 }
-                vprev = v;
-                if constexpr (slow) {
-                    if ((unsigned)(i - r_v0 - 1) < (unsigned)(r_v1 - r_v0)) vacc += vfirst_sel ? vfirst : v;
-                    if (i == r_h) {
-#pragma unroll
-                        for (int w = 0; w < W; ++w) if (j0 + w >= jlo && j0 + w <= jhi) hsum += h[w];
-                    }
-                    if (T == 0 && i == 0) hsum += sqdist<D>(x, z[0]);   // r_11 = D_11
-                }
+                vp0 = va; vp1 = vb;
+            } else {
+                const int i0 = RP * (c * CH + t - lane);
+                if ((unsigned)i0 < (unsigned)n) { slow_row(i0, xa, va); vp0 = va; }
+                if ((unsigned)(i0 + 1) < (unsigned)n) { slow_row(i0 + 1, xb, vb); vp1 = vb; }
             }
-            if (lane == 31) vout_s[t] = vprev;
+            if (lane == 31) vout_s[t] = make_float2(vp0, vp1);
         };
         auto checkpoint = [&](const int idx) {             // state after step idx*TR - 1
             float* ck = CKme + (long long)idx * CK_FLOATS;
 #pragma unroll
             for (int g = 0; g < W / 4; ++g)
-                reinterpret_cast<float4*>(ck)[g * 32 + lane] = make_float4(h[4 * g], h[4 * g + 1], h[4 * g + 2], h[4 * g + 3]);
-            ck[W * 32 + lane] = vprev;
+                __stcs(reinterpret_cast<float4*>(ck) + g * 32 + lane, make_float4(h[4 * g], h[4 * g + 1], h[4 * g + 2], h[4 * g + 3]));
+            __stcs(reinterpret_cast<float2*>(ck + W * 32) + lane, make_float2(vp0, vp1));
         };
 
-        unsigned seen = 0;
+        // prefetch of chunk 0: the cycle's rows (cp.async) and the left strip's boundary values (registers)
+        stage_x_async<D>(xs0, p.Xs, pm.x_off, n, 0, lane);
+        const int vlane = (lane < CH) ? lane : 0;          // lanes >= CH duplicate lane 0's poll (CH < 32 only)
+        float2 vreg = make_float2(0.f, 0.f);
+        if (J > 0) vreg = ld_relaxed_f2(VSprev + 2 * vlane);
+        auto unpublished = [&](const float2 v, const int r) {   // rows >= n are never used
+            return (r < n && is_sentinel(v.x)) || (r + 1 < n && is_sentinel(v.y));
+        };
+
         for (int c = 0; c < C; ++c) {
-            if (J > 0) {                                   // wait until the left strip has published what this chunk reads
-                const unsigned need = (unsigned)min(c + 2, C);
-                while (seen < need) { seen = ld_acquire(p.prog_f + item - 1); if (seen < need) __nanosleep(128); }
+            const int rbase = c * CROWS + 2 * vlane;       // lane 0 works on rows rbase, rbase + 1 at step `vlane`
+#ifdef SDTW_EXPERIMENT_NODEP
+            if (false) {
+#else
+            if (J > 0) {                                   // valid = the left strip has published these rows
+#endif
+                bool bad = unpublished(vreg, rbase);
+                if (__any_sync(FULL, bad)) {
+                    if (SLACK > 0) {                       // caught up with the producer: let it get SLACK chunks ahead
+                        const int rw = min(c + SLACK, C - 1) * CROWS + 2 * vlane;
+                        for (;;) {
+                            const float2 t = ld_relaxed_f2(VSprev + rw);
+                            if (!__any_sync(FULL, unpublished(t, rw))) break;
+                            __nanosleep(400);
+                        }
+                    }
+                    for (;;) {
+                        if (bad) vreg = ld_relaxed_f2(VSprev + rbase);
+                        bad = unpublished(vreg, rbase);
+                        if (!__any_sync(FULL, bad)) break;
+                        __nanosleep(100);
+                    }
+                }
+            } else {
+                vreg = make_float2(rbase == 0 ? BIG : 0.f, 0.f);
             }
-            {
-                const int s = c * CH + lane;               // lane 0 works on row s at step s
-                vin_s[lane] = (J > 0) ? VSprev[s + 31] : ((s == 0) ? BIG : 0.f);
-                stage_x<D>(xs, p.X, pm.x_off, n, c, lane, p.sqrtk);
-            }
+            cp_async_wait_all();
+            if (lane < CH) vin_s[lane] = vreg;
             __syncwarp();
+            if (c + 1 < C) {                               // prefetch of chunk c + 1 (the other x buffer)
+                stage_x_async<D>(xs0 + ((c + 1) & 1) * XWIN * D, p.Xs, pm.x_off, n, c + 1, lane);
+                if (J > 0) vreg = ld_relaxed_f2(VSprev + rbase + CROWS);
+            }
+            xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;    // rows of step t: xs_lane[2t], [2t+1]
             if (interior_chunk(c, n) && (c < c_v0 || c > c_v1)) {
 #pragma unroll 1
                 for (int b = 0; b < CH / TR; ++b) {
@@ -284,15 +442,15 @@ __global__ void __launch_bounds__(WARPS * 32) forward_kernel(const Params p) {
                 }
             }
             __syncwarp();
-            VSme[c * CH + lane] = vout_s[lane];
-            __syncwarp();                                  // orders every lane's VS store before lane 0's release
-            if (lane == 0) st_release(p.prog_f + item, (unsigned)(c + 1));
+            // lane 31 worked on rows c CROWS - SKEW + 2t (+1) at step t
+            if (lane < CH) st_relaxed_f2(VSme + c * CROWS - SKEW + 2 * lane, vout_s[lane]);
         }
         // value partial of this item
         double part = (double)hsum + (double)vacc;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(FULL, part, o);
         if (lane == 0) p.VP[item] = part;
+        __syncwarp();
     }
 }
 
@@ -305,12 +463,12 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
     extern __shared__ __align__(16) float smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float* base = smem + warp * bwd_smem_floats<D>();
-    float2* stash = reinterpret_cast<float2*>(base) + lane;     // [TR][W][32] (+ lane)
-    float* xs = base + TR * W * 32 * 2;
-    float* vin_s = xs + 64 * D;
-    float* ein_s = vin_s + 32;
-    float* eout_s = ein_s + 32;
-    const float* xs_lane = xs + (32 - lane) * D;
+    float2* stash = reinterpret_cast<float2*>(base) + lane;     // [TR][RP][W][32] (+ lane)
+    float* xs = base + TR * RP * W * 32 * 2;                    // [XWIN][D]
+    float2* vin_s = reinterpret_cast<float2*>(xs + XWIN * D);   // [CH]
+    float2* ein_s = vin_s + 32;                                 // [CH] messages into lane 31: (.x row 2(s-31), .y the next)
+    float2* eout_s = ein_s + 32;                                // [CH] messages out of lane 0
+    const float* xs_lane = xs + (XPAD - 2 * lane) * D;
     const int m = p.m;
     constexpr int BPC = CH / TR;
 
@@ -326,8 +484,8 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
         const int item = ps * p.NS + J;
         const int j0 = (J * 32 + lane) * W;
         const bool has_right = (J < p.NS - 1);
-        const float* VSprev = p.VS + pm.vs_off + (long long)(J - 1) * pm.vs_stride;
-        float* ESme = p.ES + pm.vs_off + (long long)J * pm.vs_stride + 32;       // 32 floats of front padding
+        const float* VSprev = p.VS + pm.vs_off + (long long)(J - 1) * pm.vs_stride + VS_PAD;
+        float* ESme = p.ES + pm.vs_off + (long long)J * pm.vs_stride + VS_PAD;   // indexed by row
         const float* ESnext = ESme + pm.vs_stride;
         const float* CKme = p.CK + pm.ck_off + (long long)J * pm.ck_stride;
 
@@ -336,94 +494,136 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
         for (int w = 0; w < W; ++w) {
             const int j = j0 + w;
 #pragma unroll
-            for (int c = 0; c < D; ++c) { z[w][c] = (j < m) ? __ldg(p.Z + (long long)j * D + c) * p.sqrtk : 0.f; g[w][c] = 0.f; }
+            for (int c = 0; c < D; ++c) { z[w][c] = (j < m) ? __ldg(p.Zs + (long long)j * D + c) : 0.f; g[w][c] = 0.f; }
             A[w] = (j == m - 1) ? 1.f : 0.f;                  // E[n+1][m+1] = 1 flows into cell (n, m)
+            h[w] = 0.f;
         }
-        float vprev = 0.f, msg_prev = 0.f, cdf_prev = 0.f;
+        float vp0 = 0.f, vp1 = 0.f;
+        float msg0_prev = 0.f, msg1_prev = 0.f, cdf_prev = 0.f;
 
         // prefetch of the next checkpoint to restore
-        float4 ph[W / 4]; float pv = 0.f;
+        float4 ph[W / 4]; float2 pv = make_float2(0.f, 0.f);
         auto prefetch = [&](int bidx) {
             if (bidx >= 1) {
                 const float* ck = CKme + (long long)bidx * CK_FLOATS;
 #pragma unroll
                 for (int gq = 0; gq < W / 4; ++gq) ph[gq] = __ldcs(reinterpret_cast<const float4*>(ck) + gq * 32 + lane);
-                pv = __ldcs(ck + W * 32 + lane);
+                pv = __ldcs(reinterpret_cast<const float2*>(ck + W * 32) + lane);
             }
         };
         prefetch(C * BPC - 1);
 
-        // recompute step t of the chunk (u = t - t0 within the block), keeping the transition weights
+        // one row of the recompute, keeping the transition weights
+        auto rec_row = [&](const XRow<D>& x, float& v, const int slot) {
+#pragma unroll
+            for (int w = 0; w < W; ++w) {
+                float tl, acc, wu, wl;
+                sqdist2<D>(x, z[w], tl, acc);
+                cell<true, (D > 1)>(tl, acc, h[w], v, wu, wl);
+                stash[(slot * W + w) * 32] = make_float2(wu, wl);
+            }
+        };
+        // recompute step t of the chunk (u = t - t0 within the block)
         auto recompute = [&](const int c, const int t, const int u, auto tag) {
             constexpr bool slow = decltype(tag)::slow;
-            float v = __shfl_up_sync(FULL, vprev, 1);
-            if (lane == 0) v = vin_s[t];
-            const int i = c * CH + t - lane;
-            if (!slow || (unsigned)i < (unsigned)n) {
-                const XRow<D> x = load_x<D>(xs_lane, t);
+            float va = __shfl_up_sync(FULL, vp0, 1), vb = __shfl_up_sync(FULL, vp1, 1);
+            if (lane == 0) { const float2 qv = vin_s[t]; va = qv.x; vb = qv.y; }
+            XRow<D> xa, xb;
+            load_x2<D>(xs_lane, 2 * t, xa, xb);
+            if constexpr (!slow) {
 #pragma unroll
                 for (int w = 0; w < W; ++w) {
                     float tl, acc, wu, wl;
-                    sqdist2<D>(x, z[w], tl, acc);
-                    cell<true, (D > 1)>(tl, acc, h[w], v, wu, wl);
-                    stash[(u * W + w) * 32] = make_float2(wu, wl);
+                    sqdist2<D>(xa, z[w], tl, acc);
+                    cell<true, (D > 1)>(tl, acc, h[w], va, wu, wl);
+                    stash[((u * RP + 0) * W + w) * 32] = make_float2(wu, wl);
+                    sqdist2<D>(xb, z[w], tl, acc);
+                    cell<true, (D > 1)>(tl, acc, h[w], vb, wu, wl);
+                    stash[((u * RP + 1) * W + w) * 32] = make_float2(wu, wl);
                 }
-                vprev = v;
+                vp0 = va; vp1 = vb;
+            } else {
+                const int i0 = RP * (c * CH + t - lane);
+                if ((unsigned)i0 < (unsigned)n) { rec_row(xa, va, u * RP + 0); vp0 = va; }
+                if ((unsigned)(i0 + 1) < (unsigned)n) { rec_row(xb, vb, u * RP + 1); vp1 = vb; }
             }
         };
-        // E recurrence for the same step, backwards (probability flow, mass conserving)
+        // E recurrence of one row, right to left: E_in = flow into the last column's cell from the right neighbour;
+        // returns the left flow out of column 0 (cl) and the diagonal share of column 0 (cd)
+        auto e_row = [&](const XRow<D>& x, const float e_in, const int slot, float& cl, float& cd) {
+            float E = A[W - 1] + e_in;
+            float cd_right = 0.f;
+#pragma unroll
+            for (int w = W - 1; w >= 0; --w) {
+                const float2 wt = stash[(slot * W + w) * 32];
+#pragma unroll
+                for (int ch = 0; ch < D; ++ch) g[w][ch] = fmaf(E, z[w][ch] - x.c[ch], g[w][ch]);
+                const float Anew = fmaf(E, wt.x, cd_right);       // into (i-1, j): from (i, j) and, diagonally, (i, j+1)
+                cd_right = fmaf(-E, wt.y, fmaf(-E, wt.x, E));     // diagonal share of this cell
+                if (w > 0) E = fmaf(E, wt.y, A[w - 1]); else cl = E * wt.y;
+                A[w] = Anew;
+            }
+            cd = cd_right;
+        };
+        // E recurrence for the same step, backwards (probability flow, mass conserving): row 2(s-l)+1, then row 2(s-l)
         auto eflow = [&](const int c, const int t, const int u, auto tag) {
             constexpr bool slow = decltype(tag)::slow;
-            float msg_in = __shfl_down_sync(FULL, msg_prev, 1);
-            if (lane == 31) msg_in = ein_s[t];
-            const int i = c * CH + t - lane;
-            if (!slow || (unsigned)i < (unsigned)n) {
-                const XRow<D> x = load_x<D>(xs_lane, t);
-                float E = A[W - 1] + msg_in;
-                float cd_right = 0.f, cl_out = 0.f;
-#pragma unroll
-                for (int w = W - 1; w >= 0; --w) {
-                    const float2 wt = stash[(u * W + w) * 32];
-#pragma unroll
-                    for (int ch = 0; ch < D; ++ch) g[w][ch] = fmaf(E, z[w][ch] - x.c[ch], g[w][ch]);
-                    const float Anew = fmaf(E, wt.x, cd_right);       // into (i-1, j): from (i, j) and, diagonally, (i, j+1)
-                    cd_right = fmaf(-E, wt.y, fmaf(-E, wt.x, E));     // diagonal share of this cell
-                    if (w > 0) E = fmaf(E, wt.y, A[w - 1]); else cl_out = E * wt.y;
-                    A[w] = Anew;
-                }
-                msg_prev = cl_out + cdf_prev;                // flow into the left neighbour's cell (i, j0-1)
-                cdf_prev = cd_right;
+            float in0 = __shfl_down_sync(FULL, msg0_prev, 1), in1 = __shfl_down_sync(FULL, msg1_prev, 1);
+            if (lane == 31) { const float2 qe = ein_s[t]; in0 = qe.x; in1 = qe.y; }
+            XRow<D> xa, xb;
+            load_x2<D>(xs_lane, 2 * t, xa, xb);
+            const int i0 = RP * (c * CH + t - lane);
+            float cd_mid = cdf_prev;                           // row i0+1 missing (i0 + 1 == n): its diagonal share is 0
+            if (!slow || (unsigned)(i0 + 1) < (unsigned)n) {
+                float cl1, cd1;
+                e_row(xb, in1, u * RP + 1, cl1, cd1);
+                msg1_prev = cl1 + cdf_prev;                    // into the left neighbour's cell (i0+1, j0-1)
+                cd_mid = cd1;
             }
-            if (lane == 0) eout_s[t] = msg_prev;
+            if (!slow || (unsigned)i0 < (unsigned)n) {
+                float cl0, cd0;
+                e_row(xa, in0, u * RP + 0, cl0, cd0);
+                msg0_prev = cl0 + cd_mid;                      // into (i0, j0-1)
+                cdf_prev = cd0;
+            }
+            if (lane == 0) eout_s[t] = make_float2(msg0_prev, msg1_prev);
         };
 
         unsigned seen = 0;
         int pf = C * BPC - 1;                                  // block whose checkpoint (ph, pv) currently holds
         unsigned long long skipped = 0;
         for (int c = C - 1; c >= 0; --c) {
-            if (has_right) {                                   // right strip must have finished chunks >= max(c-1, 0)
-                const unsigned need = (unsigned)(C - max(c - 1, 0));
+            if (has_right) {                                   // right strip must have finished chunks >= max(c-LAGC, 0)
+                const unsigned need = (unsigned)(C - max(c - LAGC, 0));
                 while (seen < need) { seen = ld_acquire(p.prog_b + item + 1); if (seen < need) __nanosleep(64); }
             }
-            const int s = c * CH + lane;
-            const float ein = has_right ? ESnext[s - 31] : 0.f;   // lane 31 works on row s - 31 at step s
+            // lane 31 works on rows c CROWS - SKEW + 2t (+1) at step t; lane t fetches its message pair
+            const int erow = c * CROWS - SKEW + 2 * lane;
+            const float2 ein = (has_right && lane < CH && erow >= 0) ? *reinterpret_cast<const float2*>(ESnext + erow)
+                                                                     : make_float2(0.f, 0.f);
             // Exact skip: every flow that could enter this chunk's cells is +0 (E underflows to zero off the
             // alignment band), so every product and sum below would be +0 and g would not change.
             if (!p.dense_reverse) {
-                unsigned bits = __float_as_uint(ein) | __float_as_uint(msg_prev) | __float_as_uint(cdf_prev);
+                unsigned bits = __float_as_uint(ein.x) | __float_as_uint(ein.y) | __float_as_uint(msg0_prev) |
+                                __float_as_uint(msg1_prev) | __float_as_uint(cdf_prev);
 #pragma unroll
                 for (int w = 0; w < W; ++w) bits |= __float_as_uint(A[w]);
                 if (!__any_sync(FULL, bits != 0u)) {
-                    if (J > 0) ESme[c * CH + lane] = 0.f;
+                    if (J > 0 && lane < CH) *reinterpret_cast<float2*>(ESme + c * CROWS + 2 * lane) = make_float2(0.f, 0.f);
                     __syncwarp();
                     if (lane == 0) st_release(p.prog_b + item, (unsigned)(C - c));
                     ++skipped;
                     continue;
                 }
             }
-            vin_s[lane] = (J > 0) ? __ldcs(VSprev + s + 31) : ((s == 0) ? BIG : 0.f);
-            ein_s[lane] = ein;
-            stage_x<D>(xs, p.X, pm.x_off, n, c, lane, p.sqrtk);
+            stage_x_async<D>(xs, p.Xs, pm.x_off, n, c, lane);
+            if (lane < CH) {
+                const int rbase = c * CROWS + 2 * lane;
+                vin_s[lane] = (J > 0) ? __ldcs(reinterpret_cast<const float2*>(VSprev + rbase))
+                                      : make_float2(rbase == 0 ? BIG : 0.f, 0.f);
+                ein_s[lane] = ein;
+            }
+            cp_async_wait_all();
             __syncwarp();
             const bool fast = interior_chunk(c, n);
 #pragma unroll 1
@@ -432,12 +632,12 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
                 if (bidx == 0) {
 #pragma unroll
                     for (int w = 0; w < W; ++w) h[w] = (j0 + w == 0) ? BIG : 0.f;
-                    vprev = 0.f;
+                    vp0 = vp1 = 0.f;
                 } else {
                     if (pf != bidx) prefetch(bidx);            // the chunk below was skipped: nothing was prefetched
 #pragma unroll
                     for (int gq = 0; gq < W / 4; ++gq) { h[4 * gq] = ph[gq].x; h[4 * gq + 1] = ph[gq].y; h[4 * gq + 2] = ph[gq].z; h[4 * gq + 3] = ph[gq].w; }
-                    vprev = pv;
+                    vp0 = pv.x; vp1 = pv.y;
                 }
                 prefetch(bidx - 1);
                 pf = bidx - 1;
@@ -454,7 +654,8 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
                 }
             }
             __syncwarp();
-            if (J > 0) ESme[c * CH + lane] = eout_s[lane];
+            // lane 0 worked on rows 64c + 2t (+1) at step t
+            if (J > 0 && lane < CH) *reinterpret_cast<float2*>(ESme + c * CROWS + 2 * lane) = eout_s[lane];
             __syncwarp();                                      // orders every lane's ES store before lane 0's release
             if (lane == 0) st_release(p.prog_b + item, (unsigned)(C - c));
         }
@@ -468,6 +669,7 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
                 for (int ch = 0; ch < D; ++ch) p.Gk[((long long)ps * m + j) * D + ch] = g[w][ch] * p.gscale;
             }
         }
+        __syncwarp();
     }
 }
 

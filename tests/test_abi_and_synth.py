@@ -46,9 +46,11 @@ def test_workspace_bytes_planner(binding):
     fwd = binding.sdtw_workspace_bytes(30000, 1, off, False)
     assert 0 < fwd < full
     ti = binding.sdtw_tile_info()
-    # checkpoints dominate: (W+1) floats per thread per ckpt_steps => 4 (W+1) / (W ckpt_steps) bytes per cell
+    # checkpoints dominate: (W + R) floats per thread per ckpt_steps (W columns x R rows per step)
+    #   => 4 (W + R) / (W R ckpt_steps) bytes per cell
     cells = 90000 * 30000
-    per_cell = 4 * (ti["cols_per_thread"] + 1) / (ti["cols_per_thread"] * ti["ckpt_steps"])
+    Wc, Rr = ti["cols_per_thread"], ti["rows_per_step"]
+    per_cell = 4 * (Wc + Rr) / (Wc * Rr * ti["ckpt_steps"])
     assert 0.9 * per_cell * cells < full < 1.3 * per_cell * cells
     # invalid arguments -> 0
     assert binding.sdtw_workspace_bytes(0, 1, off, True) == 0
