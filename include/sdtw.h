@@ -135,6 +135,13 @@ int sdtw_measure_mufu_peak(int32_t kind, double* ops_per_s, int32_t* sm_count);
 int sdtw_set_reverse_mode(int dense);
 int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped);
 
+/*
+ * Forward schedule (tuning, does not change any result bit): the forward kernel hands out UNITS of `unit_strips`
+ * adjacent column strips of one pair to its CTAs (sdtw_kernels.cuh).  0 restores the automatic choice; values above
+ * the kernel's warps per CTA are clamped.  Negative => SDTW_ERR_INVALID_ARG.
+ */
+int sdtw_set_schedule(int unit_strips);
+
 /* Compile-time tile constants, for DESIGN.md / bench.py reporting: columns per thread, columns per strip (work item),
  * wavefront steps between checkpoints, steps per strip-boundary exchange, rows a lane works on per step.  Any pointer
  * may be NULL. */

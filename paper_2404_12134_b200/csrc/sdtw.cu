@@ -22,6 +22,7 @@ void* g_user_ws = nullptr;
 size_t g_user_ws_bytes = 0;
 bool g_profile = false;
 int g_dense_reverse = 0;
+int g_unit_strips = 0;        // 0 = automatic (sdtw_set_schedule)
 const unsigned long long* g_last_stats = nullptr;   // device address of the last evaluation's reverse statistics
 
 struct ProfRec { cudaEvent_t e[5]; };   // start | prologue | forward | reverse | small kernels
@@ -193,7 +194,7 @@ int persistent_grid(K kernel, int smem_bytes, int sms, long long items, int* gri
 template <int D> constexpr int fwd_warps() { return D <= 2 ? 32 : 16; }   // warps per CTA = strips per unit
 
 template <int D, bool CKPT>
-int launch_forward_t(const Params& P, int sms, cudaStream_t stream) {
+int launch_forward_t(Params P, int sms, cudaStream_t stream) {
     constexpr int FW = fwd_warps<D>();
     const int smem = FW * fwd_smem_floats<D>() * 4;
     auto kernel = forward_kernel<D, CKPT, FW>;
@@ -201,7 +202,12 @@ int launch_forward_t(const Params& P, int sms, cudaStream_t stream) {
     int occ = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, FW * 32, smem));
     if (occ < 1) return SDTW_ERR_UNSUPPORTED;
-    const long long units = (long long)((P.NS + FW - 1) / FW) * P.N;
+    // Strips per unit.  Throughput regime (more strips than resident warps): a unit fills a CTA, so a strip and its
+    // producer share an SM.  Latency regime (every strip resident at once: few or short pairs): one strip per unit
+    // spreads each pair's dependency chain over as many SMs as possible.
+    const bool all_resident = (long long)P.NS * P.N <= (long long)sms * occ * FW;
+    P.unit_strips = (g_unit_strips > 0) ? std::min(g_unit_strips, FW) : (all_resident ? 1 : FW);
+    const long long units = (long long)((P.NS + P.unit_strips - 1) / P.unit_strips) * P.N;
     const int grid = (int)std::max(1LL, std::min(units, (long long)sms * occ));
     kernel<<<grid, FW * 32, smem, stream>>>(P);
     ++g_launches;
@@ -544,6 +550,13 @@ int sdtw_profile_read(double* ms_forward, double* ms_backward, double* ms_other,
     if (ms_other) *ms_other = o;
     if (evaluations) *evaluations = (int64_t)g_prof.size();
     g_prof.clear();
+    return SDTW_OK;
+}
+
+int sdtw_set_schedule(int unit_strips) {
+    if (unit_strips < 0) return SDTW_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    g_unit_strips = unit_strips;
     return SDTW_OK;
 }
 

@@ -41,7 +41,7 @@ namespace sdtw {
 #define SDTW_CH 32
 #endif
 #ifndef SDTW_SLACK
-#define SDTW_SLACK 2
+#define SDTW_SLACK 0
 #endif
 
 constexpr int W = SDTW_W;       // columns per thread
@@ -92,6 +92,7 @@ struct Params {
     unsigned num_items;
     unsigned long long* stats;  // [0] reverse chunks visited, [1] reverse chunks skipped (instrumentation; may be null)
     int dense_reverse;    // 1: never skip a reverse chunk (for measurement / validation of the exact skip)
+    int unit_strips;      // forward schedule: adjacent strips of one pair per unit (1 .. warps per CTA)
     float gscale;         // 2 / sqrt(kappa)
 };
 
@@ -243,7 +244,7 @@ __global__ void scale_inputs_kernel(const float* __restrict__ X, long long nx, c
 // earlier units.  So a strip and the strip it waits on run on the SAME SM (8 consecutive ones on the same scheduler): a
 // warp that has caught up with its producer stops competing with it for the MUFU pipe, which is what balances the
 // chain; chains that span SMs leave every SM partly idle.
-constexpr int UNIT_RING = 8;
+constexpr int UNIT_RING = 16;
 struct RollCtl { int popped; int lock; int uid[UNIT_RING]; int seen[32]; };
 
 template <int D, bool CKPT, int FW>
@@ -255,7 +256,8 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
     float2* vin_s = reinterpret_cast<float2*>(xs0 + 2 * XWIN * D);   // [CH] (v_in of lane 0 for the step's two rows)
     float2* vout_s = vin_s + 32;                                     // [CH] (v_out of lane 31)
     const int m = p.m;
-    const int NG = (p.NS + FW - 1) / FW, NU = NG * p.N;              // groups per pair, units
+    const int US = p.unit_strips;                                    // strips per unit, <= FW
+    const int NG = (p.NS + US - 1) / US, NU = NG * p.N;              // groups per pair, units
     // position of this warp in the rolling stream: consecutive positions share a scheduler (warp id mod 4)
     const int mypos = (warp & 3) * (FW / 4) + (warp >> 2);
     if (threadIdx.x < 32) { ctl.seen[threadIdx.x] = 0; if (threadIdx.x == 0) { ctl.popped = 0; ctl.lock = 0; } }
@@ -293,11 +295,11 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
         u = __shfl_sync(FULL, u, 0);
         if (u >= NU) break;
         const int g = u / p.N, ps = u - g * p.N;
-        const int S = min(FW, p.NS - g * FW);              // strips of this unit
+        const int S = min(US, p.NS - g * US);              // strips of this unit
         const int sidx = (mypos - base + FW) % FW;
         base = (base + S) % FW;
         if (sidx >= S) continue;
-        const int J = g * FW + sidx;
+        const int J = g * US + sidx;
         const PairMeta pm = p.pm[ps];
         const int n = pm.n, C = pm.C;
         const int item = ps * p.NS + J;
