@@ -87,8 +87,9 @@ def forward_R(D, gamma):
     return R
 
 
-def pair(x, z, gamma, want_grad=True, want_E=False, want_R=False, mode="full"):
-    """One (x, z) pair.  Returns dict(value, grad (m,d) or None, E (n,m) or None, R or None)."""
+def pair(x, z, gamma, want_grad=True, want_E=False, want_R=False, mode="full", band=-1):
+    """One (x, z) pair.  Returns dict(value, grad (m,d) or None, E (n,m) or None, R or None).
+    band >= 0: Sakoe-Chiba band |i - j| <= band (Table 1); band < 0: none."""
     x = _as2d(x)
     z = _as2d(z)
     n, d = x.shape
@@ -99,15 +100,16 @@ def pair(x, z, gamma, want_grad=True, want_E=False, want_R=False, mode="full"):
     lib = _load()
     if mode == "checkpointed":
         assert not want_E and not want_R
-        _chk(lib.oracle_pair_checkpointed(_d(x), ctypes.c_int64(n), _d(z), ctypes.c_int64(m), ctypes.c_int(d),
-                                          ctypes.c_double(gamma), ctypes.byref(value),
-                                          _d(grad) if want_grad else None))
+        _chk(lib.oracle_pair_checkpointed_banded(_d(x), ctypes.c_int64(n), _d(z), ctypes.c_int64(m), ctypes.c_int(d),
+                                                 ctypes.c_double(gamma), ctypes.c_int64(band), ctypes.byref(value),
+                                                 _d(grad) if want_grad else None))
         return dict(value=value.value, grad=grad, E=None, R=None)
     E = np.empty((n, m), np.float64) if want_E else None
     R = np.empty((n + 2, m + 2), np.float64) if want_R else None
-    _chk(lib.oracle_pair_full(_d(x), ctypes.c_int64(n), _d(z), ctypes.c_int64(m), ctypes.c_int(d),
-                              ctypes.c_double(gamma), ctypes.byref(value), _d(grad) if want_grad else None,
-                              _d(E) if want_E else None, _d(R) if want_R else None))
+    _chk(lib.oracle_pair_full_banded(_d(x), ctypes.c_int64(n), _d(z), ctypes.c_int64(m), ctypes.c_int(d),
+                                     ctypes.c_double(gamma), ctypes.c_int64(band), ctypes.byref(value),
+                                     _d(grad) if want_grad else None, _d(E) if want_E else None,
+                                     _d(R) if want_R else None))
     return dict(value=value.value, grad=grad, E=E, R=R)
 
 
@@ -145,23 +147,38 @@ def _f32_inputs(Z, X_concat, offsets):
     return Z, X, off
 
 
-def value_grad(Z, X_concat, offsets, gamma, want_grad=True, mode="full", nthreads=0):
-    """Mirror of the C-ABI sdtw_value_grad: fp32 inputs promoted to float64.
-    Returns (values (N,) float64, grad (m, d) float64 or None)."""
+def _weights(weights, N):
+    if weights is None:
+        return None, None
+    w = np.ascontiguousarray(weights, np.float64)
+    assert w.shape == (N,)
+    return w, _d(w)
+
+
+def value_grad(Z, X_concat, offsets, gamma, want_grad=True, mode="full", nthreads=0, weights=None, band=-1,
+               want_objective=False):
+    """Mirror of the C-ABI sdtw_value_grad / sdtw_value_grad_ex: fp32 inputs promoted to float64.
+    Returns (values (N,) float64, grad (m, d) float64 or None) [+ objective if want_objective];
+    grad = sum_k w_k grad_k, objective = sum_k w_k values[k] (weights None = 1), band < 0 = none."""
     Z, X, off = _f32_inputs(Z, X_concat, offsets)
     m, d = Z.shape
     N = len(off) - 1
     values = np.zeros(N, np.float64)
     grad = np.zeros((m, d), np.float64) if want_grad else None
-    _chk(_load().oracle_value_grad_f32(Z.ctypes.data_as(_c_float_p), ctypes.c_int64(m), ctypes.c_int(d),
-                                       X.ctypes.data_as(_c_float_p), off.ctypes.data_as(_c_i64_p), ctypes.c_int(N),
-                                       ctypes.c_double(gamma), _d(values), _d(grad) if want_grad else None,
-                                       ctypes.c_int(1 if mode == "checkpointed" else 0), ctypes.c_int(nthreads)))
+    w, wp = _weights(weights, N)
+    obj = ctypes.c_double(0.0)
+    _chk(_load().oracle_value_grad_ex_f32(Z.ctypes.data_as(_c_float_p), ctypes.c_int64(m), ctypes.c_int(d),
+                                          X.ctypes.data_as(_c_float_p), off.ctypes.data_as(_c_i64_p), ctypes.c_int(N),
+                                          ctypes.c_double(gamma), wp, ctypes.c_int64(band), _d(values),
+                                          _d(grad) if want_grad else None, ctypes.byref(obj),
+                                          ctypes.c_int(1 if mode == "checkpointed" else 0), ctypes.c_int(nthreads)))
+    if want_objective:
+        return values, grad, obj.value
     return values, grad
 
 
-def barycenter(Z0, X_concat, offsets, gamma, iters, step, mode="full", nthreads=0):
-    """Mirror of sdtw_barycenter: fixed-step GD in float64.
+def barycenter(Z0, X_concat, offsets, gamma, iters, step, mode="full", nthreads=0, weights=None, band=-1):
+    """Mirror of sdtw_barycenter / sdtw_barycenter_ex: fixed-step GD in float64 on sum_k w_k value_k.
     Returns (Z (m,d) float64, values (N,) at the last evaluated iterate, objective (iters,))."""
     Z0, X, off = _f32_inputs(Z0, X_concat, offsets)
     m, d = Z0.shape
@@ -169,9 +186,10 @@ def barycenter(Z0, X_concat, offsets, gamma, iters, step, mode="full", nthreads=
     Z = np.zeros((m, d), np.float64)
     values = np.zeros(N, np.float64)
     obj = np.zeros(max(iters, 1), np.float64)
-    _chk(_load().oracle_barycenter_f32(Z0.ctypes.data_as(_c_float_p), ctypes.c_int64(m), ctypes.c_int(d),
-                                       X.ctypes.data_as(_c_float_p), off.ctypes.data_as(_c_i64_p), ctypes.c_int(N),
-                                       ctypes.c_double(gamma), ctypes.c_int(iters), ctypes.c_double(step), _d(Z),
-                                       _d(values), _d(obj), ctypes.c_int(1 if mode == "checkpointed" else 0),
-                                       ctypes.c_int(nthreads)))
+    w, wp = _weights(weights, N)
+    _chk(_load().oracle_barycenter_ex_f32(Z0.ctypes.data_as(_c_float_p), ctypes.c_int64(m), ctypes.c_int(d),
+                                          X.ctypes.data_as(_c_float_p), off.ctypes.data_as(_c_i64_p), ctypes.c_int(N),
+                                          ctypes.c_double(gamma), wp, ctypes.c_int64(band), ctypes.c_int(iters),
+                                          ctypes.c_double(step), _d(Z), _d(values), _d(obj),
+                                          ctypes.c_int(1 if mode == "checkpointed" else 0), ctypes.c_int(nthreads)))
     return Z, values, obj[:iters]

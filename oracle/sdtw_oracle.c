@@ -26,6 +26,13 @@
  *   Def. 7 / eq. 7  barycenter objective, read (C6, C8) as the plain sum
  *                               over k minimised by fixed-step gradient descent.
  *   Def. 4 / eq. 1  classic DTW (the gamma = 0 case), used as a pin.
+ *   Table 1  Sakoe-Chiba band: read (C18) as the classic adjustment
+ *                               window |i - j| <= band on the cell indices; cells outside it belong
+ *                               to no admissible path (Delta = +inf there, so r = +inf, E = 0).
+ *                               band < 0 means no band.  The *_ex entry points take it.
+ *   eq. 7  per-series weights lambda_i / m_i: the *_ex entry points take one
+ *                               weight w_k per pair; objective = sum_k w_k value_k and
+ *                               grad = sum_k w_k grad_k (values[k] stay unweighted).
  *
  * Index convention: x has n rows (time steps) of d channels, z has m rows of d channels,
  * both row-major [t][c].  R is stored with the paper's 0-row/0-column border (and one more
@@ -66,6 +73,15 @@ static double min3(double a, double b, double c) {
     return mn;
 }
 
+/* ---- Sakoe-Chiba band (Table 1; reading C18): cell (i, j) is admissible iff
+ * |i - j| <= band; band < 0 = no band.  Same for 0- or 1-based (i, j). ---- */
+static int admissible(int64_t i, int64_t j, int64_t band) {
+    if (band < 0) return 1;
+    int64_t t = i - j;
+    if (t < 0) t = -t;
+    return t <= band;
+}
+
 /* ---- Def. 3: delta(x_i, z_j) = sum_c (x_ic - z_jc)^2 ---- */
 static double delta_sq(const double *xi, const double *zj, int d) {
     double s = 0.0;
@@ -86,7 +102,12 @@ int oracle_cost_matrix(const double *x, int64_t n, const double *z, int64_t m, i
 
 /* ---- Def. 6 / eq. 5 on a given cost matrix.  R is (n+2) x (m+2); on return rows 0..n and
  * columns 0..m hold r_ij (border: r_00 = 0, r_i0 = r_0j = +inf).  gamma == 0 gives eq. 1. ---- */
+int oracle_forward_R_banded(const double *D, int64_t n, int64_t m, double gamma, int64_t band, double *R);
 int oracle_forward_R(const double *D, int64_t n, int64_t m, double gamma, double *R) {
+    return oracle_forward_R_banded(D, n, m, gamma, -1, R);
+}
+/* the same with a Sakoe-Chiba band: inadmissible cells get r = +inf */
+int oracle_forward_R_banded(const double *D, int64_t n, int64_t m, double gamma, int64_t band, double *R) {
     if (!D || !R || n < 1 || m < 1 || !(gamma >= 0.0)) return ORACLE_ERR_ARG;
     const int64_t ld = m + 2;
     for (int64_t j = 0; j <= m + 1; ++j) R[j] = INFINITY;
@@ -94,6 +115,7 @@ int oracle_forward_R(const double *D, int64_t n, int64_t m, double gamma, double
     R[0] = 0.0;
     for (int64_t i = 1; i <= n; ++i)
         for (int64_t j = 1; j <= m; ++j) {
+            if (!admissible(i, j, band)) { R[i * ld + j] = INFINITY; continue; }
             double rd = R[(i - 1) * ld + (j - 1)], ru = R[(i - 1) * ld + j], rl = R[i * ld + (j - 1)];
             double sm = (gamma > 0.0) ? softmin3(rd, ru, rl, gamma) : min3(rd, ru, rl);
             R[i * ld + j] = D[(i - 1) * m + (j - 1)] + sm;
@@ -110,8 +132,15 @@ int oracle_forward_R(const double *D, int64_t n, int64_t m, double gamma, double
  *           + E[i+1][j+1] exp((R[i+1][j+1] - R[i][j] - D[i+1][j+1]) / gamma).
  * R must be the (n+2) x (m+2) array filled by oracle_forward_R (it is padded in place).
  * E is n x m row-major (0-based). ---- */
+int oracle_backward_E_banded(const double *D, int64_t n, int64_t m, double gamma, int64_t band, double *R, double *E);
 int oracle_backward_E(const double *D, int64_t n, int64_t m, double gamma, double *R, double *E) {
+    return oracle_backward_E_banded(D, n, m, gamma, -1, R, E);
+}
+/* the same with a Sakoe-Chiba band: an inadmissible cell has E = 0 and contributes nothing to its
+ * predecessors (it lies on no admissible path); requires |n - m| <= band (else no path exists). */
+int oracle_backward_E_banded(const double *D, int64_t n, int64_t m, double gamma, int64_t band, double *R, double *E) {
     if (!D || !R || !E || n < 1 || m < 1 || !(gamma > 0.0)) return ORACLE_ERR_ARG;
+    if (!admissible(n, m, band)) return ORACLE_ERR_ARG;
     const int64_t ld = m + 2;
     double *Ep = (double *)calloc((size_t)((n + 2) * ld), sizeof(double));
     if (!Ep) return ORACLE_ERR_MEM;
@@ -120,14 +149,17 @@ int oracle_backward_E(const double *D, int64_t n, int64_t m, double gamma, doubl
     R[(n + 1) * ld + (m + 1)] = R[n * ld + m];
     Ep[(n + 1) * ld + (m + 1)] = 1.0;
 #define DPAD(i, j) (((i) <= n && (j) <= m) ? D[((i)-1) * m + ((j)-1)] : 0.0)
+#define OK_S(i, j) (((i) > n || (j) > m) ? 1 : admissible((i), (j), band)) /* pad cells are not masked */
     for (int64_t j = m; j >= 1; --j)
         for (int64_t i = n; i >= 1; --i) {
+            if (!admissible(i, j, band)) continue; /* E = 0 */
             double r = R[i * ld + j];
-            double a = exp((R[(i + 1) * ld + j] - r - DPAD(i + 1, j)) / gamma);
-            double b = exp((R[i * ld + (j + 1)] - r - DPAD(i, j + 1)) / gamma);
-            double c = exp((R[(i + 1) * ld + (j + 1)] - r - DPAD(i + 1, j + 1)) / gamma);
+            double a = OK_S(i + 1, j) ? exp((R[(i + 1) * ld + j] - r - DPAD(i + 1, j)) / gamma) : 0.0;
+            double b = OK_S(i, j + 1) ? exp((R[i * ld + (j + 1)] - r - DPAD(i, j + 1)) / gamma) : 0.0;
+            double c = OK_S(i + 1, j + 1) ? exp((R[(i + 1) * ld + (j + 1)] - r - DPAD(i + 1, j + 1)) / gamma) : 0.0;
             Ep[i * ld + j] = Ep[(i + 1) * ld + j] * a + Ep[i * ld + (j + 1)] * b + Ep[(i + 1) * ld + (j + 1)] * c;
         }
+#undef OK_S
 #undef DPAD
     for (int64_t i = 1; i <= n; ++i)
         for (int64_t j = 1; j <= m; ++j) E[(i - 1) * m + (j - 1)] = Ep[i * ld + j];
@@ -178,9 +210,16 @@ static void contract_gradient(const double *E, const double *x, int64_t n, const
 
 /* ---- one pair, full-matrix mode: value = r_{n,m}; grad (may be NULL) incremented by eq. 6;
  * E_out / R_out (may be NULL) receive the n x m E and the (n+2) x (m+2) R. ---- */
+int oracle_pair_full_banded(const double *x, int64_t n, const double *z, int64_t m, int d, double gamma,
+                            int64_t band, double *value, double *grad, double *E_out, double *R_out);
 int oracle_pair_full(const double *x, int64_t n, const double *z, int64_t m, int d, double gamma, double *value,
                      double *grad, double *E_out, double *R_out) {
+    return oracle_pair_full_banded(x, n, z, m, d, gamma, -1, value, grad, E_out, R_out);
+}
+int oracle_pair_full_banded(const double *x, int64_t n, const double *z, int64_t m, int d, double gamma,
+                            int64_t band, double *value, double *grad, double *E_out, double *R_out) {
     if (!x || !z || !value || n < 1 || m < 1 || d < 1 || !(gamma > 0.0)) return ORACLE_ERR_ARG;
+    if (!admissible(n, m, band)) return ORACLE_ERR_ARG; /* no complete path inside the band */
     double *D = (double *)malloc((size_t)(n * m) * sizeof(double));
     double *R = (double *)malloc((size_t)((n + 2) * (m + 2)) * sizeof(double));
     if (!D || !R) {
@@ -189,7 +228,7 @@ int oracle_pair_full(const double *x, int64_t n, const double *z, int64_t m, int
         return ORACLE_ERR_MEM;
     }
     oracle_cost_matrix(x, n, z, m, d, D);
-    oracle_forward_R(D, n, m, gamma, R);
+    oracle_forward_R_banded(D, n, m, gamma, band, R);
     *value = R[n * (m + 2) + m];
     int rc = ORACLE_OK;
     if (grad || E_out) {
@@ -199,7 +238,7 @@ int oracle_pair_full(const double *x, int64_t n, const double *z, int64_t m, int
             if (R_out) { /* keep the unpadded forward R for the caller */
                 memcpy(R_out, R, (size_t)((n + 2) * (m + 2)) * sizeof(double));
             }
-            rc = oracle_backward_E(D, n, m, gamma, R, E);
+            rc = oracle_backward_E_banded(D, n, m, gamma, band, R, E);
             if (rc == ORACLE_OK && grad) contract_gradient(E, x, n, z, m, d, grad);
         }
         if (!E_out) free(E);
@@ -216,18 +255,26 @@ int oracle_pair_full(const double *x, int64_t n, const double *z, int64_t m, int
  * of R going backwards, hold only two rows of E.  Every cell is computed by exactly the
  * same expressions, in the same order, as in oracle_pair_full, so value and grad are
  * BITWISE identical to the full mode (tests/test_oracle_pins.py checks this). ---- */
-static void forward_row(const double *xi, const double *z, int64_t m, int d, double gamma, const double *Rprev,
-                        double *Rcur /* both (m+2) wide, 1-based */) {
+static void forward_row(const double *xi, int64_t i /* 1-based row */, const double *z, int64_t m, int d, double gamma,
+                        int64_t band, const double *Rprev, double *Rcur /* both (m+2) wide, 1-based */) {
     Rcur[0] = INFINITY;
     for (int64_t j = 1; j <= m; ++j) {
+        if (!admissible(i, j, band)) { Rcur[j] = INFINITY; continue; }
         double dij = delta_sq(xi, z + (j - 1) * d, d);
         Rcur[j] = dij + softmin3(Rprev[j - 1], Rprev[j], Rcur[j - 1], gamma);
     }
 }
 
+int oracle_pair_checkpointed_banded(const double *x, int64_t n, const double *z, int64_t m, int d, double gamma,
+                                    int64_t band, double *value, double *grad);
 int oracle_pair_checkpointed(const double *x, int64_t n, const double *z, int64_t m, int d, double gamma,
                              double *value, double *grad) {
+    return oracle_pair_checkpointed_banded(x, n, z, m, d, gamma, -1, value, grad);
+}
+int oracle_pair_checkpointed_banded(const double *x, int64_t n, const double *z, int64_t m, int d, double gamma,
+                                    int64_t band, double *value, double *grad) {
     if (!x || !z || !value || n < 1 || m < 1 || d < 1 || !(gamma > 0.0)) return ORACLE_ERR_ARG;
+    if (!admissible(n, m, band)) return ORACLE_ERR_ARG;
     const int64_t ld = m + 2;
     int64_t K = (int64_t)ceil(sqrt((double)n));
     if (K < 1) K = 1;
@@ -247,7 +294,7 @@ int oracle_pair_checkpointed(const double *x, int64_t n, const double *z, int64_
     prev[0] = 0.0;
     memcpy(ck, prev, (size_t)ld * sizeof(double));
     for (int64_t i = 1; i <= n; ++i) {
-        forward_row(x + (i - 1) * d, z, m, d, gamma, prev, cur);
+        forward_row(x + (i - 1) * d, i, z, m, d, gamma, band, prev, cur);
         cur[m + 1] = INFINITY;
         if (i % K == 0) memcpy(ck + (i / K) * ld, cur, (size_t)ld * sizeof(double));
         double *t = prev; prev = cur; cur = t;
@@ -262,7 +309,7 @@ int oracle_pair_checkpointed(const double *x, int64_t n, const double *z, int64_
             if (b1 > n) b1 = n;
             memcpy(blk, ck + (b0 / K) * ld, (size_t)ld * sizeof(double));
             for (int64_t i = b0 + 1; i <= b1; ++i)
-                forward_row(x + (i - 1) * d, z, m, d, gamma, blk + (i - 1 - b0) * ld, blk + (i - b0) * ld);
+                forward_row(x + (i - 1) * d, i, z, m, d, gamma, band, blk + (i - 1 - b0) * ld, blk + (i - b0) * ld);
             /* row b1+1 of R: the pad row (-inf, corner R[n][m]) if b1 == n, else the first row of
              * the block processed just before (kept in blk's last slot by the copy below). */
             double *Rnext = blk + (b1 - b0 + 1) * ld;
@@ -281,13 +328,17 @@ int oracle_pair_checkpointed(const double *x, int64_t n, const double *z, int64_
                 Ri[m + 1] = -INFINITY; /* pad column of the reverse pass */
                 Eb[m + 1] = 0.0;
                 for (int64_t j = m; j >= 1; --j) {
+                    if (!admissible(i, j, band)) { Eb[j] = 0.0; continue; }
                     double r = Ri[j];
                     double d_dn = last_row ? 0.0 : delta_sq(x + i * d, z + (j - 1) * d, d);              /* D[i+1][j]   */
                     double d_rt = (j == m) ? 0.0 : delta_sq(x + (i - 1) * d, z + j * d, d);              /* D[i][j+1]   */
                     double d_dg = (last_row || j == m) ? 0.0 : delta_sq(x + i * d, z + j * d, d);        /* D[i+1][j+1] */
-                    double a = exp((Ri1[j] - r - d_dn) / gamma);
-                    double b = exp((Ri[j + 1] - r - d_rt) / gamma);
-                    double c = exp((Ri1[j + 1] - r - d_dg) / gamma);
+                    /* successors inside the matrix but outside the band contribute nothing */
+                    const int ok_dn = last_row || admissible(i + 1, j, band);
+                    const int ok_rt = (j == m) || admissible(i, j + 1, band);
+                    double a = ok_dn ? exp((Ri1[j] - r - d_dn) / gamma) : 0.0;
+                    double b = ok_rt ? exp((Ri[j + 1] - r - d_rt) / gamma) : 0.0;
+                    double c = exp((Ri1[j + 1] - r - d_dg) / gamma); /* (i+1, j+1) has the same i - j */
                     Eb[j] = Ea[j] * a + Eb[j + 1] * b + Ea[j + 1] * c;
                 }
                 for (int64_t j = 0; j < m; ++j) {
@@ -309,8 +360,18 @@ int oracle_pair_checkpointed(const double *x, int64_t n, const double *z, int64_
  * promoted to double; values[k] = Soft-DTW(x_k, Z); grad = sum_k grad_k in k order (NULL =>
  * values only).  mode 0 = full matrices, 1 = row-checkpointed.  OpenMP over pairs only;
  * per-pair gradients are added into grad in ascending k whatever the thread count. ---- */
+int oracle_value_grad_ex_f32(const float *Z, int64_t m, int d, const float *X, const int64_t *offsets, int N,
+                             double gamma, const double *weights, int64_t band, double *values, double *grad,
+                             double *objective, int mode, int nthreads);
 int oracle_value_grad_f32(const float *Z, int64_t m, int d, const float *X, const int64_t *offsets, int N,
                           double gamma, double *values, double *grad, int mode, int nthreads) {
+    return oracle_value_grad_ex_f32(Z, m, d, X, offsets, N, gamma, NULL, -1, values, grad, NULL, mode, nthreads);
+}
+/* the same with eq. 7's per-pair weights w_k (NULL = all 1) and Table 1's Sakoe-Chiba band (< 0 = none):
+ * values[k] unweighted, grad = sum_k w_k grad_k (k ascending), *objective = sum_k w_k values[k]. */
+int oracle_value_grad_ex_f32(const float *Z, int64_t m, int d, const float *X, const int64_t *offsets, int N,
+                             double gamma, const double *weights, int64_t band, double *values, double *grad,
+                             double *objective, int mode, int nthreads) {
     if (!Z || !X || !offsets || !values || m < 1 || d < 1 || N < 1 || !(gamma > 0.0)) return ORACLE_ERR_ARG;
     for (int k = 0; k < N; ++k)
         if (offsets[k + 1] <= offsets[k]) return ORACLE_ERR_ARG;
@@ -332,8 +393,8 @@ int oracle_value_grad_f32(const float *Z, int64_t m, int d, const float *X, cons
         if (rc == ORACLE_OK) {
             for (int64_t t = 0; t < n * d; ++t) x[t] = (double)X[offsets[k] * d + t];
             double *g = gk ? gk + (size_t)k * (size_t)(m * d) : NULL;
-            if (mode == 1) rc = oracle_pair_checkpointed(x, n, z, m, d, gamma, &values[k], g);
-            else rc = oracle_pair_full(x, n, z, m, d, gamma, &values[k], g, NULL, NULL);
+            if (mode == 1) rc = oracle_pair_checkpointed_banded(x, n, z, m, d, gamma, band, &values[k], g);
+            else rc = oracle_pair_full_banded(x, n, z, m, d, gamma, band, &values[k], g, NULL, NULL);
         }
         free(x);
         if (rc != ORACLE_OK) {
@@ -343,8 +404,15 @@ int oracle_value_grad_f32(const float *Z, int64_t m, int d, const float *X, cons
     }
     if (grad) {
         for (int64_t t = 0; t < m * d; ++t) grad[t] = 0.0;
-        for (int k = 0; k < N; ++k)
-            for (int64_t t = 0; t < m * d; ++t) grad[t] += gk[(size_t)k * (size_t)(m * d) + t];
+        for (int k = 0; k < N; ++k) {
+            const double w = weights ? weights[k] : 1.0;
+            for (int64_t t = 0; t < m * d; ++t) grad[t] += w * gk[(size_t)k * (size_t)(m * d) + t];
+        }
+    }
+    if (objective) {
+        double obj = 0.0;
+        for (int k = 0; k < N; ++k) obj += (weights ? weights[k] : 1.0) * values[k];
+        *objective = obj;
     }
     free(z);
     free(gk);
@@ -357,9 +425,19 @@ int oracle_value_grad_f32(const float *Z, int64_t m, int d, const float *X, cons
  * objective[t] = sum_k value_k(Z(t)) (before the t-th update); values = the per-pair values
  * at the last evaluated iterate Z(iters-1).  Because the pair routines take Z as float in
  * oracle_value_grad_f32, this routine carries its own double-Z loop. ---- */
+int oracle_barycenter_ex_f32(const float *Z0, int64_t m, int d, const float *X, const int64_t *offsets, int N,
+                             double gamma, const double *weights, int64_t band, int iters, double step,
+                             double *Z_out, double *values, double *objective, int mode, int nthreads);
 int oracle_barycenter_f32(const float *Z0, int64_t m, int d, const float *X, const int64_t *offsets, int N,
                           double gamma, int iters, double step, double *Z_out, double *values, double *objective,
                           int mode, int nthreads) {
+    return oracle_barycenter_ex_f32(Z0, m, d, X, offsets, N, gamma, NULL, -1, iters, step, Z_out, values, objective,
+                                    mode, nthreads);
+}
+/* eq. 7 proper: objective sum_k w_k Soft-DTW(Z, x_k) (w_k = lambda_k / n_k in the paper), optional band */
+int oracle_barycenter_ex_f32(const float *Z0, int64_t m, int d, const float *X, const int64_t *offsets, int N,
+                             double gamma, const double *weights, int64_t band, int iters, double step,
+                             double *Z_out, double *values, double *objective, int mode, int nthreads) {
     if (!Z0 || !X || !offsets || !Z_out || m < 1 || d < 1 || N < 1 || !(gamma > 0.0) || iters < 0)
         return ORACLE_ERR_ARG;
     for (int k = 0; k < N; ++k)
@@ -385,8 +463,8 @@ int oracle_barycenter_f32(const float *Z0, int64_t m, int d, const float *X, con
             if (rc == ORACLE_OK) {
                 for (int64_t t = 0; t < n * d; ++t) x[t] = (double)X[offsets[k] * d + t];
                 double *g = gk + (size_t)k * (size_t)md;
-                if (mode == 1) rc = oracle_pair_checkpointed(x, n, Z_out, m, d, gamma, &vals[k], g);
-                else rc = oracle_pair_full(x, n, Z_out, m, d, gamma, &vals[k], g, NULL, NULL);
+                if (mode == 1) rc = oracle_pair_checkpointed_banded(x, n, Z_out, m, d, gamma, band, &vals[k], g);
+                else rc = oracle_pair_full_banded(x, n, Z_out, m, d, gamma, band, &vals[k], g, NULL, NULL);
             }
             free(x);
             if (rc != ORACLE_OK) {
@@ -396,12 +474,12 @@ int oracle_barycenter_f32(const float *Z0, int64_t m, int d, const float *X, con
         }
         if (rc_all != ORACLE_OK) break;
         double obj = 0.0;
-        for (int k = 0; k < N; ++k) obj += vals[k];
+        for (int k = 0; k < N; ++k) obj += (weights ? weights[k] : 1.0) * vals[k];
         if (objective) objective[it] = obj;
         if (values) memcpy(values, vals, (size_t)N * sizeof(double));
         for (int64_t t = 0; t < md; ++t) {
             double G = 0.0;
-            for (int k = 0; k < N; ++k) G += gk[(size_t)k * (size_t)md + t];
+            for (int k = 0; k < N; ++k) G += (weights ? weights[k] : 1.0) * gk[(size_t)k * (size_t)md + t];
             Z_out[t] -= step * G;
         }
     }

@@ -329,3 +329,114 @@ def test_barycenter_tiny_config_descends_and_matches_manual_loop(oracle):
     # the GD fixed point lowers the objective relative to the Euclidean-mean start
     vend, _ = oracle.value_grad(Z.astype(np.float32), data["X"], data["offsets"], cfg.gamma, want_grad=False)
     assert vend.sum() < obj[0]
+
+
+# ----------------------------------------------------------------------------- Sakoe-Chiba band (Table 1)
+def brute_force_banded(x, z, gamma, band):
+    """Soft-min over the complete alignment paths that stay inside |i - j| <= band (reading C18), by enumeration."""
+    D = sqdist(x, z)
+    n, m = D.shape
+    paths = [p for p in all_paths(n, m) if all(abs(i - j) <= band for i, j in p)]
+    costs = np.array([sum(D[i, j] for i, j in p) for p in paths])
+    cmin = costs.min()
+    w = np.exp(-(costs - cmin) / gamma)
+    value = cmin - gamma * math.log(w.sum())
+    E = np.zeros((n, m))
+    for pk, path in zip(w / w.sum(), paths):
+        for i, j in path:
+            E[i, j] += pk
+    return value, E, len(paths)
+
+
+@pytest.mark.parametrize("gamma", [1.0, 0.05])
+@pytest.mark.parametrize("shape_band", [((5, 5, 1), 0), ((5, 5, 2), 1), ((6, 6, 1), 2), ((6, 4, 1), 2), ((4, 6, 2), 2),
+                                        ((4, 6, 1), 3), ((6, 5, 1), 1), ((6, 6, 1), 5), ((1, 3, 1), 2), ((3, 1, 1), 2)])
+def test_band_brute_force_value_E_grad(oracle, gamma, shape_band):
+    (n, m, d), band = shape_band
+    rng = np.random.default_rng(77 * n + 7 * m + d + band)
+    x = rng.normal(size=(n, d))
+    z = rng.normal(size=(m, d))
+    v_bf, E_bf, npaths = brute_force_banded(x, z, gamma, band)
+    assert npaths >= 1
+    r = oracle.pair(x, z, gamma, want_E=True, want_R=True, band=band)
+    assert abs(r["value"] - v_bf) <= 1e-12 * max(1.0, abs(v_bf))
+    assert np.abs(r["E"] - E_bf).max() <= 1e-12
+    assert np.abs(r["grad"] - grad_from_E(E_bf, x, z)).max() <= 1e-11
+    # cells outside the band: r = +inf, E = 0 exactly
+    ii, jj = np.indices((n, m))
+    out = np.abs(ii - jj) > band
+    assert np.all(np.isinf(r["R"][1:n + 1, 1:m + 1][out])) and np.all(r["E"][out] == 0.0)
+    # checkpointed mode: same bits
+    rc = oracle.pair(x, z, gamma, mode="checkpointed", band=band)
+    assert rc["value"] == r["value"] and np.array_equal(rc["grad"], r["grad"])
+
+
+def test_band_limits_and_infeasible(oracle):
+    rng = np.random.default_rng(5)
+    n, m, d, gamma = 17, 13, 2, 0.3
+    x = rng.normal(size=(n, d))
+    z = rng.normal(size=(m, d))
+    free = oracle.pair(x, z, gamma, want_E=True)
+    wide = oracle.pair(x, z, gamma, want_E=True, band=max(n, m) - 1)       # every cell admissible
+    assert wide["value"] == free["value"] and np.array_equal(wide["E"], free["E"])
+    # a narrower band removes paths: the soft-min over fewer paths is larger (eq. 3-4), and monotone in the band
+    vals = [oracle.pair(x, z, gamma, want_grad=False, band=b)["value"] for b in range(n - m, n)]
+    assert all(a >= b - 1e-12 for a, b in zip(vals, vals[1:])) and vals[0] > free["value"]
+    # band 0 with n == m leaves the single diagonal path: value = trace(D), E = I, g_j = 2 (z_j - x_j)
+    xs = rng.normal(size=(9, d))
+    zs = rng.normal(size=(9, d))
+    r0 = oracle.pair(xs, zs, gamma, want_E=True, band=0)
+    assert abs(r0["value"] - np.trace(sqdist(xs, zs))) < 1e-12
+    assert np.abs(r0["E"] - np.eye(9)).max() < 1e-12 and np.abs(r0["grad"] - 2 * (zs - xs)).max() < 1e-11
+    # |n - m| > band: no complete path inside the band -> rejected
+    with pytest.raises(RuntimeError):
+        oracle.pair(x, z, gamma, band=n - m - 1)
+    # finite differences of the banded value
+    band = 6
+    g = oracle.pair(x, z, gamma, band=band)["grad"]
+    for (j, c) in [(0, 0), (5, 1), (12, 0)]:
+        h = 1e-6
+        zp, zm = z.copy(), z.copy()
+        zp[j, c] += h
+        zm[j, c] -= h
+        fd = (oracle.pair(x, zp, gamma, want_grad=False, band=band)["value"] -
+              oracle.pair(x, zm, gamma, want_grad=False, band=band)["value"]) / (2 * h)
+        assert abs(fd - g[j, c]) <= 1e-6 * max(1.0, abs(g[j, c]))
+
+
+# ----------------------------------------------------------------------------- eq. 7 weights lambda_k / n_k
+def test_weighted_objective_and_gradient(oracle):
+    rng = np.random.default_rng(21)
+    d, m, gamma = 2, 12, 0.4
+    lens = [9, 15, 12, 7]
+    X = rng.normal(size=(sum(lens), d)).astype(np.float32)
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    Z = rng.normal(size=(m, d)).astype(np.float32)
+    lam = np.array([1.0, 0.5, 2.0, 1.5])
+    w = lam / np.array(lens)                                    # eq. 7: lambda_i / m_i
+    vals, G, obj = oracle.value_grad(Z, X, off, gamma, weights=w, want_objective=True)
+    vals1, _ = oracle.value_grad(Z, X, off, gamma)
+    assert np.array_equal(vals, vals1)                          # per-pair values stay unweighted
+    Gs = np.zeros_like(G)
+    for k in range(4):
+        r = oracle.pair(X[off[k]:off[k + 1]].astype(np.float64), Z.astype(np.float64), gamma)
+        Gs += w[k] * r["grad"]
+    assert np.abs(G - Gs).max() < 1e-13 and abs(obj - float(w @ vals)) < 1e-13
+    # all-ones weights == the unweighted call, bitwise
+    v2, G2 = oracle.value_grad(Z, X, off, gamma, weights=np.ones(4))
+    _, G3 = oracle.value_grad(Z, X, off, gamma)
+    assert np.array_equal(G2, G3)
+    # finite differences of the weighted objective
+    for (j, c) in [(0, 1), (6, 0), (11, 1)]:
+        h = 1e-3                                                # Z is fp32 at this interface: exact fp32 steps
+        Zp, Zm = Z.copy(), Z.copy()
+        Zp[j, c] += np.float32(h)
+        Zm[j, c] -= np.float32(h)
+        op = oracle.value_grad(Zp, X, off, gamma, want_grad=False, weights=w, want_objective=True)[2]
+        om = oracle.value_grad(Zm, X, off, gamma, want_grad=False, weights=w, want_objective=True)[2]
+        fd = (op - om) / (float(Zp[j, c]) - float(Zm[j, c]))
+        assert abs(fd - G[j, c]) <= 2e-5 * max(1.0, abs(G[j, c]))
+    # descent on the weighted, banded objective: first update = Z0 - step * weighted gradient
+    Z1, _, o1 = oracle.barycenter(Z, X, off, gamma, 1, 0.05, weights=w, band=8)
+    vb, Gb, ob = oracle.value_grad(Z, X, off, gamma, weights=w, band=8, want_objective=True)
+    assert np.abs(Z1 - (Z.astype(np.float64) - 0.05 * Gb)).max() < 1e-15 and abs(o1[0] - ob) < 1e-13
