@@ -72,6 +72,29 @@ int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat,
                     float gamma, int32_t iters, float step, float* out_values, float* out_objective, void* stream);
 
 /*
+ * Extended calls: the paper's variants of the same path (Def. 7 / eq. 7, l.187-192; Table 1, l.318-319).
+ *   weights  HOST [N] float32 or NULL.  w_k multiplies pair k in the objective and in the gradient:
+ *            objective = sum_k w_k value_k,  out_grad = sum_k w_k g_k  (eq. 7 has w_k = lambda_k / n_k; NULL = all 1, the
+ *            plain sum of sdtw_value_grad).  out_values[k] stay the UNWEIGHTED Soft-DTW values.  Read during the call
+ *            only.  Non-finite weight => SDTW_ERR_INVALID_ARG.
+ *   band     Sakoe-Chiba band (Table 1 "Bandwidth", a fraction of the longest length: the caller passes
+ *            band = floor(0.6 * max(m, max_k n_k)) for the paper's setting).  Read (C18) as the classic
+ *            adjustment window: cell (i, j) belongs to an admissible path iff |i - j| <= band; cells outside are
+ *            excluded from eq. 5 (r = +inf) and have E = 0.  band < 0 = no band.
+ *            band < |n_k - m| for some k => SDTW_ERR_INVALID_ARG (no complete path fits).  A band that excludes cells
+ *            of pair k but is narrower than |n_k - m| + 4 (ceil(n_k / m) + 2) + 2 => SDTW_ERR_UNSUPPORTED (the kernel's
+ *            value staircase must fit inside the band).
+ *   out_objective  dev [1] (value_grad_ex) / dev [iters] (barycenter_ex) float32, sum_k w_k value_k; may be NULL.
+ * Everything else is as in sdtw_value_grad / sdtw_barycenter, which are these calls with weights = NULL, band = -1.
+ */
+int sdtw_value_grad_ex(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                       float gamma, const float* weights, int64_t band, float* out_values, float* out_grad,
+                       float* out_objective, void* stream);
+int sdtw_barycenter_ex(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                       float gamma, const float* weights, int64_t band, int32_t iters, float step, float* out_values,
+                       float* out_objective, void* stream);
+
+/*
  * sdtw_gd_update -- the descent step alone: Z[t] <- Z[t] - step * G[t] for t < count (= m*d).  Used when the
  * gradient is all-reduced across GPUs between sdtw_value_grad and the update.
  */

@@ -23,6 +23,8 @@ _i64p = ctypes.POINTER(ctypes.c_int64)
 SYMBOLS = {
     "sdtw_value_grad": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_barycenter": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _i32, _f32, _vp, _vp, _vp]),
+    "sdtw_value_grad_ex": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _i64, _vp, _vp, _vp, _vp]),
+    "sdtw_barycenter_ex": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _i64, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_gd_update": (ctypes.c_int, [_vp, _vp, _i64, _f32, _vp]),
     "sdtw_value_grad_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_barycenter_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _i32, _f32, _vp, _vp, _vp]),
@@ -125,6 +127,68 @@ def sdtw_barycenter(Z_inout, X_concat, offsets, gamma, iters, step, out_values=N
     with torch.cuda.device(Z.device):
         _check(_lib.sdtw_barycenter(_ptr(Z), m, d, _ptr(X), offp, N, float(gamma), int(iters), float(step),
                                     _ptr(out_values), _ptr(out_objective) if iters > 0 else None, _stream(stream)))
+    return Z, out_values, out_objective
+
+
+def _weights(weights, N):
+    if weights is None:
+        return None, None
+    w = np.ascontiguousarray(np.asarray(weights, dtype=np.float32))
+    if w.shape != (N,):
+        raise ValueError("weights must have one entry per pair")
+    return w, ctypes.c_void_p(w.ctypes.data)
+
+
+def eq7_weights(lengths, lam=None):
+    """w_k = lambda_k / n_k of eq. 7; lambda defaults to 1."""
+    n = np.asarray(lengths, np.float64)
+    return ((1.0 if lam is None else np.asarray(lam, np.float64)) / n).astype(np.float32)
+
+
+def table1_band(m, lengths, fraction=0.6):
+    """Table 1's Sakoe-Chiba bandwidth: a fraction of the longest signal length, in cells."""
+    return int(np.floor(fraction * max(int(m), int(np.max(lengths)))))
+
+
+def sdtw_value_grad_ex(Z, X_concat, offsets, gamma, weights=None, band=-1, out_values=None, out_grad=None,
+                       out_objective=None, want_grad=True, stream=None):
+    """sdtw_value_grad with eq. 7 weights (host array, one per pair) and a Sakoe-Chiba band (include/sdtw.h).
+    Returns (values, grad or None, objective[1])."""
+    import torch
+    Z = _dev_f32(Z, "Z")
+    X = _dev_f32(X_concat, "X_concat")
+    m, d = _dims(Z)
+    off, offp, N = _offsets(offsets)
+    w, wp = _weights(weights, N)
+    if out_values is None:
+        out_values = torch.empty(N, dtype=torch.float32, device=Z.device)
+    if want_grad and out_grad is None:
+        out_grad = torch.empty_like(Z)
+    if out_objective is None:
+        out_objective = torch.zeros(1, dtype=torch.float32, device=Z.device)
+    with torch.cuda.device(Z.device):
+        _check(_lib.sdtw_value_grad_ex(_ptr(Z), m, d, _ptr(X), offp, N, float(gamma), wp, int(band), _ptr(out_values),
+                                       _ptr(out_grad) if want_grad else None, _ptr(out_objective), _stream(stream)))
+    return out_values, (out_grad if want_grad else None), out_objective
+
+
+def sdtw_barycenter_ex(Z_inout, X_concat, offsets, gamma, iters, step, weights=None, band=-1, out_values=None,
+                       out_objective=None, stream=None):
+    """sdtw_barycenter on eq. 7's weighted objective with an optional band.  Returns (Z_inout, values, objective)."""
+    import torch
+    Z = _dev_f32(Z_inout, "Z_inout")
+    X = _dev_f32(X_concat, "X_concat")
+    m, d = _dims(Z)
+    off, offp, N = _offsets(offsets)
+    w, wp = _weights(weights, N)
+    if out_values is None:
+        out_values = torch.zeros(N, dtype=torch.float32, device=Z.device)
+    if out_objective is None:
+        out_objective = torch.zeros(max(int(iters), 0), dtype=torch.float32, device=Z.device)
+    with torch.cuda.device(Z.device):
+        _check(_lib.sdtw_barycenter_ex(_ptr(Z), m, d, _ptr(X), offp, N, float(gamma), wp, int(band), int(iters),
+                                       float(step), _ptr(out_values), _ptr(out_objective) if iters > 0 else None,
+                                       _stream(stream)))
     return Z, out_values, out_objective
 
 

@@ -131,19 +131,24 @@ struct Plan {
     int32_t d = 0, N = 0;
     bool want_grad = false;
     std::vector<int64_t> offsets;
+    std::vector<float> weights;   // caller order; empty = unweighted
+    std::vector<float> weights_sched;   // schedule order (source of the upload; lives as long as the plan)
     Layout L;
     PairMeta* d_pm = nullptr;
+    float* d_w = nullptr;         // weights in schedule order (null when unweighted)
     cudaEvent_t uploaded = nullptr;
     uint64_t stamp = 0;
 };
 std::vector<Plan*> g_plans;
 uint64_t g_stamp = 0;
 
-int get_plan(int dev, int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, cudaStream_t stream,
-             Plan** out) {
+int get_plan(int dev, int64_t m, int32_t d, const int64_t* offsets, int32_t N, const float* weights, bool want_grad,
+             cudaStream_t stream, Plan** out) {
     for (Plan* pl : g_plans) {
         if (pl->dev == dev && pl->m == m && pl->d == d && pl->N == N && pl->want_grad == want_grad &&
-            std::memcmp(pl->offsets.data(), offsets, sizeof(int64_t) * (size_t)(N + 1)) == 0) {
+            std::memcmp(pl->offsets.data(), offsets, sizeof(int64_t) * (size_t)(N + 1)) == 0 &&
+            (weights ? (!pl->weights.empty() && std::memcmp(pl->weights.data(), weights, sizeof(float) * (size_t)N) == 0)
+                     : pl->weights.empty())) {
             pl->stamp = ++g_stamp;
             CUDA_TRY(cudaStreamWaitEvent(stream, pl->uploaded, 0));
             *out = pl;
@@ -157,11 +162,19 @@ int get_plan(int dev, int64_t m, int32_t d, const int64_t* offsets, int32_t N, b
     pl->offsets.assign(offsets, offsets + N + 1);
     cudaError_t e = cudaMalloc(&pl->d_pm, sizeof(PairMeta) * (size_t)N);
     if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_pm, pl->L.pm.data(), sizeof(PairMeta) * (size_t)N, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess && weights) {                 // eq. 7 weights, permuted to schedule order
+        pl->weights.assign(weights, weights + N);
+        pl->weights_sched.resize((size_t)N);
+        for (int ps = 0; ps < N; ++ps) pl->weights_sched[ps] = weights[pl->L.pm[ps].k];
+        e = cudaMalloc(&pl->d_w, sizeof(float) * (size_t)N);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_w, pl->weights_sched.data(), sizeof(float) * (size_t)N, cudaMemcpyHostToDevice, stream);
+    }
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pl->uploaded, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventRecord(pl->uploaded, stream);
     if (e != cudaSuccess) {
         g_last_cuda_error = (int)e;
         if (pl->d_pm) cudaFree(pl->d_pm);
+        if (pl->d_w) cudaFree(pl->d_w);
         delete pl;
         return SDTW_ERR_CUDA;
     }
@@ -169,6 +182,7 @@ int get_plan(int dev, int64_t m, int32_t d, const int64_t* offsets, int32_t N, b
     if (g_plans.size() >= 8) {   // evict the least recently used plan
         auto it = std::min_element(g_plans.begin(), g_plans.end(), [](Plan* a, Plan* b) { return a->stamp < b->stamp; });
         cudaFree((*it)->d_pm);
+        if ((*it)->d_w) cudaFree((*it)->d_w);
         cudaEventDestroy((*it)->uploaded);
         delete *it;
         g_plans.erase(it);
@@ -254,7 +268,7 @@ int dispatch_backward(int d, const Params& P, int sms, cudaStream_t s) {
 bool finite_pos(float g) { return std::isfinite(g) && g > 0.f; }
 
 // one evaluation: values (+ gradient) at Z.  If Z_update != nullptr the descent step is fused into the reduction.
-int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, const float* X, float gamma,
+int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, const float* X, float gamma, int band,
              float* out_values, float* out_objective, float* out_grad, float* Z_update, float step, cudaStream_t stream) {
     const Layout& L = pl.L;
     Params P{};
@@ -270,6 +284,8 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     P.Gk = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_Gk) : nullptr;
     P.stats = reinterpret_cast<unsigned long long*>(ws + L.off_stats);
     P.dense_reverse = g_dense_reverse;
+    P.band = band;
+    P.wts = pl.d_w;
     g_last_stats = P.stats;
     P.m = (int)pl.m; P.N = pl.N; P.NS = L.NS;
     P.num_items = (unsigned)L.items;
@@ -302,14 +318,14 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     }
     if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[3], stream));
     if (out_values || out_objective) {
-        finalize_values_kernel<<<1, 256, 0, stream>>>(P.VP, pl.d_pm, pl.N, L.NS, inv_kappa, out_values, out_objective);
+        finalize_values_kernel<<<1, 256, 0, stream>>>(P.VP, pl.d_pm, P.wts, pl.N, L.NS, inv_kappa, out_values, out_objective);
         ++g_launches;
         CUDA_TRY(cudaGetLastError());
     }
     if (pl.want_grad) {
         const long long md = (long long)pl.m * pl.d;
         const int blocks = (int)((md + 255) / 256);
-        reduce_pairs_kernel<<<blocks, 256, 0, stream>>>(P.Gk, pl.N, md, out_grad, Z_update, step);
+        reduce_pairs_kernel<<<blocks, 256, 0, stream>>>(P.Gk, P.wts, pl.N, md, out_grad, Z_update, step);
         ++g_launches;
         CUDA_TRY(cudaGetLastError());
     }
@@ -326,6 +342,30 @@ int check_common(const void* Z, int64_t m, int32_t d, const void* X, const int64
     for (int k = 0; k < N; ++k)
         if (offsets[k + 1] <= offsets[k]) return SDTW_ERR_INVALID_ARG;
     if (d > SDTW_MAX_D) return SDTW_ERR_UNSUPPORTED;
+    return SDTW_OK;
+}
+
+// Extended arguments (eq. 7 weights, Table 1 band).  *band_eff: -1 when the band excludes no cell of any pair.
+int check_ex(int64_t m, const int64_t* offsets, int32_t N, const float* weights, int64_t band, int* band_eff) {
+    if (weights)
+        for (int k = 0; k < N; ++k)
+            if (!std::isfinite(weights[k])) return SDTW_ERR_INVALID_ARG;
+    *band_eff = -1;
+    if (band < 0) return SDTW_OK;
+    bool excludes = false, narrow = false;
+    for (int k = 0; k < N; ++k) {
+        const int64_t n = offsets[k + 1] - offsets[k];
+        const int64_t gap = n > m ? n - m : m - n;
+        if (band < gap) return SDTW_ERR_INVALID_ARG;          // no complete alignment path inside the band
+        if (band >= std::max(n, m) - 1) continue;             // every cell of this pair is admissible
+        excludes = true;
+        // the value staircase (sdtw_kernels.cuh) strays at most W columns / W ceil(n/m) rows from the line
+        // i = j n / m, which itself stays within |i - j| <= |n - m|
+        const int64_t need = gap + (int64_t)W * ((n + m - 1) / m + 2) + 2;
+        if (band < need) narrow = true;
+    }
+    if (narrow) return SDTW_ERR_UNSUPPORTED;
+    if (excludes) *band_eff = (int)std::min<int64_t>(band, (1LL << 30));
     return SDTW_OK;
 }
 
@@ -371,9 +411,13 @@ struct Workspace {
 // =================================================================================================================
 extern "C" {
 
-int sdtw_value_grad(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
-                    float gamma, float* out_values, float* out_grad, void* stream_) {
+int sdtw_value_grad_ex(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                       float gamma, const float* weights, int64_t band, float* out_values, float* out_grad,
+                       float* out_objective, void* stream_) {
     int rc = check_common(Z, m, d, X_concat, offsets, N, gamma);
+    if (rc) return rc;
+    int band_eff = -1;
+    rc = check_ex(m, offsets, N, weights, band, &band_eff);
     if (rc) return rc;
     std::lock_guard<std::mutex> lock(g_mutex);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
@@ -381,19 +425,28 @@ int sdtw_value_grad(const float* Z, int64_t m, int32_t d, const float* X_concat,
     rc = get_device(di);
     if (rc) return rc;
     Plan* pl = nullptr;
-    rc = get_plan(di.dev, m, d, offsets, N, out_grad != nullptr, stream, &pl);
+    rc = get_plan(di.dev, m, d, offsets, N, weights, out_grad != nullptr, stream, &pl);
     if (rc) return rc;
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
     if (rc) return rc;
-    return evaluate(*pl, ws.ptr, di, Z, X_concat, gamma, out_values, nullptr, out_grad, nullptr, 0.f, stream);
+    return evaluate(*pl, ws.ptr, di, Z, X_concat, gamma, band_eff, out_values, out_objective, out_grad, nullptr, 0.f, stream);
 }
 
-int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
-                    float gamma, int32_t iters, float step, float* out_values, float* out_objective, void* stream_) {
+int sdtw_value_grad(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                    float gamma, float* out_values, float* out_grad, void* stream_) {
+    return sdtw_value_grad_ex(Z, m, d, X_concat, offsets, N, gamma, nullptr, -1, out_values, out_grad, nullptr, stream_);
+}
+
+int sdtw_barycenter_ex(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                       float gamma, const float* weights, int64_t band, int32_t iters, float step, float* out_values,
+                       float* out_objective, void* stream_) {
     int rc = check_common(Z_inout, m, d, X_concat, offsets, N, gamma);
     if (rc) return rc;
     if (iters < 0 || !std::isfinite(step)) return SDTW_ERR_INVALID_ARG;
+    int band_eff = -1;
+    rc = check_ex(m, offsets, N, weights, band, &band_eff);
+    if (rc) return rc;
     std::lock_guard<std::mutex> lock(g_mutex);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     DeviceInfo di;
@@ -401,7 +454,7 @@ int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat,
     if (rc) return rc;
     if (iters == 0) return SDTW_OK;
     Plan* pl = nullptr;
-    rc = get_plan(di.dev, m, d, offsets, N, true, stream, &pl);
+    rc = get_plan(di.dev, m, d, offsets, N, weights, true, stream, &pl);
     if (rc) return rc;
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
@@ -409,10 +462,16 @@ int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat,
     for (int it = 0; it < iters; ++it) {
         float* vals = (it == iters - 1) ? out_values : nullptr;
         float* obj = out_objective ? out_objective + it : nullptr;
-        rc = evaluate(*pl, ws.ptr, di, Z_inout, X_concat, gamma, vals, obj, nullptr, Z_inout, step, stream);
+        rc = evaluate(*pl, ws.ptr, di, Z_inout, X_concat, gamma, band_eff, vals, obj, nullptr, Z_inout, step, stream);
         if (rc) return rc;
     }
     return SDTW_OK;
+}
+
+int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                    float gamma, int32_t iters, float step, float* out_values, float* out_objective, void* stream_) {
+    return sdtw_barycenter_ex(Z_inout, m, d, X_concat, offsets, N, gamma, nullptr, -1, iters, step, out_values,
+                              out_objective, stream_);
 }
 
 int sdtw_gd_update(float* Z_inout, const float* G, int64_t count, float step, void* stream_) {

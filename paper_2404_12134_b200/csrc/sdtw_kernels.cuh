@@ -93,6 +93,8 @@ struct Params {
     unsigned long long* stats;  // [0] reverse chunks visited, [1] reverse chunks skipped (instrumentation; may be null)
     int dense_reverse;    // 1: never skip a reverse chunk (for measurement / validation of the exact skip)
     int unit_strips;      // forward schedule: adjacent strips of one pair per unit (1 .. warps per CTA)
+    int band;             // Sakoe-Chiba band (Table 1): cell (i, j) admissible iff |i - j| <= band; < 0: none
+    const float* wts;     // [N] per-pair weights of eq. 7 in schedule order, or null (all 1)
     float gscale;         // 2 / sqrt(kappa)
 };
 
@@ -222,6 +224,16 @@ struct SlowTag { static constexpr bool slow = true; };
 // chunk c (steps c CH .. c CH + CH-1, rows c CROWS - SKEW .. c CROWS + CROWS-1 over the 32 lanes) touches only valid rows
 __device__ __forceinline__ bool interior_chunk(int c, int n) { return c * CROWS >= SKEW && c * CROWS + CROWS <= n; }
 
+// Sakoe-Chiba band in the difference form.  The band |i - j| <= r is closed under diagonal moves, so an admissible cell's
+// diagonal predecessor is admissible (or the border) and only two overrides are needed: on the upper edge (j - i == r) the
+// "up" predecessor is outside the band, h_in = +inf; on the lower edge (i - j == r) the "left" one is, v_in = +inf.  Their
+// transition weights are then exactly 0 (2^-BIG = 0), so E never leaves the band either.  Cells outside the band compute
+// finite values nobody uses.  A (chunk, strip) block needs the overrides only if it can contain an edge cell:
+__device__ __forceinline__ bool band_clear(int c, int J, int band) {
+    const int lo = c * CROWS - SKEW, hi = c * CROWS + CROWS - 1, jl = J * SW, jh = jl + SW - 1;
+    return band < 0 || (hi - jl < band && jh - lo < band);
+}
+
 // ------------------------------------------------------------------------------------------------------------------
 // prologue: the scaled copies of the inputs the two wavefront kernels read
 __global__ void scale_inputs_kernel(const float* __restrict__ X, long long nx, const float* __restrict__ Z, long long nz,
@@ -336,6 +348,7 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
         const int c_v1 = (__reduce_max_sync(FULL, max(r_h, r_v1)) / RP + 31) / CH;
 
         const float* xs_lane = xs0;                        // set per chunk
+        const int band = p.band;
         // general row: all W cells of row i, plus this thread's piece of the value staircase
         auto slow_row = [&](const int i, const XRow<D>& x, float& v) {
             float vfirst = 0.f, dummy0, dummy1;
@@ -343,6 +356,10 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
             for (int w = 0; w < W; ++w) {
                 float tl, acc;
                 sqdist2<D>(x, z[w], tl, acc);
+                if (band >= 0) {                           // band edges: the predecessor outside the band counts as +inf
+                    if (j0 + w - i == band) h[w] = BIG;
+                    if (i - (j0 + w) == band) v = BIG;
+                }
                 cell<false, (D > 1)>(tl, acc, h[w], v, dummy0, dummy1);
                 if (w == 0) vfirst = v;
             }
@@ -429,7 +446,7 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
                 if (J > 0) vreg = ld_relaxed_f2(VSprev + rbase + CROWS);
             }
             xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;    // rows of step t: xs_lane[2t], [2t+1]
-            if (interior_chunk(c, n) && (c < c_v0 || c > c_v1)) {
+            if (interior_chunk(c, n) && (c < c_v0 || c > c_v1) && band_clear(c, J, band)) {
 #pragma unroll 1
                 for (int b = 0; b < CH / TR; ++b) {
 #pragma unroll
@@ -486,6 +503,7 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
         const int item = ps * p.NS + J;
         const int j0 = (J * 32 + lane) * W;
         const bool has_right = (J < p.NS - 1);
+        const int band = p.band;
         const float* VSprev = p.VS + pm.vs_off + (long long)(J - 1) * pm.vs_stride + VS_PAD;
         float* ESme = p.ES + pm.vs_off + (long long)J * pm.vs_stride + VS_PAD;   // indexed by row
         const float* ESnext = ESme + pm.vs_stride;
@@ -516,11 +534,15 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
         prefetch(C * BPC - 1);
 
         // one row of the recompute, keeping the transition weights
-        auto rec_row = [&](const XRow<D>& x, float& v, const int slot) {
+        auto rec_row = [&](const int i, const XRow<D>& x, float& v, const int slot) {
 #pragma unroll
             for (int w = 0; w < W; ++w) {
                 float tl, acc, wu, wl;
                 sqdist2<D>(x, z[w], tl, acc);
+                if (band >= 0) {                              // band edges, as in the forward kernel
+                    if (j0 + w - i == band) h[w] = BIG;
+                    if (i - (j0 + w) == band) v = BIG;
+                }
                 cell<true, (D > 1)>(tl, acc, h[w], v, wu, wl);
                 stash[(slot * W + w) * 32] = make_float2(wu, wl);
             }
@@ -546,8 +568,8 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
                 vp0 = va; vp1 = vb;
             } else {
                 const int i0 = RP * (c * CH + t - lane);
-                if ((unsigned)i0 < (unsigned)n) { rec_row(xa, va, u * RP + 0); vp0 = va; }
-                if ((unsigned)(i0 + 1) < (unsigned)n) { rec_row(xb, vb, u * RP + 1); vp1 = vb; }
+                if ((unsigned)i0 < (unsigned)n) { rec_row(i0, xa, va, u * RP + 0); vp0 = va; }
+                if ((unsigned)(i0 + 1) < (unsigned)n) { rec_row(i0 + 1, xb, vb, u * RP + 1); vp1 = vb; }
             }
         };
         // E recurrence of one row, right to left: E_in = flow into the last column's cell from the right neighbour;
@@ -627,7 +649,7 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
             }
             cp_async_wait_all();
             __syncwarp();
-            const bool fast = interior_chunk(c, n);
+            const bool fast = interior_chunk(c, n) && band_clear(c, J, band);
 #pragma unroll 1
             for (int b = BPC - 1; b >= 0; --b) {
                 const int bidx = c * BPC + b, t0 = b * TR;
@@ -677,7 +699,8 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
 
 // ------------------------------------------------------------------------------------------------------------------
 // small kernels: per-pair values from the item partials, objective, reduction over pairs, descent step
-__global__ void finalize_values_kernel(const double* __restrict__ VP, const PairMeta* __restrict__ pm, int N, int NS,
+__global__ void finalize_values_kernel(const double* __restrict__ VP, const PairMeta* __restrict__ pm,
+                                       const float* __restrict__ wts, int N, int NS,
                                        double inv_kappa, float* __restrict__ out_values, float* __restrict__ out_objective) {
     __shared__ double red[256];
     double local = 0.0;
@@ -686,7 +709,7 @@ __global__ void finalize_values_kernel(const double* __restrict__ VP, const Pair
         for (int J = 0; J < NS; ++J) s += VP[(long long)ps * NS + J];
         s *= inv_kappa;
         if (out_values) out_values[pm[ps].k] = (float)s;
-        local += s;
+        local += wts ? (double)wts[ps] * s : s;              // eq. 7: objective = sum_k w_k value_k
     }
     // objective: fixed-shape tree over the block (deterministic)
     red[threadIdx.x] = local;
@@ -699,12 +722,13 @@ __global__ void finalize_values_kernel(const double* __restrict__ VP, const Pair
 }
 
 // G[e] = sum over pairs (schedule order, fp64 accumulator: deterministic, no atomics); optional descent step
-__global__ void reduce_pairs_kernel(const float* __restrict__ Gk, int N, long long md, float* __restrict__ out_grad,
-                                    float* __restrict__ Z, float step) {
+__global__ void reduce_pairs_kernel(const float* __restrict__ Gk, const float* __restrict__ wts, int N, long long md,
+                                    float* __restrict__ out_grad, float* __restrict__ Z, float step) {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= md) return;
     double acc = 0.0;
-    for (int ps = 0; ps < N; ++ps) acc += (double)Gk[(long long)ps * md + e];
+    if (wts) { for (int ps = 0; ps < N; ++ps) acc += (double)wts[ps] * (double)Gk[(long long)ps * md + e]; }
+    else     { for (int ps = 0; ps < N; ++ps) acc += (double)Gk[(long long)ps * md + e]; }
     const float gsum = (float)acc;
     if (out_grad) out_grad[e] = gsum;
     if (Z) Z[e] = Z[e] - step * gsum;

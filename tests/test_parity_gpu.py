@@ -316,3 +316,105 @@ def test_full_size_cfg3_cfg4_cfg5_sampled_against_oracle(B, oracle):
             assert e <= 1e-5
         del Z, X, vals, G
         torch.cuda.empty_cache()
+
+
+# ------------------------------------------------------------------------------------------- eq. 7 weights, Table 1 band
+@pytest.mark.parametrize("idx,scale,N,frac", [(2, 1.0, 12, 0.6), (2, 1.0, 12, 0.25), (3, 0.1, 5, 0.6), (4, 0.1, 8, 0.6),
+                                              (4, 0.1, 8, 0.3), (4, 0.2, 3, 0.35)])
+def test_band_and_weights_value_grad(B, oracle, idx, scale, N, frac):
+    """sdtw_value_grad_ex against the banded / weighted oracle: Sakoe-Chiba band |i - j| <= frac * longest length
+    (Table 1; 0.6 is the paper's value) and w_k = lambda_k / n_k (eq. 7)."""
+    import torch
+    cfg = synth.scaled(synth.CONFIGS[idx], scale, N=N)
+    data = synth.make(cfg)
+    lens = data["lengths"]
+    band = B.table1_band(cfg.m, lens, frac)
+    assert band >= np.abs(lens - cfg.m).max() and band < min(cfg.m, lens.min()) - 1      # feasible, and it excludes cells
+    rng = np.random.default_rng(idx)
+    w = B.eq7_weights(lens, lam=rng.uniform(0.5, 2.0, size=N))
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    vals, G, obj = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, weights=w, band=band)
+    torch.cuda.synchronize()
+    ov, oG, oobj = oracle.value_grad(data["Z0"], data["X"], data["offsets"], cfg.gamma, mode="checkpointed",
+                                     weights=w.astype(np.float64), band=band, want_objective=True)
+    check_values(vals.cpu().numpy(), ov, lens, cfg, f"{cfg.name} band {band}")
+    e = rel_l2(G.cpu().numpy(), oG)
+    print(f"[{cfg.name} band {band} ({frac} x longest), weighted] gradient rel L2 {e:.3e}; objective {obj.item():.6f} vs {oobj:.6f}")
+    assert e <= GRAD_TOL
+    assert abs(obj.item() - oobj) <= 1e-4 * max(abs(oobj), float(np.sum(np.abs(w) * cfg.gamma * (lens + cfg.m))))
+    # the band changes the result (it is not silently ignored), and a band that excludes nothing changes no bit
+    v_free, g_free = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+    v_all, g_all, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=int(max(cfg.m, lens.max())))
+    assert torch.equal(v_free, v_all) and torch.equal(g_free, g_all)
+    ov_free, _ = oracle.value_grad(data["Z0"], data["X"], data["offsets"], cfg.gamma, want_grad=False, mode="checkpointed")
+    assert np.all(ov >= ov_free - 1e-9)                       # fewer paths -> larger soft-min (eq. 3-4)
+    # forward-only banded sweep computes the same values
+    vf, none, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band, want_grad=False)
+    assert none is None and torch.equal(vf, vals)
+
+
+def test_band_barycenter_weighted_descent(B, oracle):
+    cfg = synth.scaled(synth.CONFIGS[4], 0.1, N=8)
+    data = synth.make(cfg)
+    lens = data["lengths"]
+    band = B.table1_band(cfg.m, lens, 0.6)
+    w = B.eq7_weights(lens)
+    step = 0.02 / cfg.N * float(np.mean(lens))                # eq. 7 divides by n_k: rescale the step accordingly
+    iters = 3
+    Z, vals, obj = B.sdtw_barycenter_ex(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, iters, step,
+                                        weights=w, band=band)
+    Zo, vo, oo = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, iters, step, mode="checkpointed",
+                                   weights=w.astype(np.float64), band=band)
+    e = rel_l2(Z.cpu().numpy(), Zo)
+    moved = np.linalg.norm(Z.cpu().numpy() - Zo) / np.linalg.norm(Zo - data["Z0"])
+    print(f"[{cfg.name} band {band}, eq. 7 weights] barycenter rel L2 {e:.3e}, relative to distance moved {moved:.3e}; objective {oo}")
+    assert e <= BARY_TOL and moved <= 5e-2
+    assert np.allclose(obj.cpu().numpy(), oo, rtol=1e-4, atol=1e-4 * cfg.gamma * 2)
+    check_values(vals.cpu().numpy(), vo, lens, cfg, "banded weighted barycenter values")
+
+
+def test_band_argument_errors(B):
+    import torch
+    data = synth.make(2)
+    cfg = data["cfg"]
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    gap = int(np.abs(data["lengths"] - cfg.m).max())
+    vals = torch.full((cfg.N,), 7.0, device="cuda")
+    G = torch.full_like(Z, 7.0)
+    with pytest.raises(B.SdtwError) as ei:                    # no complete path fits
+        B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=gap - 1, out_values=vals, out_grad=G)
+    assert ei.value.status == B.SDTW_ERR_INVALID_ARG
+    with pytest.raises(B.SdtwError) as ei:                    # feasible but narrower than the kernel's value staircase
+        B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=gap + 1, out_values=vals, out_grad=G)
+    assert ei.value.status == B.SDTW_ERR_UNSUPPORTED
+    w = np.ones(cfg.N, np.float32)
+    w[3] = np.nan
+    with pytest.raises(B.SdtwError) as ei:
+        B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, weights=w, out_values=vals, out_grad=G)
+    assert ei.value.status == B.SDTW_ERR_INVALID_ARG
+    torch.cuda.synchronize()
+    assert float(vals.min()) == 7.0 and float(G.min()) == 7.0
+
+
+@pytest.mark.parametrize("n_lo,n_hi,m,d,gamma,band", [(990, 1010, 1000, 1, 0.1, 40), (990, 1010, 1000, 1, 0.1, 80),
+                                                      (480, 520, 500, 2, 1.0, 50), (560, 560, 500, 1, 0.1, 80),
+                                                      (500, 500, 560, 2, 0.5, 76), (420, 424, 400, 1, 0.2, 45)])
+def test_band_that_matters(B, oracle, n_lo, n_hi, m, d, gamma, band):
+    """Warped cycles against a band narrow enough to cut their alignment (longer and shorter than m, d = 1..2): value
+    and gradient visibly depend on the band, so a kernel that ignored it, or put its edge one cell off, fails here."""
+    import torch
+    cfg = dataclasses.replace(synth.CONFIGS[2], N=6, n_lo=n_lo, n_hi=n_hi, m=m, d=d, gamma=gamma, name=f"band{band}")
+    data = synth.make(cfg, seed=band)
+    lens = data["lengths"]
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    vals, G, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], gamma, band=band)
+    ov, oG = oracle.value_grad(data["Z0"], data["X"], data["offsets"], gamma, band=band, mode="checkpointed")
+    ov_free, oG_free = oracle.value_grad(data["Z0"], data["X"], data["offsets"], gamma, mode="checkpointed")
+    ov_off, oG_off = oracle.value_grad(data["Z0"], data["X"], data["offsets"], gamma, band=band + 1, mode="checkpointed")
+    den = np.maximum(np.abs(ov), gamma * (lens + m))
+    assert (np.abs(ov - ov_free) / den).max() > 5 * VAL_TOL             # the band matters on this input
+    check_values(vals.cpu().numpy(), ov, lens, cfg, cfg.name)
+    e = rel_l2(G.cpu().numpy(), oG)
+    print(f"[{cfg.name}] gradient rel L2 {e:.3e} (unbanded oracle differs by {rel_l2(oG_free, oG):.3e}, band+1 by {rel_l2(oG_off, oG):.3e})")
+    assert e <= GRAD_TOL and rel_l2(oG_free, oG) > 10 * GRAD_TOL
+    assert rel_l2(oG_off, oG) > 2 * GRAD_TOL                            # ... and so does a one-cell shift of its edge
