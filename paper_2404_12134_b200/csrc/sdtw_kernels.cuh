@@ -234,6 +234,17 @@ __device__ __forceinline__ bool band_clear(int c, int J, int band) {
     return band < 0 || (hi - jl < band && jh - lo < band);
 }
 
+// Chunks of strip J that hold at least one admissible row: [cf, cl].  Chunk c covers rows c CROWS - SKEW .. c CROWS +
+// CROWS - 1 over the 32 lanes; column j admits rows j - band .. j + band.  Every column has an admissible row because
+// band >= |n - m| (checked on the host), so cf <= cl.
+__device__ __forceinline__ void band_chunks(int J, int band, int C, int& cf, int& cl) {
+    cf = 0; cl = C - 1;
+    if (band < 0) return;
+    const long long jl = (long long)J * SW, jh = jl + SW - 1;
+    if (jl - band > 0) cf = (int)((jl - band) / CROWS);
+    cl = (int)min((long long)(C - 1), (jh + band + SKEW) / CROWS);
+}
+
 // ------------------------------------------------------------------------------------------------------------------
 // prologue: the scaled copies of the inputs the two wavefront kernels read
 __global__ void scale_inputs_kernel(const float* __restrict__ X, long long nx, const float* __restrict__ Z, long long nz,
@@ -403,15 +414,19 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
         };
 
         // prefetch of chunk 0: the cycle's rows (cp.async) and the left strip's boundary values (registers)
-        stage_x_async<D>(xs0, p.Xs, pm.x_off, n, 0, lane);
+        // band: chunks above / below the band are not swept.  Starting at chunk cf from the zero state is exact: whatever
+        // an admissible cell takes from a skipped chunk is an input the band-edge override replaces.
+        int cf, cl;
+        band_chunks(J, band, C, cf, cl);
+        stage_x_async<D>(xs0 + (cf & 1) * XWIN * D, p.Xs, pm.x_off, n, cf, lane);
         const int vlane = (lane < CH) ? lane : 0;          // lanes >= CH duplicate lane 0's poll (CH < 32 only)
         float2 vreg = make_float2(0.f, 0.f);
-        if (J > 0) vreg = ld_relaxed_f2(VSprev + 2 * vlane);
+        if (J > 0) vreg = ld_relaxed_f2(VSprev + cf * CROWS + 2 * vlane);
         auto unpublished = [&](const float2 v, const int r) {   // rows >= n are never used
             return (r < n && is_sentinel(v.x)) || (r + 1 < n && is_sentinel(v.y));
         };
 
-        for (int c = 0; c < C; ++c) {
+        for (int c = cf; c <= cl; ++c) {
             const int rbase = c * CROWS + 2 * vlane;       // lane 0 works on rows rbase, rbase + 1 at step `vlane`
 #ifdef SDTW_EXPERIMENT_NODEP
             if (false) {
@@ -441,7 +456,7 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
             cp_async_wait_all();
             if (lane < CH) vin_s[lane] = vreg;
             __syncwarp();
-            if (c + 1 < C) {                               // prefetch of chunk c + 1 (the other x buffer)
+            if (c + 1 <= cl) {                             // prefetch of chunk c + 1 (the other x buffer)
                 stage_x_async<D>(xs0 + ((c + 1) & 1) * XWIN * D, p.Xs, pm.x_off, n, c + 1, lane);
                 if (J > 0) vreg = ld_relaxed_f2(VSprev + rbase + CROWS);
             }
@@ -463,6 +478,12 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
             __syncwarp();
             // lane 31 worked on rows c CROWS - SKEW + 2t (+1) at step t
             if (lane < CH) st_relaxed_f2(VSme + c * CROWS - SKEW + 2 * lane, vout_s[lane]);
+        }
+        if (cl < C - 1) {
+            // the right strip's last chunks (its band ends SW rows lower) still poll rows this strip never reaches: they
+            // feed only cells outside the band or overridden inputs, so publish zeros for them
+            const int r0 = (cl + 1) * CROWS - SKEW, r1 = min(C, cl + 2 + SW / CROWS + 1) * CROWS;
+            for (int r = r0 + 2 * lane; r < r1; r += 64) st_relaxed_f2(VSme + r, make_float2(0.f, 0.f));
         }
         // value partial of this item
         double part = (double)hsum + (double)vacc;
@@ -504,6 +525,9 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
         const int j0 = (J * 32 + lane) * W;
         const bool has_right = (J < p.NS - 1);
         const int band = p.band;
+        int cf, cl;                                           // chunks of this strip with rows inside the band
+        band_chunks(J, band, C, cf, cl);
+        const int bfirst = cf * BPC;
         const float* VSprev = p.VS + pm.vs_off + (long long)(J - 1) * pm.vs_stride + VS_PAD;
         float* ESme = p.ES + pm.vs_off + (long long)J * pm.vs_stride + VS_PAD;   // indexed by row
         const float* ESnext = ESme + pm.vs_stride;
@@ -524,14 +548,14 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
         // prefetch of the next checkpoint to restore
         float4 ph[W / 4]; float2 pv = make_float2(0.f, 0.f);
         auto prefetch = [&](int bidx) {
-            if (bidx >= 1) {
+            if (bidx > bfirst) {                              // block bfirst starts from the zero state, not a checkpoint
                 const float* ck = CKme + (long long)bidx * CK_FLOATS;
 #pragma unroll
                 for (int gq = 0; gq < W / 4; ++gq) ph[gq] = __ldcs(reinterpret_cast<const float4*>(ck) + gq * 32 + lane);
                 pv = __ldcs(reinterpret_cast<const float2*>(ck + W * 32) + lane);
             }
         };
-        prefetch(C * BPC - 1);
+        prefetch((cl + 1) * BPC - 1);
 
         // one row of the recompute, keeping the transition weights
         auto rec_row = [&](const int i, const XRow<D>& x, float& v, const int slot) {
@@ -614,9 +638,9 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
         };
 
         unsigned seen = 0;
-        int pf = C * BPC - 1;                                  // block whose checkpoint (ph, pv) currently holds
+        int pf = (cl + 1) * BPC - 1;                           // block whose checkpoint (ph, pv) currently holds
         unsigned long long skipped = 0;
-        for (int c = C - 1; c >= 0; --c) {
+        for (int c = cl; c >= cf; --c) {
             if (has_right) {                                   // right strip must have finished chunks >= max(c-LAGC, 0)
                 const unsigned need = (unsigned)(C - max(c - LAGC, 0));
                 while (seen < need) { seen = ld_acquire(p.prog_b + item + 1); if (seen < need) __nanosleep(64); }
@@ -653,9 +677,9 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
 #pragma unroll 1
             for (int b = BPC - 1; b >= 0; --b) {
                 const int bidx = c * BPC + b, t0 = b * TR;
-                if (bidx == 0) {
+                if (bidx == bfirst) {                          // the forward sweep started here from the zero state
 #pragma unroll
-                    for (int w = 0; w < W; ++w) h[w] = (j0 + w == 0) ? BIG : 0.f;
+                    for (int w = 0; w < W; ++w) h[w] = (bidx == 0 && j0 + w == 0) ? BIG : 0.f;
                     vp0 = vp1 = 0.f;
                 } else {
                     if (pf != bidx) prefetch(bidx);            // the chunk below was skipped: nothing was prefetched
@@ -683,6 +707,17 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
             __syncwarp();                                      // orders every lane's ES store before lane 0's release
             if (lane == 0) st_release(p.prog_b + item, (unsigned)(C - c));
         }
+        if (cf > 0) {
+            // chunks above the band: no flow reaches them.  The left strip's band starts up to SW rows higher, so it
+            // still reads this strip's messages for a few of those chunks: publish zeros, then report everything done.
+            if (J > 0) {
+                const int r0 = max(0, cf - SW / CROWS - 2) * CROWS, r1 = cf * CROWS;
+                for (int r = r0 + 2 * lane; r < r1; r += 64) *reinterpret_cast<float2*>(ESme + r) = make_float2(0.f, 0.f);
+            }
+            __syncwarp();
+            if (lane == 0) st_release(p.prog_b + item, (unsigned)C);
+        }
+        skipped += (unsigned long long)(C - 1 - cl + cf);
         if (lane == 0 && p.stats) { atomicAdd(p.stats + 0, (unsigned long long)C); atomicAdd(p.stats + 1, skipped); }
         // eq. 6 partial of this pair for this strip's columns, back in natural units
 #pragma unroll

@@ -418,3 +418,25 @@ def test_band_that_matters(B, oracle, n_lo, n_hi, m, d, gamma, band):
     print(f"[{cfg.name}] gradient rel L2 {e:.3e} (unbanded oracle differs by {rel_l2(oG_free, oG):.3e}, band+1 by {rel_l2(oG_off, oG):.3e})")
     assert e <= GRAD_TOL and rel_l2(oG_free, oG) > 10 * GRAD_TOL
     assert rel_l2(oG_off, oG) > 2 * GRAD_TOL                            # ... and so does a one-cell shift of its edge
+
+
+def test_band_dense_reverse_and_schedule_are_bitwise_neutral(B):
+    """With a band the reverse kernel only sweeps chunks that hold admissible rows; the dense mode (no zero-skip) and
+    any forward unit size must give the same bits."""
+    import torch
+    cfg = synth.scaled(synth.CONFIGS[4], 0.1, N=6)
+    data = synth.make(cfg)
+    band = B.table1_band(cfg.m, data["lengths"], 0.3)
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    v0, g0, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
+    try:
+        B.sdtw_set_reverse_mode(True)
+        v1, g1, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
+        B.sdtw_set_reverse_mode(False)
+        B.sdtw_set_schedule(3)
+        v2, g2, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
+    finally:
+        B.sdtw_set_reverse_mode(False)
+        B.sdtw_set_schedule(0)
+    assert torch.equal(v0, v1) and torch.equal(g0, g1) and torch.equal(v0, v2) and torch.equal(g0, g2)
+    assert torch.isfinite(g0).all()
