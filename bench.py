@@ -37,9 +37,9 @@ UNIT = "cells/s"
 # roofline constants: MUFU (ex2/lg2/rcp) results per clock per SM on sm_100, SM count, max clock
 MUFU_PER_CLK_PER_SM = 16
 ALGO_MUFU_FWD, ALGO_MUFU_BWD = 3, 3          # algorithmic special-function evaluations per cell (2 ex2 + lg2; 3 ex2)
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE reverse-kernel launch at this workload, from the ncu --set full
-# capture summarised in profiles/ (None until a capture of the current kernel exists)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the named kernel at the named config, from the
+# ncu --set full capture summarised in profiles/ (null for workloads without a capture)
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {("forward_kernel", 4): 498770944 + 36701090000}   # profiles/r1b_forward_kernel_cfg4_full.txt
 
 
 def workload_string(cfg):
@@ -283,7 +283,8 @@ def run_ours(args):
         roofline = {
             "bound": "alu", "kernel": dom, "achieved": achieved / 1e9, "peak": mufu_peak / 1e9, "unit": "GMUFU-op/s",
             "frac": achieved / mufu_peak,
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((dom, args.config)) if world == 1 else None,
+            "algorithmic_bytes": None if forward_only else int(ncells_local * 0.375 + ncells_local * 4 / 128),
             "peak_source": f"derived: {MUFU_PER_CLK_PER_SM} MUFU results/clk/SM x {sms} SMs x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm); "
                            "MEASURED_PEAKS.json holds no ALU figure (DESIGN.md section 8)",
             "mufu_measured_gops": {k: v / 1e9 for k, v in mufu.items()},
