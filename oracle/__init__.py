@@ -135,6 +135,36 @@ def dtw(x, z):
     return v.value
 
 
+def dtw_path(x, z, want_path=False):
+    """eq. 1 + eq. 8's |pi| in float64: (DTW value, path length[, path as (len, 2) 1-based (i, j)])."""
+    x = _as2d(x)
+    z = _as2d(z)
+    n, m = x.shape[0], z.shape[0]
+    v = ctypes.c_double(0.0)
+    ln = ctypes.c_int64(0)
+    path = np.zeros((n + m, 2), np.int64) if want_path else None
+    _chk(_load().oracle_dtw_path(_d(x), ctypes.c_int64(n), _d(z), ctypes.c_int64(m), ctypes.c_int(x.shape[1]),
+                                 ctypes.byref(v), ctypes.byref(ln), path.ctypes.data_as(_c_i64_p) if want_path else None))
+    if want_path:
+        return v.value, ln.value, path[:ln.value]
+    return v.value, ln.value
+
+
+def dtw_score(Z, X_concat, offsets, nthreads=0):
+    """Mirror of the C-ABI sdtw_dtw_score (eq. 8), decisions in float32: (DTW (N,) f32, |pi| (N,) i32, score (N,) f32)."""
+    Z, X, off = _f32_inputs(Z, X_concat, offsets)
+    m, d = Z.shape
+    N = len(off) - 1
+    values = np.zeros(N, np.float32)
+    plen = np.zeros(N, np.int32)
+    score = np.zeros(N, np.float32)
+    _chk(_load().oracle_dtw_score_f32(Z.ctypes.data_as(_c_float_p), ctypes.c_int64(m), ctypes.c_int(d),
+                                      X.ctypes.data_as(_c_float_p), off.ctypes.data_as(_c_i64_p), ctypes.c_int(N),
+                                      values.ctypes.data_as(_c_float_p), plen.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
+                                      score.ctypes.data_as(_c_float_p), ctypes.c_int(nthreads)))
+    return values, plen, score
+
+
 def _f32_inputs(Z, X_concat, offsets):
     Z = np.ascontiguousarray(Z, np.float32)
     if Z.ndim == 1:

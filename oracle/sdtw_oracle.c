@@ -30,6 +30,8 @@
  *                               window |i - j| <= band on the cell indices; cells outside it belong
  *                               to no admissible path (Delta = +inf there, so r = +inf, E = 0).
  *                               band < 0 means no band.  The *_ex entry points take it.
+ *   Def. 8 / eq. 8  similarity score d_score = DTW / |pi| (Step 3 scoring): oracle_dtw_path
+ *                               (float64, the definition) and oracle_dtw_score_f32 (decisions in float32).
  *   eq. 7  per-series weights lambda_i / m_i: the *_ex entry points take one
  *                               weight w_k per pair; objective = sum_k w_k value_k and
  *                               grad = sum_k w_k grad_k (values[k] stay unweighted).
@@ -501,6 +503,107 @@ int oracle_dtw(const double *x, int64_t n, const double *z, int64_t m, int d, do
     free(D);
     free(R);
     return ORACLE_OK;
+}
+
+/* ---- Def. 8 / eq. 8: d_score(B, C_k) = DTW(B, C_k) / |pi|, pi the optimal alignment path of
+ * eq. 1.  The paper does not say which optimal path is meant when several tie (reading C20): the one obtained by
+ * backtracking from (n, m) preferring the diagonal predecessor, then (i-1, j), then (i, j-1) -- equivalently the
+ * length is carried forward with the minimum: len[i][j] = 1 + len[argmin], ties resolved in that order.
+ * float64 version (the definition): value, path length, and optionally the path itself (i, j pairs, 1-based,
+ * from (1,1) to (n,m); path must hold 2 (n + m) int64). ---- */
+int oracle_dtw_path(const double *x, int64_t n, const double *z, int64_t m, int d, double *value, int64_t *pathlen,
+                    int64_t *path) {
+    if (!x || !z || !value || !pathlen || n < 1 || m < 1 || d < 1) return ORACLE_ERR_ARG;
+    const int64_t ld = m + 1;
+    double *R = (double *)malloc((size_t)((n + 1) * ld) * sizeof(double));
+    if (!R) return ORACLE_ERR_MEM;
+    for (int64_t j = 0; j <= m; ++j) R[j] = INFINITY;
+    for (int64_t i = 0; i <= n; ++i) R[i * ld] = INFINITY;
+    R[0] = 0.0;
+    for (int64_t i = 1; i <= n; ++i)
+        for (int64_t j = 1; j <= m; ++j)
+            R[i * ld + j] = delta_sq(x + (i - 1) * d, z + (j - 1) * d, d) +
+                            min3(R[(i - 1) * ld + (j - 1)], R[(i - 1) * ld + j], R[i * ld + (j - 1)]);
+    *value = R[n * ld + m];
+    int64_t i = n, j = m, len = 0;
+    int64_t *rev = path ? (int64_t *)malloc((size_t)(2 * (n + m)) * sizeof(int64_t)) : NULL;
+    for (;;) {
+        if (rev) { rev[2 * len] = i; rev[2 * len + 1] = j; }
+        ++len;
+        if (i == 1 && j == 1) break;
+        const double rd = R[(i - 1) * ld + (j - 1)], ru = R[(i - 1) * ld + j], rl = R[i * ld + (j - 1)];
+        const double mn = min3(rd, ru, rl);
+        if (rd == mn) { --i; --j; }
+        else if (ru == mn) { --i; }
+        else { --j; }
+    }
+    *pathlen = len;
+    if (rev) {
+        for (int64_t t = 0; t < len; ++t) { path[2 * t] = rev[2 * (len - 1 - t)]; path[2 * t + 1] = rev[2 * (len - 1 - t) + 1]; }
+        free(rev);
+    }
+    free(R);
+    return ORACLE_OK;
+}
+
+/* ---- the same quantities with every DECISION taken in float32, the precision the CUDA path works in (the path
+ * length is an integer decided by float comparisons, so both sides must compare the same numbers): per cell
+ *   D = sum_c fl(fl(x_c - z_c)^2)   (c ascending, one rounding per operation, no fused multiply-add)
+ *   r = fl(D + min(r_diag, r_up, r_left)),   len = 1 + len of the first of (diag, up, left) that attains the min.
+ * Two rows are kept (forward only).  values[k] = DTW, pathlen[k] = |pi|, score[k] = fl(values[k] / fl(pathlen[k])).
+ * Mirror of the C-ABI sdtw_dtw_score.  This file is compiled with -ffp-contract=off. ---- */
+int oracle_dtw_score_f32(const float *Z, int64_t m, int d, const float *X, const int64_t *offsets, int N,
+                         float *values, int32_t *pathlen, float *score, int nthreads) {
+    if (!Z || !X || !offsets || !values || !pathlen || !score || m < 1 || d < 1 || N < 1) return ORACLE_ERR_ARG;
+    for (int k = 0; k < N; ++k)
+        if (offsets[k + 1] <= offsets[k]) return ORACLE_ERR_ARG;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+    int rc_all = ORACLE_OK;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int k = 0; k < N; ++k) {
+        const int64_t n = offsets[k + 1] - offsets[k];
+        const float *x = X + offsets[k] * d;
+        float *r = (float *)malloc((size_t)(2 * (m + 1)) * sizeof(float));
+        int32_t *l = (int32_t *)malloc((size_t)(2 * (m + 1)) * sizeof(int32_t));
+        if (!r || !l) {
+            free(r); free(l);
+#pragma omp critical
+            rc_all = ORACLE_ERR_MEM;
+            continue;
+        }
+        float *rp = r, *rc = r + (m + 1);
+        int32_t *lp = l, *lc = l + (m + 1);
+        for (int64_t j = 0; j <= m; ++j) { rp[j] = INFINITY; lp[j] = 0; }
+        rp[0] = 0.0f;
+        for (int64_t i = 1; i <= n; ++i) {
+            rc[0] = INFINITY; lc[0] = 0;
+            for (int64_t j = 1; j <= m; ++j) {
+                float D = 0.0f;
+                for (int c = 0; c < d; ++c) {
+                    const float t = x[(i - 1) * d + c] - Z[(j - 1) * d + c];
+                    const float t2 = t * t;
+                    D = (c == 0) ? t2 : D + t2;
+                }
+                const float rd = rp[j - 1], ru = rp[j], rl = rc[j - 1];
+                float mn = rd;
+                if (ru < mn) mn = ru;
+                if (rl < mn) mn = rl;
+                rc[j] = D + mn;
+                lc[j] = 1 + ((rd == mn) ? lp[j - 1] : (ru == mn) ? lp[j] : lc[j - 1]);
+            }
+            float *tr = rp; rp = rc; rc = tr;
+            int32_t *tl = lp; lp = lc; lc = tl;
+        }
+        values[k] = rp[m];
+        pathlen[k] = lp[m];
+        score[k] = rp[m] / (float)lp[m];
+        free(r); free(l);
+    }
+    return rc_all;
 }
 
 int oracle_num_threads(void) {

@@ -440,3 +440,68 @@ def test_weighted_objective_and_gradient(oracle):
     Z1, _, o1 = oracle.barycenter(Z, X, off, gamma, 1, 0.05, weights=w, band=8)
     vb, Gb, ob = oracle.value_grad(Z, X, off, gamma, weights=w, band=8, want_objective=True)
     assert np.abs(Z1 - (Z.astype(np.float64) - 0.05 * Gb)).max() < 1e-15 and abs(o1[0] - ob) < 1e-13
+
+
+# ----------------------------------------------------------------------------- Def. 8 / eq. 8: d_score = DTW / |pi|
+def brute_force_dtw(x, z):
+    """eq. 1 by enumeration: (min cost, the cost-sorted list of (cost, path))."""
+    D = sqdist(x, z)
+    paths = all_paths(*D.shape)
+    costs = np.array([sum(D[i, j] for i, j in p) for p in paths])
+    order = np.argsort(costs)
+    return costs[order[0]], [(costs[k], paths[k]) for k in order]
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 1), (1, 4, 2), (5, 1, 1), (3, 3, 1), (4, 6, 1), (6, 5, 2), (6, 6, 3)])
+def test_dtw_path_length_brute_force(oracle, shape):
+    n, m, d = shape
+    rng = np.random.default_rng(31 * n + 5 * m + d)
+    x = rng.normal(size=(n, d))
+    z = rng.normal(size=(m, d))
+    best, ranked = brute_force_dtw(x, z)
+    assert len(ranked) == 1 or ranked[1][0] - ranked[0][0] > 1e-9          # the optimal path is unique on this draw
+    v, ln, path = oracle.dtw_path(x, z, want_path=True)
+    assert abs(v - best) <= 1e-12 * max(1.0, best) and ln == len(ranked[0][1])
+    assert [(i - 1, j - 1) for i, j in path.tolist()] == ranked[0][1]      # and it is THE path, cell by cell
+    assert max(n, m) <= ln <= n + m - 1
+    assert abs(v - oracle.dtw(x, z)) == 0.0 and abs(v - dtw_minplus(sqdist(x, z))) <= 1e-12
+    # float32-decision mirror: same path length, value within float32 round-off
+    v32, l32, s32 = oracle.dtw_score(z.astype(np.float32), x.astype(np.float32), np.array([0, n]))
+    v64, l64 = oracle.dtw_path(x.astype(np.float32).astype(np.float64), z.astype(np.float32).astype(np.float64))
+    assert l32[0] == l64 and abs(v32[0] - v64) <= 1e-5 * max(1.0, v64)
+    assert s32[0] == np.float32(v32[0]) / np.float32(l32[0])
+
+
+def test_dtw_score_ties_special_cases_and_batch(oracle):
+    # all costs equal (constant series): every path is optimal; the stated tie-break (diagonal, then up, then left)
+    # walks the diagonal and then one edge: |pi| = max(n, m), DTW = (a - b)^2 |pi|
+    for n, m in [(5, 5), (4, 9), (9, 4), (1, 6), (7, 1)]:
+        x = np.full((n, 1), 0.5, np.float32)
+        z = np.full((m, 1), 0.25, np.float32)
+        v, ln, sc = oracle.dtw_score(z, x, np.array([0, n]))
+        assert ln[0] == max(n, m) and v[0] == np.float32(0.0625 * max(n, m)) and sc[0] == np.float32(0.0625)
+        v64, l64, path = oracle.dtw_path(x, z, want_path=True)
+        assert l64 == max(n, m) and abs(v64 - 0.0625 * max(n, m)) < 1e-15
+        steps = np.diff(path, axis=0)
+        assert np.all((steps >= 0) & (steps <= 1)) and np.all(steps.sum(1) >= 1)       # a valid alignment path (Def. 1)
+        assert tuple(path[0]) == (1, 1) and tuple(path[-1]) == (n, m)
+    # identical series: DTW = 0 along the diagonal, |pi| = n
+    rng = np.random.default_rng(3)
+    x = rng.normal(size=(40, 2)).astype(np.float32)
+    v, ln, sc = oracle.dtw_score(x, x, np.array([0, 40]))
+    assert v[0] == 0.0 and ln[0] == 40 and sc[0] == 0.0
+    # a series and its copy with every sample repeated twice: DTW = 0, |pi| = 2n (each z_j matched to two rows)
+    v, ln, sc = oracle.dtw_score(x, np.repeat(x, 2, axis=0), np.array([0, 80]))
+    assert v[0] == 0.0 and ln[0] == 80
+    # batch == single calls; soft-DTW sandwich (eq. 3: gamma -> 0) ties the hard value to the pinned soft one
+    data = synth.make(1)
+    cfg = data["cfg"]
+    v, ln, sc = oracle.dtw_score(data["Z0"], data["X"], data["offsets"])
+    for k in range(cfg.N):
+        a, b = data["offsets"][k], data["offsets"][k + 1]
+        vk, lk, sk = oracle.dtw_score(data["Z0"], data["X"][a:b], np.array([0, b - a]))
+        assert vk[0] == v[k] and lk[0] == ln[k] and sk[0] == sc[k]
+        v64, l64 = oracle.dtw_path(data["X"][a:b].astype(np.float64), data["Z0"].astype(np.float64))
+        assert abs(v[k] - v64) <= 1e-5 * v64 and ln[k] == l64
+        soft = oracle.pair(data["X"][a:b].astype(np.float64), data["Z0"].astype(np.float64), 1e-3, want_grad=False)["value"]
+        assert v64 - 1e-3 * math.log(delannoy(b - a - 1, cfg.m - 1)) - 1e-9 <= soft <= v64 + 1e-9
