@@ -95,6 +95,21 @@ int sdtw_barycenter_ex(float* Z_inout, int64_t m, int32_t d, const float* X_conc
                        float* out_objective, void* stream);
 
 /*
+ * sdtw_dtw_score -- Step 3 of the paper (section 3.4, Def. 8 / eq. 8, l.233-242): the classic DTW of eq. 1 (l.123-127;
+ * eq. 5 with gamma = 0, squared-Euclidean delta) between the prototype Z and each cycle x_k, the number of cells
+ * |pi_k| of the optimal alignment path, and the similarity score d_score = DTW / |pi|.  When several paths attain the
+ * minimum the path is the one obtained by preferring the diagonal predecessor, then (i-1, j), then (i, j-1)
+ * (C20; the paper does not say).  Arithmetic is plain float32, one rounding per operation, in the order
+ * D = sum_c (x_c - z_c)^2 (c ascending), r = D + min(.), score = DTW / float(|pi|).
+ *   out_dtw      dev [N] float32, DTW(x_k, Z) in the caller's pair order; may be NULL
+ *   out_pathlen  dev [N] int32, |pi_k|  (max(n_k, m) <= |pi_k| <= n_k + m - 1); may be NULL
+ *   out_score    dev [N] float32, out_dtw[k] / out_pathlen[k]; may be NULL
+ * Forward only, full matrix (no band), no special functions; same argument / stream / workspace conventions.
+ */
+int sdtw_dtw_score(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                   float* out_dtw, int32_t* out_pathlen, float* out_score, void* stream);
+
+/*
  * sdtw_gd_update -- the descent step alone: Z[t] <- Z[t] - step * G[t] for t < count (= m*d).  Used when the
  * gradient is all-reduced across GPUs between sdtw_value_grad and the update.
  */

@@ -25,6 +25,7 @@ SYMBOLS = {
     "sdtw_barycenter": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_value_grad_ex": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _i64, _vp, _vp, _vp, _vp]),
     "sdtw_barycenter_ex": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _i64, _i32, _f32, _vp, _vp, _vp]),
+    "sdtw_dtw_score": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _vp, _vp, _vp, _vp]),
     "sdtw_gd_update": (ctypes.c_int, [_vp, _vp, _i64, _f32, _vp]),
     "sdtw_value_grad_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_barycenter_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _i32, _f32, _vp, _vp, _vp]),
@@ -190,6 +191,21 @@ def sdtw_barycenter_ex(Z_inout, X_concat, offsets, gamma, iters, step, weights=N
                                        float(step), _ptr(out_values), _ptr(out_objective) if iters > 0 else None,
                                        _stream(stream)))
     return Z, out_values, out_objective
+
+
+def sdtw_dtw_score(Z, X_concat, offsets, stream=None):
+    """eq. 8: (DTW [N] f32, |pi| [N] i32, d_score [N] f32) of every cycle against the prototype Z (include/sdtw.h)."""
+    import torch
+    Z = _dev_f32(Z, "Z")
+    X = _dev_f32(X_concat, "X_concat")
+    m, d = _dims(Z)
+    off, offp, N = _offsets(offsets)
+    dtw = torch.empty(N, dtype=torch.float32, device=Z.device)
+    plen = torch.empty(N, dtype=torch.int32, device=Z.device)
+    score = torch.empty(N, dtype=torch.float32, device=Z.device)
+    with torch.cuda.device(Z.device):
+        _check(_lib.sdtw_dtw_score(_ptr(Z), m, d, _ptr(X), offp, N, _ptr(dtw), _ptr(plen), _ptr(score), _stream(stream)))
+    return dtw, plen, score
 
 
 def sdtw_gd_update(Z_inout, G, step, stream=None):

@@ -1,0 +1,178 @@
+// dtw_kernel.cuh -- sm_100a kernel of the Step-3 scoring path: classic DTW (eq. 1,
+// PAPER.md:123-127) between the prototype Z and each cycle x_k, the length |pi| of the optimal alignment path, and
+// the similarity score d_score = DTW / |pi| (Def. 8 / eq. 8).
+//
+//   r_ij = D_ij + min(r_{i-1,j-1}, r_{i-1,j}, r_{i,j-1}),   r_00 = 0, r_i0 = r_0j = +inf          (eq. 5 with gamma = 0)
+//   len_ij = 1 + len of the FIRST of (diagonal, up, left) that attains the minimum                 (C20)
+//
+// Natural units (no scaling), plain float32 with one rounding per operation and no fused multiply-add, so that the
+// integer |pi| -- decided by float comparisons -- can be compared bit for bit with a float32 mirror of the same
+// recurrence:  D = sum_c fl(fl(x_c - z_c)^2) (c ascending),  r = fl(D + min).
+//
+// Same wavefront as the Soft-DTW forward kernel (sdtw_kernels.cuh): a work item is one strip of 32 x W columns of one
+// pair swept by one warp, lane l on rows 2(s-l), 2(s-l)+1 at step s; (r, len) of a lane's last column goes to the next
+// lane by shuffle and to the next strip through a sentinel-preset global column polled one chunk ahead.  No special
+// functions: the bound is the FP32/ALU issue rate.  Items are handed out strip-major from one atomic counter (every
+// item's producer was handed out earlier, so a waiting warp never blocks the warp it waits for).
+#pragma once
+#include "sdtw_kernels.cuh"
+
+namespace sdtw {
+
+constexpr int DTW_WARPS = 8;
+constexpr unsigned F_INF = 0x7f800000u;
+
+struct DtwParams {
+    const float* Z;       // [m][D] natural units
+    const float* X;       // [sum n][D]
+    const PairMeta* pm;   // schedule order; vs_off / vs_stride in 32-bit words, 2 words (r, len) per row
+    unsigned* counter;    // work queue
+    unsigned* VS;         // strip-boundary columns: word 2 row = r bits, word 2 row + 1 = len
+    float* out_dtw;       // [N] caller order (may be null)
+    int* out_len;         // [N] (may be null)
+    float* out_score;     // [N] (may be null)
+    int m, N, NS;
+    unsigned num_items;
+};
+
+struct RL { float r; int l; };
+
+__device__ __forceinline__ uint4 ld_relaxed_u4(const unsigned* p) {
+    uint4 v;
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed_u4(unsigned* p, uint4 v) {
+    asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+template <int D> __host__ __device__ constexpr int dtw_smem_floats() { return 2 * XWIN * D + 2 * 4 * 32; }
+
+// one cell: (rd, ld) diagonal, (ru, lu) up [in: old row value of this column; out: this cell], (rl, ll) left [in/out]
+template <int D>
+__device__ __forceinline__ void dtw_cell(const XRow<D>& x, const float (&z)[D], float& rd, int& ld, float& ru, int& lu,
+                                         float& rl, int& ll) {
+    float t = __fsub_rn(x.c[0], z[0]);
+    float dist = __fmul_rn(t, t);
+#pragma unroll
+    for (int c = 1; c < D; ++c) { t = __fsub_rn(x.c[c], z[c]); dist = __fadd_rn(dist, __fmul_rn(t, t)); }
+    const float mn = fminf(fminf(rd, ru), rl);
+    const int lsel = (rd == mn) ? ld : (ru == mn) ? lu : ll;
+    const float rn = __fadd_rn(dist, mn);
+    rd = ru; ld = lu;                      // this column's old row value is the next column's diagonal
+    ru = rn; lu = lsel + 1;
+    rl = rn; ll = lsel + 1;
+}
+
+template <int D>
+__global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) {
+    extern __shared__ __align__(16) float smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float* xs0 = smem + warp * dtw_smem_floats<D>();                 // [2][XWIN][D]
+    uint4* vin_s = reinterpret_cast<uint4*>(xs0 + 2 * XWIN * D);     // [CH] (r, len) of the left strip for lane 0's two rows
+    uint4* vout_s = vin_s + 32;                                      // [CH] (r, len) of lane 31's last column
+    const int m = p.m;
+    const float INF = __uint_as_float(F_INF);
+
+    for (;;) {
+        unsigned q = 0;
+        if (lane == 0) q = atomicAdd(p.counter, 1u);
+        q = __shfl_sync(FULL, q, 0);
+        if (q >= p.num_items) break;
+        const int J = q / p.N, ps = q - J * p.N;             // strip-major: every pair's strip J before any strip J + 1
+        const PairMeta pm = p.pm[ps];
+        const int n = pm.n, C = pm.C;
+        const int j0 = (J * 32 + lane) * W;
+        unsigned* VSme = p.VS + pm.vs_off + (long long)J * pm.vs_stride + 2 * VS_PAD;   // word 2 row
+        const unsigned* VSprev = VSme - pm.vs_stride;
+
+        float z[W][D], ru[W];
+        int lu[W];
+#pragma unroll
+        for (int w = 0; w < W; ++w) {
+            const int j = j0 + w;
+#pragma unroll
+            for (int c = 0; c < D; ++c) z[w][c] = (j < m) ? __ldg(p.Z + (long long)j * D + c) : 0.f;
+            ru[w] = INF; lu[w] = 0;                          // virtual row 0: r_0j = +inf
+        }
+        RL oA{INF, 0}, oB{INF, 0};                           // this lane's last column, rows 2(s-l) and 2(s-l)+1
+        RL dprev{(J == 0 && lane == 0) ? 0.f : INF, 0};      // diagonal of the first column's upper row; r_00 = 0
+        const float* xs_lane = xs0;
+
+        auto step = [&](const int c, const int t, auto tag) {
+            constexpr bool slow = decltype(tag)::slow;
+            RL inA{__shfl_up_sync(FULL, oA.r, 1), __shfl_up_sync(FULL, oA.l, 1)};
+            RL inB{__shfl_up_sync(FULL, oB.r, 1), __shfl_up_sync(FULL, oB.l, 1)};
+            if (lane == 0) {
+                const uint4 qv = vin_s[t];
+                inA.r = __uint_as_float(qv.x); inA.l = (int)qv.y; inB.r = __uint_as_float(qv.z); inB.l = (int)qv.w;
+            }
+            XRow<D> xa, xb;
+            load_x2<D>(xs_lane, 2 * t, xa, xb);
+            const int i0 = RP * (c * CH + t - lane);
+            if (!slow || (unsigned)i0 < (unsigned)n) {
+                float rd = dprev.r, rl = inA.r; int ld = dprev.l, ll = inA.l;
+#pragma unroll
+                for (int w = 0; w < W; ++w) dtw_cell<D>(xa, z[w], rd, ld, ru[w], lu[w], rl, ll);
+                oA.r = rl; oA.l = ll;
+            }
+            if (!slow || (unsigned)(i0 + 1) < (unsigned)n) {
+                float rd = inA.r, rl = inB.r; int ld = inA.l, ll = inB.l;
+#pragma unroll
+                for (int w = 0; w < W; ++w) dtw_cell<D>(xb, z[w], rd, ld, ru[w], lu[w], rl, ll);
+                oB.r = rl; oB.l = ll;
+            }
+            dprev = inB;
+            if (lane == 31) vout_s[t] = make_uint4(__float_as_uint(oA.r), (unsigned)oA.l, __float_as_uint(oB.r), (unsigned)oB.l);
+        };
+
+        stage_x_async<D>(xs0, p.X, pm.x_off, n, 0, lane);
+        const int vlane = (lane < CH) ? lane : 0;
+        uint4 vreg = make_uint4(F_INF, 0u, F_INF, 0u);      // column 0 of the border: r_i0 = +inf
+        if (J > 0) vreg = ld_relaxed_u4(VSprev + 2 * (2 * vlane));
+        auto unpublished = [&](const uint4 v, const int r) {   // rows >= n are never used
+            return (r < n && (v.x == SENTINEL || v.y == SENTINEL)) || (r + 1 < n && (v.z == SENTINEL || v.w == SENTINEL));
+        };
+
+        for (int c = 0; c < C; ++c) {
+            const int rbase = c * CROWS + 2 * vlane;
+            if (J > 0) {
+                bool bad = unpublished(vreg, rbase);
+                while (__any_sync(FULL, bad)) {
+                    __nanosleep(100);
+                    if (bad) vreg = ld_relaxed_u4(VSprev + 2 * rbase);
+                    bad = unpublished(vreg, rbase);
+                }
+            }
+            cp_async_wait_all();
+            if (lane < CH) vin_s[lane] = vreg;
+            __syncwarp();
+            if (c + 1 < C) {
+                stage_x_async<D>(xs0 + ((c + 1) & 1) * XWIN * D, p.X, pm.x_off, n, c + 1, lane);
+                if (J > 0) vreg = ld_relaxed_u4(VSprev + 2 * (rbase + CROWS));
+            }
+            xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;
+            if (interior_chunk(c, n)) {
+#pragma unroll 4
+                for (int t = 0; t < CH; ++t) step(c, t, FastTag{});
+            } else {
+#pragma unroll 1
+                for (int t = 0; t < CH; ++t) step(c, t, SlowTag{});
+            }
+            __syncwarp();
+            if (lane < CH) st_relaxed_u4(VSme + 2 * (c * CROWS - SKEW + 2 * lane), vout_s[lane]);
+        }
+        // rows >= n were never touched, so ru / lu hold row n of every column: r_{n,m} sits in column m - 1
+#pragma unroll
+        for (int w = 0; w < W; ++w) {
+            if (j0 + w == m - 1) {
+                if (p.out_dtw) p.out_dtw[pm.k] = ru[w];
+                if (p.out_len) p.out_len[pm.k] = lu[w];
+                if (p.out_score) p.out_score[pm.k] = __fdiv_rn(ru[w], (float)lu[w]);
+            }
+        }
+        __syncwarp();
+    }
+}
+
+}  // namespace sdtw

@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "sdtw_kernels.cuh"
+#include "dtw_kernel.cuh"
 
 namespace {
 using namespace sdtw;
@@ -52,7 +53,7 @@ struct Layout {
     std::vector<PairMeta> pm;   // schedule order
 };
 
-int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, Layout& L) {
+int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, Layout& L, int vs_words = 1) {
     if (!offsets || m < 1 || d < 1 || N < 1) return SDTW_ERR_INVALID_ARG;
     if (offsets[0] != 0) return SDTW_ERR_INVALID_ARG;
     for (int k = 0; k < N; ++k)
@@ -78,7 +79,7 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
         pm.x_off = offsets[k];
         pm.n = (int)(offsets[k + 1] - offsets[k]);
         pm.C = ((pm.n + RP - 1) / RP + 31 + CH - 1) / CH;
-        pm.vs_stride = VS_PAD + pm.C * CROWS;
+        pm.vs_stride = vs_words * (VS_PAD + pm.C * CROWS);   // 32-bit words per strip (the DTW kernel keeps 2 per row)
         pm.vs_off = vs_floats;
         vs_floats += (long long)pm.vs_stride * L.NS;
         pm.ck_stride = (long long)(pm.C * (CH / TR) + 1) * CK_FLOATS;
@@ -130,6 +131,7 @@ struct Plan {
     int64_t m = 0;
     int32_t d = 0, N = 0;
     bool want_grad = false;
+    int vs_words = 1;
     std::vector<int64_t> offsets;
     std::vector<float> weights;   // caller order; empty = unweighted
     std::vector<float> weights_sched;   // schedule order (source of the upload; lives as long as the plan)
@@ -143,9 +145,10 @@ std::vector<Plan*> g_plans;
 uint64_t g_stamp = 0;
 
 int get_plan(int dev, int64_t m, int32_t d, const int64_t* offsets, int32_t N, const float* weights, bool want_grad,
-             cudaStream_t stream, Plan** out) {
+             cudaStream_t stream, Plan** out, int vs_words = 1) {
     for (Plan* pl : g_plans) {
         if (pl->dev == dev && pl->m == m && pl->d == d && pl->N == N && pl->want_grad == want_grad &&
+            pl->vs_words == vs_words &&
             std::memcmp(pl->offsets.data(), offsets, sizeof(int64_t) * (size_t)(N + 1)) == 0 &&
             (weights ? (!pl->weights.empty() && std::memcmp(pl->weights.data(), weights, sizeof(float) * (size_t)N) == 0)
                      : pl->weights.empty())) {
@@ -156,8 +159,9 @@ int get_plan(int dev, int64_t m, int32_t d, const int64_t* offsets, int32_t N, c
         }
     }
     Plan* pl = new Plan();
-    int rc = build_layout(m, d, offsets, N, want_grad, pl->L);
+    int rc = build_layout(m, d, offsets, N, want_grad, pl->L, vs_words);
     if (rc != SDTW_OK) { delete pl; return rc; }
+    pl->vs_words = vs_words;
     pl->dev = dev; pl->m = m; pl->d = d; pl->N = N; pl->want_grad = want_grad;
     pl->offsets.assign(offsets, offsets + N + 1);
     cudaError_t e = cudaMalloc(&pl->d_pm, sizeof(PairMeta) * (size_t)N);
@@ -263,6 +267,21 @@ int dispatch_backward(int d, const Params& P, int sms, cudaStream_t s) {
         case 4: return launch_backward<4>(P, sms, s);
     }
     return SDTW_ERR_UNSUPPORTED;
+}
+
+template <int D>
+int launch_dtw(const DtwParams& P, int sms, cudaStream_t stream) {
+    const int smem = DTW_WARPS * dtw_smem_floats<D>() * 4;
+    CUDA_TRY(cudaFuncSetAttribute(dtw_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    int occ = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dtw_kernel<D>, DTW_WARPS * 32, smem));
+    if (occ < 1) return SDTW_ERR_UNSUPPORTED;
+    const long long want = ((long long)P.num_items + DTW_WARPS - 1) / DTW_WARPS;
+    const int grid = (int)std::max(1LL, std::min(want, (long long)sms * occ));
+    dtw_kernel<D><<<grid, DTW_WARPS * 32, smem, stream>>>(P);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return SDTW_OK;
 }
 
 bool finite_pos(float g) { return std::isfinite(g) && g > 0.f; }
@@ -472,6 +491,51 @@ int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat,
                     float gamma, int32_t iters, float step, float* out_values, float* out_objective, void* stream_) {
     return sdtw_barycenter_ex(Z_inout, m, d, X_concat, offsets, N, gamma, nullptr, -1, iters, step, out_values,
                               out_objective, stream_);
+}
+
+int sdtw_dtw_score(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                   float* out_dtw, int32_t* out_pathlen, float* out_score, void* stream_) {
+    int rc = check_common(Z, m, d, X_concat, offsets, N, 1.0f);
+    if (rc) return rc;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    DeviceInfo di;
+    rc = get_device(di);
+    if (rc) return rc;
+    Plan* pl = nullptr;
+    rc = get_plan(di.dev, m, d, offsets, N, nullptr, false, stream, &pl, 2);
+    if (rc) return rc;
+    Workspace ws;
+    rc = ws.acquire(pl->L.total, di.dev, stream);
+    if (rc) return rc;
+    const Layout& L = pl->L;
+    DtwParams P{};
+    P.Z = Z; P.X = X_concat; P.pm = pl->d_pm;
+    P.counter = reinterpret_cast<unsigned*>(ws.ptr + L.off_counters);
+    P.VS = reinterpret_cast<unsigned*>(ws.ptr + L.off_VS);
+    P.out_dtw = out_dtw; P.out_len = out_pathlen; P.out_score = out_score;
+    P.m = (int)m; P.N = N; P.NS = L.NS; P.num_items = (unsigned)L.items;
+    ProfRec pr{};
+    if (g_profile) for (auto& e : pr.e) CUDA_TRY(cudaEventCreate(&e));
+    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[0], stream));
+    CUDA_TRY(cudaMemsetAsync(ws.ptr + L.off_counters, 0, L.sync_bytes, stream));
+    CUDA_TRY(cudaMemsetAsync(ws.ptr + L.off_VS, 0xFF, L.vs_bytes, stream));   // sentinel preset (dtw_kernel.cuh)
+    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[1], stream));
+    switch (d) {
+        case 1: rc = launch_dtw<1>(P, di.sms, stream); break;
+        case 2: rc = launch_dtw<2>(P, di.sms, stream); break;
+        case 3: rc = launch_dtw<3>(P, di.sms, stream); break;
+        case 4: rc = launch_dtw<4>(P, di.sms, stream); break;
+        default: rc = SDTW_ERR_UNSUPPORTED;
+    }
+    if (rc) return rc;
+    if (g_profile) {
+        CUDA_TRY(cudaEventRecord(pr.e[2], stream));     // "forward" slot = the DTW kernel
+        CUDA_TRY(cudaEventRecord(pr.e[3], stream));
+        CUDA_TRY(cudaEventRecord(pr.e[4], stream));
+        g_prof.push_back(pr);
+    }
+    return SDTW_OK;
 }
 
 int sdtw_gd_update(float* Z_inout, const float* G, int64_t count, float step, void* stream_) {

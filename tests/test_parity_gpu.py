@@ -440,3 +440,94 @@ def test_band_dense_reverse_and_schedule_are_bitwise_neutral(B):
         B.sdtw_set_schedule(0)
     assert torch.equal(v0, v1) and torch.equal(g0, g1) and torch.equal(v0, v2) and torch.equal(g0, g2)
     assert torch.isfinite(g0).all()
+
+
+# ------------------------------------------------------------------------------------------- Step 3 scoring: eq. 8
+def _check_dtw(B, oracle, data, tag, sample=None):
+    """sdtw_dtw_score against the float32-decision oracle: DTW, |pi| and d_score BIT-EXACT (integer work, and the float
+    operations are stated one by one in include/sdtw.h); `sample` = pair indices the oracle computes one by one."""
+    import torch
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    dtw, plen, score = B.sdtw_dtw_score(Z, X, data["offsets"])
+    torch.cuda.synchronize()
+    dtw, plen, score = dtw.cpu().numpy(), plen.cpu().numpy(), score.cpu().numpy()
+    if sample is None:
+        ov, ol, osc = oracle.dtw_score(data["Z0"], data["X"], data["offsets"])
+        ks = np.arange(len(ov))
+    else:
+        from paper_2404_12134_b200.dist import take_pairs
+        ks = np.asarray(sample)
+        Xs, offs = take_pairs(data["X"], data["offsets"], ks)
+        ov, ol, osc = oracle.dtw_score(data["Z0"], Xs, offs)
+    assert np.array_equal(plen[ks], ol), (tag, plen[ks], ol)
+    assert np.array_equal(dtw[ks].view(np.uint32), ov.view(np.uint32)), (tag, dtw[ks], ov)
+    assert np.array_equal(score[ks].view(np.uint32), osc.view(np.uint32)), tag
+    lens = data["lengths"]
+    m = data["Z0"].shape[0]
+    assert np.all(plen >= np.maximum(lens, m)) and np.all(plen <= lens + m - 1) and np.all(np.isfinite(dtw))
+    print(f"[{tag}] DTW / |pi| / d_score bit-exact on {len(ks)} pairs; |pi|/max(n,m) in [{(plen / np.maximum(lens, m)).min():.3f}, {(plen / np.maximum(lens, m)).max():.3f}]")
+    return dtw, plen, score
+
+
+def test_dtw_score_configs_bit_exact(B, oracle):
+    for idx in (1, 2):
+        _check_dtw(B, oracle, synth.make(idx), f"cfg{idx}")
+    _check_dtw(B, oracle, synth.make(synth.scaled(synth.CONFIGS[3], 0.1, N=6)), "cfg3 x0.1")
+    _check_dtw(B, oracle, synth.make(synth.scaled(synth.CONFIGS[4], 0.1, N=10)), "cfg4 x0.1")
+    data = synth.make(synth.scaled(synth.CONFIGS[5], 0.05, N=60))
+    dtw, plen, score = _check_dtw(B, oracle, data, "cfg5 x0.05")
+    # what Step 3 uses the score for: anomalous cycles score higher than normal ones
+    assert np.median(score[data["anomalous"]]) > np.median(score[~data["anomalous"]])
+    # float64 definition (oracle.dtw_path): value within float32 round-off, same path length
+    for k in range(0, 60, 7):
+        a, b = data["offsets"][k], data["offsets"][k + 1]
+        v64, l64 = oracle.dtw_path(data["X"][a:b].astype(np.float64), data["Z0"].astype(np.float64))
+        assert abs(dtw[k] - v64) <= 1e-4 * v64
+        assert abs(int(plen[k]) - l64) <= 0.002 * l64      # near-ties may resolve differently in float64
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+def test_dtw_score_edge_shapes(B, oracle, shape):
+    n_lo, n_hi, m, d, N = shape
+    cfg = dataclasses.replace(synth.CONFIGS[2], N=N, n_lo=n_lo, n_hi=n_hi, m=m, d=d, name=f"edge{shape}")
+    data = synth.make(cfg, seed=hash(shape) % 10000)
+    _check_dtw(B, oracle, data, cfg.name)
+
+
+def test_dtw_score_ties_and_errors(B, oracle):
+    import torch
+    # every cell ties (constant series): |pi| = max(n, m) by the stated tie-break; identical series: DTW = 0, |pi| = n
+    for n, m in [(300, 300), (200, 500), (500, 200), (1, 300), (300, 1)]:
+        X = np.full((n, 1), 0.5, np.float32)
+        Z = np.full((m, 1), 0.25, np.float32)
+        dtw, plen, score = B.sdtw_dtw_score(_dev(Z), _dev(X), np.array([0, n]))
+        assert plen.item() == max(n, m) and dtw.item() == np.float32(0.0625) * max(n, m) and score.item() == 0.0625
+    rng = np.random.default_rng(0)
+    x = rng.normal(size=(700, 2)).astype(np.float32)
+    dtw, plen, score = B.sdtw_dtw_score(_dev(x), _dev(np.repeat(x, 2, axis=0)), np.array([0, 1400]))
+    assert dtw.item() == 0.0 and plen.item() == 1400
+    # plateaus (exact ties inside real data): quantised inputs
+    data = synth.make(synth.scaled(synth.CONFIGS[2], 0.5, N=8))
+    data["X"] = (np.round(data["X"] * 8) / 8).astype(np.float32)
+    data["Z0"] = (np.round(data["Z0"] * 8) / 8).astype(np.float32)
+    _check_dtw(B, oracle, data, "quantised (many exact ties)")
+    with pytest.raises(B.SdtwError):
+        B.sdtw_dtw_score(_dev(data["Z0"]), _dev(data["X"]), np.array([0, 5, 5]))
+    # determinism and batch == single calls
+    d1 = B.sdtw_dtw_score(_dev(data["Z0"]), _dev(data["X"]), data["offsets"])
+    d2 = B.sdtw_dtw_score(_dev(data["Z0"]), _dev(data["X"]), data["offsets"])
+    assert all(torch.equal(a, b) for a, b in zip(d1, d2))
+
+
+@pytest.mark.timeout(1500)
+def test_dtw_score_full_size_sampled(B, oracle):
+    """cfg 5 (the scoring sweep: 1000 cycles of 20-40k samples against m = 30000) in one call; the oracle computes
+    sampled pairs (one anomalous) one by one; cfg 3 (d = 4) likewise."""
+    for idx, nsample in ((5, 3), (3, 2)):
+        data = synth.make(idx)
+        rng = np.random.default_rng(idx)
+        ks = np.sort(rng.choice(data["cfg"].N, size=nsample, replace=False))
+        if idx == 5:
+            ks[0] = int(np.flatnonzero(data["anomalous"])[0])
+            ks = np.unique(ks)
+        _check_dtw(B, oracle, data, f"cfg{idx} full size", sample=ks)
