@@ -315,6 +315,78 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# ---------------------------------------------------------------------------------------------- Step-3 scoring arm
+def run_score(args):
+    """--op score: sdtw_dtw_score (eq. 8: DTW, |pi|, d_score) over one batch; default workload = configs[4], the scoring
+    sweep.  Extra to the headline line; same JSON shape.  Bound: instruction issue (no special functions): the method
+    needs 8 thread-instructions per cell at d = 1 (x - z, square, min of three, add, two compares, select, increment)."""
+    import torch
+    from paper_2404_12134_b200 import binding as B
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1 and rank != 0:
+        return                                     # replicas only: pairs are independent, nothing to exchange
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    data = synth.make(args.config)
+    cfg = data["cfg"]
+    cells = synth.cells(data)
+    Z = torch.from_numpy(data["Z0"]).to(dev)
+    X = torch.from_numpy(data["X"]).to(dev)
+    for _ in range(args.warmup):
+        B.sdtw_dtw_score(Z, X, data["offsets"])
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    n0 = B.sdtw_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        out = B.sdtw_dtw_score(Z, X, data["offsets"])
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    launches = B.sdtw_launch_count() - n0
+    clocks = sampler.stop()
+    # end to end: pinned host inputs -> device -> results back on the host, every step
+    Xh, Zh = torch.from_numpy(data["X"]).pin_memory(), torch.from_numpy(data["Z0"]).pin_memory()
+    t0 = time.perf_counter()
+    nrep = max(1, min(args.steps, 3))
+    for _ in range(nrep):
+        X.copy_(Xh, non_blocking=True); Z.copy_(Zh, non_blocking=True)
+        res = [t.cpu() for t in B.sdtw_dtw_score(Z, X, data["offsets"])]
+    t_e2e = (time.perf_counter() - t0) / nrep
+    sm_max_hz = (clocks.get("sm_max_mhz") or 1965.0) * 1e6
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
+    algo = 6 + 2 * cfg.d                            # thread-instructions per cell the recurrence needs
+    peak = 128.0 * sms * sm_max_hz
+    import oracle
+    cores = os.cpu_count() or 1
+    Zs, Xs, off, ncs, what = oracle_sample(data, cores)
+    t = time.perf_counter()
+    oracle.dtw_score(Zs, Xs, off, nthreads=cores)
+    t_cpu = time.perf_counter() - t
+    print(json.dumps({
+        "metric": "dtw_score_dp_cells_per_s", "value": cells / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_string(cfg) + "; op = sdtw_dtw_score (eq. 8)", "cells_per_step": cells,
+                   "l2": "no flush: inputs + strip-boundary columns exceed the 126 MB L2" if cells > 1e10 else "no flush (small)"},
+        "roofline": {"bound": "alu", "kernel": "dtw_kernel", "achieved": algo * cells / (ms * 1e-3) / 1e9, "peak": peak / 1e9,
+                     "unit": "Gthread-instr/s", "frac": algo * cells / (ms * 1e-3) / peak, "traffic": None,
+                     "peak_source": f"derived: 128 thread-instructions/clk/SM (4 schedulers x 32 lanes) x {sms} SMs x {sm_max_hz / 1e6:.0f} MHz",
+                     "algorithmic_per_cell": algo},
+        "cpu_baseline": {"value": ncs / t_cpu, "unit": UNIT, "cores": min(cores, oracle.num_threads()), "kind": "oracle",
+                         "sample": what.replace("value+gradient, float64", "DTW + path length, float32 decisions")},
+        "e2e": {"value": cells / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(Xh.numel() * 4 + Zh.numel() * 4),
+                "d2h_bytes_per_step": int(cfg.N * 12), "steps": nrep, "api": "pinned copies + sdtw_dtw_score + .cpu()"},
+        "gpu_launches": int(launches), "clocks": clocks,
+    }))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -322,11 +394,15 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--op", choices=["barycenter", "score"], default="barycenter",
+                    help="score = the Step-3 d_score kernel (extra; the headline is barycenter)")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs only: leave out the host-buffer leg")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs only: leave out the timed oracle leg")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.op == "score":
+        run_score(args)
     else:
         run_ours(args)
 

@@ -16,7 +16,7 @@ ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libsdtw.so"
 SOURCES = [CSRC / "sdtw.cu", CSRC / "mufu_peak.cu"]
-DEPS = SOURCES + [CSRC / "sdtw_kernels.cuh", ROOT / "include" / "sdtw.h"]
+DEPS = SOURCES + sorted(CSRC.glob("*.cuh")) + [ROOT / "include" / "sdtw.h"]
 
 
 def nvcc_path() -> str:

@@ -57,11 +57,16 @@ __device__ __forceinline__ void dtw_cell(const XRow<D>& x, const float (&z)[D], 
 #pragma unroll
     for (int c = 1; c < D; ++c) { t = __fsub_rn(x.c[c], z[c]); dist = __fadd_rn(dist, __fmul_rn(t, t)); }
     const float mn = fminf(fminf(rd, ru), rl);
-    const int lsel = (rd == mn) ? ld : (ru == mn) ? lu : ll;
+    int lsel;                              // first of (diagonal, up, left) that attains the minimum; branch-free
+    asm("{\n\t.reg .pred p, q;\n\t.reg .s32 t;\n\t"
+        "setp.eq.f32 p, %1, %2;\n\tsetp.eq.f32 q, %3, %2;\n\t"
+        "selp.s32 t, %4, %5, q;\n\tselp.s32 %0, %6, t, p;\n\t}"
+        : "=r"(lsel) : "f"(rd), "f"(mn), "f"(ru), "r"(lu), "r"(ll), "r"(ld));
+    const int l1 = lsel + 1;
     const float rn = __fadd_rn(dist, mn);
     rd = ru; ld = lu;                      // this column's old row value is the next column's diagonal
-    ru = rn; lu = lsel + 1;
-    rl = rn; ll = lsel + 1;
+    ru = rn; lu = l1;
+    rl = rn; ll = l1;
 }
 
 template <int D>
