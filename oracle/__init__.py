@@ -165,6 +165,33 @@ def dtw_score(Z, X_concat, offsets, nthreads=0):
     return values, plen, score
 
 
+def subdtw(y, z):
+    """eq. 2 in float64: reference z against the best subsequence of window y -> (value, a*, b*) 0-based inclusive."""
+    y = _as2d(y)
+    z = _as2d(z)
+    v = ctypes.c_double(0.0)
+    a, b = ctypes.c_int64(0), ctypes.c_int64(0)
+    _chk(_load().oracle_subdtw(_d(y), ctypes.c_int64(y.shape[0]), _d(z), ctypes.c_int64(z.shape[0]),
+                               ctypes.c_int(y.shape[1]), ctypes.byref(v), ctypes.byref(a), ctypes.byref(b)))
+    return v.value, a.value, b.value
+
+
+def subdtw_f32(Z, X_concat, offsets, nthreads=0):
+    """Mirror of the C-ABI sdtw_subdtw, decisions in float32: (value (N,) f32, a* (N,) i32, b* (N,) i32)."""
+    Z, X, off = _f32_inputs(Z, X_concat, offsets)
+    m, d = Z.shape
+    N = len(off) - 1
+    values = np.zeros(N, np.float32)
+    a = np.zeros(N, np.int32)
+    b = np.zeros(N, np.int32)
+    i32p = ctypes.POINTER(ctypes.c_int32)
+    _chk(_load().oracle_subdtw_f32(Z.ctypes.data_as(_c_float_p), ctypes.c_int64(m), ctypes.c_int(d),
+                                   X.ctypes.data_as(_c_float_p), off.ctypes.data_as(_c_i64_p), ctypes.c_int(N),
+                                   values.ctypes.data_as(_c_float_p), a.ctypes.data_as(i32p), b.ctypes.data_as(i32p),
+                                   ctypes.c_int(nthreads)))
+    return values, a, b
+
+
 def _f32_inputs(Z, X_concat, offsets):
     Z = np.ascontiguousarray(Z, np.float32)
     if Z.ndim == 1:

@@ -606,6 +606,101 @@ int oracle_dtw_score_f32(const float *Z, int64_t m, int d, const float *X, const
     return rc_all;
 }
 
+/* ---- Sub-DTW (eq. 2): the whole reference z (m samples) against the best subsequence of a window
+ * y (n samples):  min over subsequence alignment paths (all of z traversed, free first and last index along y)
+ *               = min_{a <= b} DTW(z, y[a..b]).
+ * In this file's index convention rows i run over y (the series with the free ends) and columns j over z:
+ *   r_00 = 0, r_i0 = 0 (free start along y), r_0j = +inf (j >= 1),  r_ij = D_ij + min(r_{i-1,j-1}, r_{i-1,j}, r_{i,j-1}),
+ *   value = min_i r_im,  b* = the smallest i attaining it,  a* = the row of the first cell of the path obtained by
+ *   backtracking from (b*, m) with the preference diagonal, up, left (reading C20) until column 1 is left towards
+ *   column 0.  a*, b* are returned 0-based, inclusive.  float64 (the definition). ---- */
+int oracle_subdtw(const double *y, int64_t n, const double *z, int64_t m, int d, double *value, int64_t *a_out,
+                  int64_t *b_out) {
+    if (!y || !z || !value || !a_out || !b_out || n < 1 || m < 1 || d < 1) return ORACLE_ERR_ARG;
+    const int64_t ld = m + 1;
+    double *R = (double *)malloc((size_t)((n + 1) * ld) * sizeof(double));
+    if (!R) return ORACLE_ERR_MEM;
+    for (int64_t j = 1; j <= m; ++j) R[j] = INFINITY;
+    for (int64_t i = 0; i <= n; ++i) R[i * ld] = 0.0;
+    for (int64_t i = 1; i <= n; ++i)
+        for (int64_t j = 1; j <= m; ++j)
+            R[i * ld + j] = delta_sq(y + (i - 1) * d, z + (j - 1) * d, d) +
+                            min3(R[(i - 1) * ld + (j - 1)], R[(i - 1) * ld + j], R[i * ld + (j - 1)]);
+    int64_t b = 1;
+    for (int64_t i = 2; i <= n; ++i)
+        if (R[i * ld + m] < R[b * ld + m]) b = i;
+    *value = R[b * ld + m];
+    int64_t i = b, j = m;
+    for (;;) {                                   /* walk back until the path enters the free column 0 */
+        const double rd = R[(i - 1) * ld + (j - 1)], ru = R[(i - 1) * ld + j], rl = R[i * ld + (j - 1)];
+        const double mn = min3(rd, ru, rl);
+        if (rd == mn) { if (j == 1) break; --i; --j; }
+        else if (ru == mn) { --i; }
+        else { if (j == 1) break; --j; }
+    }
+    *a_out = i - 1;
+    *b_out = b - 1;
+    free(R);
+    return ORACLE_OK;
+}
+
+/* ---- the same with every decision in float32 and the start row carried forward with the minimum (mirror of the
+ * C-ABI sdtw_subdtw; operation order as in oracle_dtw_score_f32).  X holds N windows back to back. ---- */
+int oracle_subdtw_f32(const float *Z, int64_t m, int d, const float *X, const int64_t *offsets, int N, float *values,
+                      int32_t *a_out, int32_t *b_out, int nthreads) {
+    if (!Z || !X || !offsets || !values || !a_out || !b_out || m < 1 || d < 1 || N < 1) return ORACLE_ERR_ARG;
+    for (int k = 0; k < N; ++k)
+        if (offsets[k + 1] <= offsets[k]) return ORACLE_ERR_ARG;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+    int rc_all = ORACLE_OK;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int k = 0; k < N; ++k) {
+        const int64_t n = offsets[k + 1] - offsets[k];
+        const float *x = X + offsets[k] * d;
+        float *r = (float *)malloc((size_t)(2 * (m + 1)) * sizeof(float));
+        int32_t *st = (int32_t *)malloc((size_t)(2 * (m + 1)) * sizeof(int32_t));
+        if (!r || !st) {
+            free(r); free(st);
+#pragma omp critical
+            rc_all = ORACLE_ERR_MEM;
+            continue;
+        }
+        float *rp = r, *rc = r + (m + 1);
+        int32_t *sp = st, *sc = st + (m + 1);
+        for (int64_t j = 1; j <= m; ++j) { rp[j] = INFINITY; sp[j] = 0; }
+        rp[0] = 0.0f; sp[0] = 0;                      /* column 0 of row i-1 starts a path at row i (0-based i-1 ... ) */
+        float best = INFINITY; int32_t best_b = 0, best_a = 0;
+        for (int64_t i = 1; i <= n; ++i) {
+            sp[0] = (int32_t)(i - 1);                 /* a path entering from (i-1, 0) or (i, 0) starts at 0-based row i-1 */
+            rc[0] = 0.0f; sc[0] = (int32_t)(i - 1);
+            for (int64_t j = 1; j <= m; ++j) {
+                float D = 0.0f;
+                for (int c = 0; c < d; ++c) {
+                    const float t = x[(i - 1) * d + c] - Z[(j - 1) * d + c];
+                    const float t2 = t * t;
+                    D = (c == 0) ? t2 : D + t2;
+                }
+                const float rd = rp[j - 1], ru = rp[j], rl = rc[j - 1];
+                float mn = rd;
+                if (ru < mn) mn = ru;
+                if (rl < mn) mn = rl;
+                rc[j] = D + mn;
+                sc[j] = (rd == mn) ? sp[j - 1] : (ru == mn) ? sp[j] : sc[j - 1];
+            }
+            if (rc[m] < best) { best = rc[m]; best_b = (int32_t)(i - 1); best_a = sc[m]; }
+            float *tr = rp; rp = rc; rc = tr;
+            int32_t *ts = sp; sp = sc; sc = ts;
+        }
+        values[k] = best; a_out[k] = best_a; b_out[k] = best_b;
+        free(r); free(st);
+    }
+    return rc_all;
+}
+
 int oracle_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -505,3 +505,62 @@ def test_dtw_score_ties_special_cases_and_batch(oracle):
         assert abs(v[k] - v64) <= 1e-5 * v64 and ln[k] == l64
         soft = oracle.pair(data["X"][a:b].astype(np.float64), data["Z0"].astype(np.float64), 1e-3, want_grad=False)["value"]
         assert v64 - 1e-3 * math.log(delannoy(b - a - 1, cfg.m - 1)) - 1e-9 <= soft <= v64 + 1e-9
+
+
+# ----------------------------------------------------------------------------- eq. 2: Sub-DTW (Step 1's primitive)
+@pytest.mark.parametrize("shape", [(1, 1, 1), (6, 1, 1), (1, 4, 1), (7, 3, 1), (9, 4, 2), (12, 5, 1), (5, 7, 2)])
+def test_subdtw_is_min_over_subsequences(oracle, shape):
+    """eq. 2, second form: Sub-DTW(X, Y) = min_{a <= b} DTW(X, Y[a:b]) -- brute force over every (a, b) with the
+    (separately pinned) classic DTW, and over every subsequence alignment path (first form) on the small cases."""
+    n, m, d = shape                       # n = window length (free ends), m = reference length (fully traversed)
+    rng = np.random.default_rng(17 * n + m + d)
+    y = rng.normal(size=(n, d))
+    z = rng.normal(size=(m, d))
+    table = {(a, b): dtw_minplus(sqdist(y[a:b + 1], z)) for a in range(n) for b in range(a, n)}
+    best = min(table.values())
+    v, a, b = oracle.subdtw(y, z)
+    assert abs(v - best) <= 1e-12 * max(1.0, best)
+    assert 0 <= a <= b < n and abs(table[(a, b)] - best) <= 1e-12 * max(1.0, best)     # (a*, b*) attains the minimum
+    assert sorted(table.values())[1] - best > 1e-9 if len(table) > 1 else True        # and it is unique on this draw
+    if n * m <= 36:                       # first form: all paths with i_1 = 1, i_k = M along the reference
+        D = sqdist(y, z)
+        costs = []
+        for a0 in range(n):
+            for b0 in range(a0, n):
+                for path in all_paths(b0 - a0 + 1, m):
+                    costs.append(sum(D[a0 + i, j] for i, j in path))
+        assert abs(min(costs) - v) <= 1e-12 * max(1.0, v)
+    # float32-decision mirror: same (a*, b*), value within float32 round-off
+    v32, a32, b32 = oracle.subdtw_f32(z.astype(np.float32), y.astype(np.float32), np.array([0, n]))
+    v64, a64, b64 = oracle.subdtw(y.astype(np.float32).astype(np.float64), z.astype(np.float32).astype(np.float64))
+    assert (a32[0], b32[0]) == (a64, b64) and abs(v32[0] - v64) <= 1e-5 * max(1.0, v64)
+
+
+def test_subdtw_embedded_copy_ties_and_batch(oracle):
+    rng = np.random.default_rng(8)
+    z = rng.normal(size=(30, 2)).astype(np.float32)
+    y = np.concatenate([3 + rng.normal(size=(17, 2)), z, 3 + rng.normal(size=(25, 2))]).astype(np.float32)
+    v, a, b = oracle.subdtw_f32(z, y, np.array([0, len(y)]))
+    assert v[0] == 0.0 and (a[0], b[0]) == (17, 46)                    # the embedded copy is found exactly
+    v64, a64, b64 = oracle.subdtw(y, z)
+    assert v64 == 0.0 and (a64, b64) == (17, 46)
+    # a time-stretched copy (every sample twice): still cost 0, spanning the 2 m stretched samples
+    y2 = np.concatenate([5 + rng.normal(size=(9, 2)), np.repeat(z, 2, axis=0), 5 + rng.normal(size=(4, 2))]).astype(np.float32)
+    v, a, b = oracle.subdtw_f32(z, y2, np.array([0, len(y2)]))
+    assert v[0] == 0.0 and 9 <= a[0] <= 10 and 67 <= b[0] <= 68        # either repeated end sample may be dropped (ties)
+    assert oracle.subdtw(y2, z) == (0.0, a[0], b[0])
+    # all cells tie (constant series): smallest b*, and the diagonal-first walk back from it
+    yc = np.full((12, 1), 0.5, np.float32)
+    zc = np.full((5, 1), 0.25, np.float32)
+    v, a, b = oracle.subdtw_f32(zc, yc, np.array([0, 12]))
+    v64, a64, b64 = oracle.subdtw(yc, zc)
+    assert (a[0], b[0]) == (a64, b64) == (0, 4) and v[0] == np.float32(5 * 0.0625)
+    # Sub-DTW <= DTW of the whole window (the whole window is one of the subsequences), and batch == single calls
+    data = synth.make(1)
+    v, a, b = oracle.subdtw_f32(data["Z0"], data["X"], data["offsets"])
+    dv, _, _ = oracle.dtw_score(data["Z0"], data["X"], data["offsets"])
+    assert np.all(v <= dv)
+    for k in range(data["cfg"].N):
+        lo, hi = data["offsets"][k], data["offsets"][k + 1]
+        vk, ak, bk = oracle.subdtw_f32(data["Z0"], data["X"][lo:hi], np.array([0, hi - lo]))
+        assert (vk[0], ak[0], bk[0]) == (v[k], a[k], b[k])
