@@ -549,12 +549,13 @@ def test_subdtw_embedded_copy_ties_and_batch(oracle):
     v, a, b = oracle.subdtw_f32(z, y2, np.array([0, len(y2)]))
     assert v[0] == 0.0 and 9 <= a[0] <= 10 and 67 <= b[0] <= 68        # either repeated end sample may be dropped (ties)
     assert oracle.subdtw(y2, z) == (0.0, a[0], b[0])
-    # all cells tie (constant series): smallest b*, and the diagonal-first walk back from it
+    # all cells tie (constant series): every path of m cells costs the same; the smallest b* is row 0 (the whole
+    # reference matched to the first sample), so a* = b* = 0
     yc = np.full((12, 1), 0.5, np.float32)
     zc = np.full((5, 1), 0.25, np.float32)
     v, a, b = oracle.subdtw_f32(zc, yc, np.array([0, 12]))
     v64, a64, b64 = oracle.subdtw(yc, zc)
-    assert (a[0], b[0]) == (a64, b64) == (0, 4) and v[0] == np.float32(5 * 0.0625)
+    assert (a[0], b[0]) == (a64, b64) == (0, 0) and v[0] == np.float32(5 * 0.0625)
     # Sub-DTW <= DTW of the whole window (the whole window is one of the subsequences), and batch == single calls
     data = synth.make(1)
     v, a, b = oracle.subdtw_f32(data["Z0"], data["X"], data["offsets"])
