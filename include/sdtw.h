@@ -110,6 +110,21 @@ int sdtw_dtw_score(const float* Z, int64_t m, int32_t d, const float* X_concat, 
                    float* out_dtw, int32_t* out_pathlen, float* out_score, void* stream);
 
 /*
+ * sdtw_subdtw -- the primitive of Step 1, segmentation into cycles (section 3.2, eq. 2, l.129-145): Sub-DTW between the
+ * reference quasi-period Z (all m samples traversed: i_1 = 1, i_k = M in the paper's notation) and the best
+ * subsequence of each window x_k (free first and last index along the window):
+ *     value_k = min_{a <= b} DTW(Z, x_k[a..b])      a*_k, b*_k = first / last row of x_k on the optimal path.
+ * Ties: b* is the smallest row attaining the minimum, and the path is the diagonal-up-left preference of
+ * sdtw_dtw_score (C20).  Same float32 arithmetic, one rounding per operation.
+ *   Z          dev [m][d]   the reference cycle;  X_concat dev, offsets HOST: the N windows back to back
+ *   out_value  dev [N] float32;  out_a, out_b  dev [N] int32, 0-based, inclusive.  Any of them may be NULL.
+ * The sliding-window loop of l.137-143 is sequential (each window starts where the previous cycle ended); the
+ * binding's segment_cycles() drives it with one call per window.
+ */
+int sdtw_subdtw(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                float* out_value, int32_t* out_a, int32_t* out_b, void* stream);
+
+/*
  * sdtw_gd_update -- the descent step alone: Z[t] <- Z[t] - step * G[t] for t < count (= m*d).  Used when the
  * gradient is all-reduced across GPUs between sdtw_value_grad and the update.
  */

@@ -26,6 +26,7 @@ SYMBOLS = {
     "sdtw_value_grad_ex": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _i64, _vp, _vp, _vp, _vp]),
     "sdtw_barycenter_ex": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _i64, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_dtw_score": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _vp, _vp, _vp, _vp]),
+    "sdtw_subdtw": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _vp, _vp, _vp, _vp]),
     "sdtw_gd_update": (ctypes.c_int, [_vp, _vp, _i64, _f32, _vp]),
     "sdtw_value_grad_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_barycenter_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _i32, _f32, _vp, _vp, _vp]),
@@ -206,6 +207,48 @@ def sdtw_dtw_score(Z, X_concat, offsets, stream=None):
     with torch.cuda.device(Z.device):
         _check(_lib.sdtw_dtw_score(_ptr(Z), m, d, _ptr(X), offp, N, _ptr(dtw), _ptr(plen), _ptr(score), _stream(stream)))
     return dtw, plen, score
+
+
+def sdtw_subdtw(Z_ref, X_windows, offsets, stream=None):
+    """eq. 2: (Sub-DTW value [N] f32, a* [N] i32, b* [N] i32) of the reference Z_ref against each window (sdtw.h)."""
+    import torch
+    Z = _dev_f32(Z_ref, "Z_ref")
+    X = _dev_f32(X_windows, "X_windows")
+    m, d = _dims(Z)
+    off, offp, N = _offsets(offsets)
+    val = torch.empty(N, dtype=torch.float32, device=Z.device)
+    a = torch.empty(N, dtype=torch.int32, device=Z.device)
+    b = torch.empty(N, dtype=torch.int32, device=Z.device)
+    with torch.cuda.device(Z.device):
+        _check(_lib.sdtw_subdtw(_ptr(Z), m, d, _ptr(X), offp, N, _ptr(val), _ptr(a), _ptr(b), _stream(stream)))
+    return val, a, b
+
+
+def segment_cycles(Y, X_ref, alpha_frac=-0.15, subdtw=None):
+    """The sliding-window loop of PAPER.md:135-145 (Step 1).  Y: the stream [T][d], X_ref: the reference quasi-period
+    [M][d] (device float32 tensors when `subdtw` is None).  Window [ws, ws + 2M); Sub-DTW gives a*, b*; the cycle
+    Y[ws + a* .. ws + b*] is recorded; the next window starts at ws + b* + 1 + alpha_frac * M.  Reading C21: the
+    extracted text prints "ws = b* alpha" with alpha = 0.15 M "to ensure that missing data between two cycles does not
+    interfere"; the default steps BACK by alpha so that the start of the next cycle stays inside the next window
+    (a positive alpha_frac gives the other reading, a skipped gap).  The paper leaves termination open (its ws < N
+    never fails when stepping back): the loop advances by at least M/4 per window and stops when fewer than M/2
+    samples remain.  `subdtw(ref, window) -> (value, a, b)` replaces the CUDA call (the tests pass the oracle's mirror:
+    this loop holds none of the method's arithmetic).  Returns a list of (start, end, value), end inclusive."""
+    M = X_ref.shape[0]
+    T = Y.shape[0]
+    alpha = int(alpha_frac * M)
+    if subdtw is None:
+        def subdtw(ref, win):
+            v, a, b = sdtw_subdtw(ref, win.contiguous(), np.array([0, win.shape[0]], np.int64))
+            return float(v.item()), int(a.item()), int(b.item())
+    cycles = []
+    ws = 0
+    while T - ws >= max(1, M // 2):
+        we = min(T, ws + 2 * M)
+        v, a, b = subdtw(X_ref, Y[ws:we])
+        cycles.append((ws + a, ws + b, v))
+        ws = max(ws + b + 1 + alpha, ws + max(1, M // 4))
+    return cycles
 
 
 def sdtw_gd_update(Z_inout, G, step, stream=None):

@@ -28,9 +28,10 @@ struct DtwParams {
     const PairMeta* pm;   // schedule order; vs_off / vs_stride in 32-bit words, 2 words (r, len) per row
     unsigned* counter;    // work queue
     unsigned* VS;         // strip-boundary columns: word 2 row = r bits, word 2 row + 1 = len
-    float* out_dtw;       // [N] caller order (may be null)
-    int* out_len;         // [N] (may be null)
-    float* out_score;     // [N] (may be null)
+    float* out_dtw;       // [N] caller order (may be null): DTW, or the Sub-DTW value
+    int* out_len;         // [N] (may be null): |pi|, or a* (Sub-DTW)
+    float* out_score;     // [N] (may be null): DTW / |pi| (not written by the Sub-DTW variant)
+    int* out_b;           // [N] (may be null): b* (Sub-DTW only)
     int m, N, NS;
     unsigned num_items;
 };
@@ -49,7 +50,8 @@ __device__ __forceinline__ void st_relaxed_u4(unsigned* p, uint4 v) {
 template <int D> __host__ __device__ constexpr int dtw_smem_floats() { return 2 * XWIN * D + 2 * 4 * 32; }
 
 // one cell: (rd, ld) diagonal, (ru, lu) up [in: old row value of this column; out: this cell], (rl, ll) left [in/out]
-template <int D>
+// SUB (Sub-DTW, eq. 2): the integer carried with the minimum is the path's first row (copied), not its length (+1)
+template <int D, bool SUB>
 __device__ __forceinline__ void dtw_cell(const XRow<D>& x, const float (&z)[D], float& rd, int& ld, float& ru, int& lu,
                                          float& rl, int& ll) {
     float t = __fsub_rn(x.c[0], z[0]);
@@ -62,14 +64,16 @@ __device__ __forceinline__ void dtw_cell(const XRow<D>& x, const float (&z)[D], 
         "setp.eq.f32 p, %1, %2;\n\tsetp.eq.f32 q, %3, %2;\n\t"
         "selp.s32 t, %4, %5, q;\n\tselp.s32 %0, %6, t, p;\n\t}"
         : "=r"(lsel) : "f"(rd), "f"(mn), "f"(ru), "r"(lu), "r"(ll), "r"(ld));
-    const int l1 = lsel + 1;
+    const int l1 = SUB ? lsel : lsel + 1;
     const float rn = __fadd_rn(dist, mn);
     rd = ru; ld = lu;                      // this column's old row value is the next column's diagonal
     ru = rn; lu = l1;
     rl = rn; ll = l1;
 }
 
-template <int D>
+// SUB = false: eq. 1 / eq. 8 (complete paths).  SUB = true: eq. 2, the rows (the series of
+// X_concat) have free ends: r_i0 = 0 for every i, value = min_i r_im, b* = the smallest such i, a* = the path's first row.
+template <int D, bool SUB>
 __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) {
     extern __shared__ __align__(16) float smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -103,6 +107,13 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
         RL oA{INF, 0}, oB{INF, 0};                           // this lane's last column, rows 2(s-l) and 2(s-l)+1
         RL dprev{(J == 0 && lane == 0) ? 0.f : INF, 0};      // diagonal of the first column's upper row; r_00 = 0
         const float* xs_lane = xs0;
+        const bool last_strip = (J == p.NS - 1);
+        float best = INF; int best_a = 0, best_b = 0;        // Sub-DTW: running min over rows of r in column m - 1
+        auto track = [&](const int i) {
+#pragma unroll
+            for (int w = 0; w < W; ++w)
+                if (j0 + w == m - 1 && ru[w] < best) { best = ru[w]; best_a = lu[w]; best_b = i; }
+        };
 
         auto step = [&](const int c, const int t, auto tag) {
             constexpr bool slow = decltype(tag)::slow;
@@ -118,14 +129,16 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
             if (!slow || (unsigned)i0 < (unsigned)n) {
                 float rd = dprev.r, rl = inA.r; int ld = dprev.l, ll = inA.l;
 #pragma unroll
-                for (int w = 0; w < W; ++w) dtw_cell<D>(xa, z[w], rd, ld, ru[w], lu[w], rl, ll);
+                for (int w = 0; w < W; ++w) dtw_cell<D, SUB>(xa, z[w], rd, ld, ru[w], lu[w], rl, ll);
                 oA.r = rl; oA.l = ll;
+                if (SUB && last_strip) track(i0);
             }
             if (!slow || (unsigned)(i0 + 1) < (unsigned)n) {
                 float rd = inA.r, rl = inB.r; int ld = inA.l, ll = inB.l;
 #pragma unroll
-                for (int w = 0; w < W; ++w) dtw_cell<D>(xb, z[w], rd, ld, ru[w], lu[w], rl, ll);
+                for (int w = 0; w < W; ++w) dtw_cell<D, SUB>(xb, z[w], rd, ld, ru[w], lu[w], rl, ll);
                 oB.r = rl; oB.l = ll;
+                if (SUB && last_strip) track(i0 + 1);
             }
             dprev = inB;
             if (lane == 31) vout_s[t] = make_uint4(__float_as_uint(oA.r), (unsigned)oA.l, __float_as_uint(oB.r), (unsigned)oB.l);
@@ -133,7 +146,12 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
 
         stage_x_async<D>(xs0, p.X, pm.x_off, n, 0, lane);
         const int vlane = (lane < CH) ? lane : 0;
-        uint4 vreg = make_uint4(F_INF, 0u, F_INF, 0u);      // column 0 of the border: r_i0 = +inf
+        // column 0 of the border: r_i0 = +inf; Sub-DTW: r_i0 = 0, and a path that enters row i from it starts at row i
+        // (the entry of row r is the diagonal predecessor of row r + 1, so it carries r + 1)
+        auto border = [&](const int r) {
+            return SUB ? make_uint4(0u, (unsigned)(r + 1), 0u, (unsigned)(r + 2)) : make_uint4(F_INF, 0u, F_INF, 0u);
+        };
+        uint4 vreg = border(2 * vlane);
         if (J > 0) vreg = ld_relaxed_u4(VSprev + 2 * (2 * vlane));
         auto unpublished = [&](const uint4 v, const int r) {   // rows >= n are never used
             return (r < n && (v.x == SENTINEL || v.y == SENTINEL)) || (r + 1 < n && (v.z == SENTINEL || v.w == SENTINEL));
@@ -154,7 +172,7 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
             __syncwarp();
             if (c + 1 < C) {
                 stage_x_async<D>(xs0 + ((c + 1) & 1) * XWIN * D, p.X, pm.x_off, n, c + 1, lane);
-                if (J > 0) vreg = ld_relaxed_u4(VSprev + 2 * (rbase + CROWS));
+                vreg = (J > 0) ? ld_relaxed_u4(VSprev + 2 * (rbase + CROWS)) : border(rbase + CROWS);
             }
             xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;
             if (interior_chunk(c, n)) {
@@ -171,9 +189,15 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
 #pragma unroll
         for (int w = 0; w < W; ++w) {
             if (j0 + w == m - 1) {
-                if (p.out_dtw) p.out_dtw[pm.k] = ru[w];
-                if (p.out_len) p.out_len[pm.k] = lu[w];
-                if (p.out_score) p.out_score[pm.k] = __fdiv_rn(ru[w], (float)lu[w]);
+                if (SUB) {
+                    if (p.out_dtw) p.out_dtw[pm.k] = best;
+                    if (p.out_len) p.out_len[pm.k] = best_a;
+                    if (p.out_b) p.out_b[pm.k] = best_b;
+                } else {
+                    if (p.out_dtw) p.out_dtw[pm.k] = ru[w];
+                    if (p.out_len) p.out_len[pm.k] = lu[w];
+                    if (p.out_score) p.out_score[pm.k] = __fdiv_rn(ru[w], (float)lu[w]);
+                }
             }
         }
         __syncwarp();

@@ -269,19 +269,29 @@ int dispatch_backward(int d, const Params& P, int sms, cudaStream_t s) {
     return SDTW_ERR_UNSUPPORTED;
 }
 
-template <int D>
+template <int D, bool SUB>
 int launch_dtw(const DtwParams& P, int sms, cudaStream_t stream) {
     const int smem = DTW_WARPS * dtw_smem_floats<D>() * 4;
-    CUDA_TRY(cudaFuncSetAttribute(dtw_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    CUDA_TRY(cudaFuncSetAttribute(dtw_kernel<D, SUB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int occ = 0;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dtw_kernel<D>, DTW_WARPS * 32, smem));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dtw_kernel<D, SUB>, DTW_WARPS * 32, smem));
     if (occ < 1) return SDTW_ERR_UNSUPPORTED;
     const long long want = ((long long)P.num_items + DTW_WARPS - 1) / DTW_WARPS;
     const int grid = (int)std::max(1LL, std::min(want, (long long)sms * occ));
-    dtw_kernel<D><<<grid, DTW_WARPS * 32, smem, stream>>>(P);
+    dtw_kernel<D, SUB><<<grid, DTW_WARPS * 32, smem, stream>>>(P);
     ++g_launches;
     CUDA_TRY(cudaGetLastError());
     return SDTW_OK;
+}
+template <bool SUB>
+int dispatch_dtw(int d, const DtwParams& P, int sms, cudaStream_t s) {
+    switch (d) {
+        case 1: return launch_dtw<1, SUB>(P, sms, s);
+        case 2: return launch_dtw<2, SUB>(P, sms, s);
+        case 3: return launch_dtw<3, SUB>(P, sms, s);
+        case 4: return launch_dtw<4, SUB>(P, sms, s);
+    }
+    return SDTW_ERR_UNSUPPORTED;
 }
 
 bool finite_pos(float g) { return std::isfinite(g) && g > 0.f; }
@@ -493,8 +503,8 @@ int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat,
                               out_objective, stream_);
 }
 
-int sdtw_dtw_score(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
-                   float* out_dtw, int32_t* out_pathlen, float* out_score, void* stream_) {
+static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets,
+                      int32_t N, float* out_val, int32_t* out_i0, float* out_score, int32_t* out_i1, void* stream_) {
     int rc = check_common(Z, m, d, X_concat, offsets, N, 1.0f);
     if (rc) return rc;
     std::lock_guard<std::mutex> lock(g_mutex);
@@ -513,7 +523,7 @@ int sdtw_dtw_score(const float* Z, int64_t m, int32_t d, const float* X_concat, 
     P.Z = Z; P.X = X_concat; P.pm = pl->d_pm;
     P.counter = reinterpret_cast<unsigned*>(ws.ptr + L.off_counters);
     P.VS = reinterpret_cast<unsigned*>(ws.ptr + L.off_VS);
-    P.out_dtw = out_dtw; P.out_len = out_pathlen; P.out_score = out_score;
+    P.out_dtw = out_val; P.out_len = out_i0; P.out_score = out_score; P.out_b = out_i1;
     P.m = (int)m; P.N = N; P.NS = L.NS; P.num_items = (unsigned)L.items;
     ProfRec pr{};
     if (g_profile) for (auto& e : pr.e) CUDA_TRY(cudaEventCreate(&e));
@@ -521,13 +531,7 @@ int sdtw_dtw_score(const float* Z, int64_t m, int32_t d, const float* X_concat, 
     CUDA_TRY(cudaMemsetAsync(ws.ptr + L.off_counters, 0, L.sync_bytes, stream));
     CUDA_TRY(cudaMemsetAsync(ws.ptr + L.off_VS, 0xFF, L.vs_bytes, stream));   // sentinel preset (dtw_kernel.cuh)
     if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[1], stream));
-    switch (d) {
-        case 1: rc = launch_dtw<1>(P, di.sms, stream); break;
-        case 2: rc = launch_dtw<2>(P, di.sms, stream); break;
-        case 3: rc = launch_dtw<3>(P, di.sms, stream); break;
-        case 4: rc = launch_dtw<4>(P, di.sms, stream); break;
-        default: rc = SDTW_ERR_UNSUPPORTED;
-    }
+    rc = sub ? dispatch_dtw<true>(d, P, di.sms, stream) : dispatch_dtw<false>(d, P, di.sms, stream);
     if (rc) return rc;
     if (g_profile) {
         CUDA_TRY(cudaEventRecord(pr.e[2], stream));     // "forward" slot = the DTW kernel
@@ -536,6 +540,16 @@ int sdtw_dtw_score(const float* Z, int64_t m, int32_t d, const float* X_concat, 
         g_prof.push_back(pr);
     }
     return SDTW_OK;
+}
+
+int sdtw_dtw_score(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                   float* out_dtw, int32_t* out_pathlen, float* out_score, void* stream_) {
+    return dtw_common(false, Z, m, d, X_concat, offsets, N, out_dtw, out_pathlen, out_score, nullptr, stream_);
+}
+
+int sdtw_subdtw(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                float* out_value, int32_t* out_a, int32_t* out_b, void* stream_) {
+    return dtw_common(true, Z, m, d, X_concat, offsets, N, out_value, out_a, nullptr, out_b, stream_);
 }
 
 int sdtw_gd_update(float* Z_inout, const float* G, int64_t count, float step, void* stream_) {

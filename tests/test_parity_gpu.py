@@ -531,3 +531,84 @@ def test_dtw_score_full_size_sampled(B, oracle):
             ks[0] = int(np.flatnonzero(data["anomalous"])[0])
             ks = np.unique(ks)
         _check_dtw(B, oracle, data, f"cfg{idx} full size", sample=ks)
+
+
+# ------------------------------------------------------------------------------------------- Step 1 primitive: eq. 2
+def _check_subdtw(B, oracle, Zref, X, offsets, tag):
+    import torch
+    v, a, b = B.sdtw_subdtw(_dev(Zref), _dev(X), offsets)
+    torch.cuda.synchronize()
+    ov, oa, ob = oracle.subdtw_f32(Zref, X, offsets)
+    v, a, b = v.cpu().numpy(), a.cpu().numpy(), b.cpu().numpy()
+    assert np.array_equal(a, oa) and np.array_equal(b, ob), (tag, a, oa, b, ob)
+    assert np.array_equal(v.view(np.uint32), ov.view(np.uint32)), (tag, v, ov)
+    print(f"[{tag}] Sub-DTW value / a* / b* bit-exact on {len(ov)} windows; spans {(b - a + 1).tolist()[:6]}")
+    return v, a, b
+
+
+def test_subdtw_bit_exact_configs_and_edges(B, oracle):
+    for idx in (1, 2):
+        data = synth.make(idx)
+        _check_subdtw(B, oracle, data["Z0"], data["X"], data["offsets"], f"cfg{idx} cycles as windows")
+    data = synth.make(synth.scaled(synth.CONFIGS[4], 0.1, N=6))
+    _check_subdtw(B, oracle, data["Z0"], data["X"], data["offsets"], "cfg4 x0.1")
+    data = synth.make(synth.scaled(synth.CONFIGS[3], 0.05, N=4))
+    _check_subdtw(B, oracle, data["Z0"], data["X"], data["offsets"], "cfg3 x0.05 (d = 4)")
+    for shape in SHAPES:
+        n_lo, n_hi, m, d, N = shape
+        cfg = dataclasses.replace(synth.CONFIGS[2], N=N, n_lo=n_lo, n_hi=n_hi, m=m, d=d, name=f"edge{shape}")
+        data = synth.make(cfg, seed=hash(shape) % 10000)
+        _check_subdtw(B, oracle, data["Z0"], data["X"], data["offsets"], cfg.name)
+    # windows of two reference lengths holding a warped copy of the reference between other material (the paper's
+    # window = 2M): the copy is found, on a sub-span of the window
+    rng = np.random.default_rng(4)
+    data = synth.make(synth.scaled(synth.CONFIGS[2], 1.0, N=6))
+    M = data["cfg"].m
+    ref = data["Z0"]
+    wins, offs, truth = [], [0], []
+    for k in range(6):
+        cyc = data["X"][data["offsets"][k]:data["offsets"][k + 1]]
+        pre = rng.integers(50, 2 * M - len(cyc) - 50)
+        w = np.concatenate([2.5 + 0.3 * rng.normal(size=(pre, 1)), cyc, 2.5 + 0.3 * rng.normal(size=(2 * M - pre - len(cyc), 1))])
+        wins.append(w.astype(np.float32)); offs.append(offs[-1] + len(w)); truth.append((pre, pre + len(cyc) - 1))
+    v, a, b = _check_subdtw(B, oracle, ref, np.concatenate(wins), np.array(offs), "embedded warped cycles")
+    for k in range(6):
+        # the match lies inside the embedded cycle and spans a good part of it (its flat ends may be left out)
+        assert a[k] >= truth[k][0] - 25 and b[k] <= truth[k][1] + 25 and b[k] - a[k] >= 0.4 * (truth[k][1] - truth[k][0]), \
+            (k, a[k], b[k], truth[k])
+    # exact copy -> value 0 and exact span; all-ties case
+    y = np.concatenate([3 + rng.normal(size=(170, 2)), ref[:300].repeat(2, 1), 3 + rng.normal(size=(250, 2))]).astype(np.float32)
+    v, a, b = B.sdtw_subdtw(_dev(ref[:300].repeat(2, 1).copy()), _dev(y), np.array([0, len(y)]))
+    assert v.item() == 0.0 and (a.item(), b.item()) == (170, 469)
+
+
+def test_segment_cycles_loop_matches_oracle_driven_loop(B, oracle):
+    """the sliding-window segmentation driven by sdtw_subdtw finds the same cycles as the same loop
+    driven by the oracle's mirror, and they are the cycles the synthetic stream was built from."""
+    import torch
+    rng = np.random.default_rng(11)
+    data = synth.make(synth.scaled(synth.CONFIGS[2], 0.6, N=7))
+    M = data["cfg"].m
+    ref = data["Z0"]
+    parts, truth, pos = [], [], 0
+    for k in range(7):
+        gap = rng.integers(0, int(0.1 * M))                     # idle time / missing data between cycles
+        if gap:
+            parts.append(np.repeat(data["X"][data["offsets"][k]][None, :], gap, axis=0)); pos += gap
+        cyc = data["X"][data["offsets"][k]:data["offsets"][k + 1]]
+        parts.append(cyc); truth.append((pos, pos + len(cyc) - 1)); pos += len(cyc)
+    Y = np.concatenate(parts).astype(np.float32)
+    got = B.segment_cycles(_dev(Y), _dev(ref))
+    def oracle_sub(r, w):
+        v, a, b = oracle.subdtw_f32(r, w, np.array([0, len(w)]))
+        return float(v[0]), int(a[0]), int(b[0])
+    want = B.segment_cycles(Y, ref, subdtw=oracle_sub)
+    assert got == want
+    print(f"[segmentation] {len(got)} cycles found: {[(s, e) for s, e, _ in got]}; built from {truth}")
+    # every found cycle lies inside one of the cycles the stream was built from, and most of those are found
+    hit = set()
+    for s, e, _ in got:
+        inside = [k for k, (ts, te) in enumerate(truth) if s >= ts - 0.15 * M and e <= te + 0.15 * M]
+        assert inside, (s, e, truth)
+        hit.add(inside[0])
+    assert len(hit) >= 5
