@@ -194,6 +194,9 @@ int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped);
  * the kernel's warps per CTA are clamped.  Negative => SDTW_ERR_INVALID_ARG.
  */
 int sdtw_set_schedule(int unit_strips);
+/* The last `tail_strips` strips of every pair are handed out in units of `tail_unit` strips (small units at the end of
+ * the queue shorten the drain).  tail_strips < 0 restores the automatic choice; tail_unit <= 0 means "as unit_strips". */
+int sdtw_set_schedule_tail(int tail_strips, int tail_unit);
 
 /* Compile-time tile constants, for DESIGN.md / bench.py reporting: columns per thread, columns per strip (work item),
  * wavefront steps between checkpoints, steps per strip-boundary exchange, rows a lane works on per step.  Any pointer

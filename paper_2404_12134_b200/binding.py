@@ -40,6 +40,7 @@ SYMBOLS = {
     "sdtw_tile_info": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int32)] * 5),
     "sdtw_set_reverse_mode": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_schedule": (ctypes.c_int, [ctypes.c_int]),
+    "sdtw_set_schedule_tail": (ctypes.c_int, [ctypes.c_int, ctypes.c_int]),
     "sdtw_reverse_stats": (ctypes.c_int, [ctypes.POINTER(ctypes.c_uint64)] * 2),
     "sdtw_measure_mufu_peak": (ctypes.c_int, [_i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int32)]),
 }
@@ -353,6 +354,11 @@ def sdtw_set_reverse_mode(dense: bool):
 def sdtw_set_schedule(unit_strips: int = 0):
     """Forward schedule tuning: adjacent strips of one pair per unit (0 = automatic).  Results do not change."""
     _check(_lib.sdtw_set_schedule(int(unit_strips)))
+
+
+def sdtw_set_schedule_tail(tail_strips: int = -1, tail_unit: int = 0):
+    """Forward schedule tuning: size of the small units at the end of the queue (-1 = automatic)."""
+    _check(_lib.sdtw_set_schedule_tail(int(tail_strips), int(tail_unit)))
 
 
 def sdtw_reverse_stats():

@@ -93,6 +93,8 @@ struct Params {
     unsigned long long* stats;  // [0] reverse chunks visited, [1] reverse chunks skipped (instrumentation; may be null)
     int dense_reverse;    // 1: never skip a reverse chunk (for measurement / validation of the exact skip)
     int unit_strips;      // forward schedule: adjacent strips of one pair per unit (1 .. warps per CTA)
+    int tail_from;        // strips >= tail_from (a multiple of unit_strips, <= NS) are handed out in units of tail_unit
+    int tail_unit;        //   strips (>= 1): the last units in the queue are small, which shortens the drain
     int band;             // Sakoe-Chiba band (Table 1): cell (i, j) admissible iff |i - j| <= band; < 0: none
     const float* wts;     // [N] per-pair weights of eq. 7 in schedule order, or null (all 1)
     float gscale;         // 2 / sqrt(kappa)
@@ -280,7 +282,8 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
     float2* vout_s = vin_s + 32;                                     // [CH] (v_out of lane 31)
     const int m = p.m;
     const int US = p.unit_strips;                                    // strips per unit, <= FW
-    const int NG = (p.NS + US - 1) / US, NU = NG * p.N;              // groups per pair, units
+    const int NG1 = p.tail_from / US;                                // full-size groups per pair
+    const int NG = NG1 + (p.NS - p.tail_from + p.tail_unit - 1) / p.tail_unit, NU = NG * p.N;   // groups per pair, units
     // position of this warp in the rolling stream: consecutive positions share a scheduler (warp id mod 4)
     const int mypos = (warp & 3) * (FW / 4) + (warp >> 2);
     if (threadIdx.x < 32) { ctl.seen[threadIdx.x] = 0; if (threadIdx.x == 0) { ctl.popped = 0; ctl.lock = 0; } }
@@ -318,11 +321,12 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
         u = __shfl_sync(FULL, u, 0);
         if (u >= NU) break;
         const int g = u / p.N, ps = u - g * p.N;
-        const int S = min(US, p.NS - g * US);              // strips of this unit
+        const int Jg = (g < NG1) ? g * US : p.tail_from + (g - NG1) * p.tail_unit;   // first strip of this unit
+        const int S = (g < NG1) ? US : min(p.tail_unit, p.NS - Jg);                    // strips of this unit
         const int sidx = (mypos - base + FW) % FW;
         base = (base + S) % FW;
         if (sidx >= S) continue;
-        const int J = g * US + sidx;
+        const int J = Jg + sidx;
         const PairMeta pm = p.pm[ps];
         const int n = pm.n, C = pm.C;
         const int item = ps * p.NS + J;

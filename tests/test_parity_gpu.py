@@ -434,10 +434,12 @@ def test_band_dense_reverse_and_schedule_are_bitwise_neutral(B):
         v1, g1, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
         B.sdtw_set_reverse_mode(False)
         B.sdtw_set_schedule(3)
+        B.sdtw_set_schedule_tail(7, 2)
         v2, g2, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
     finally:
         B.sdtw_set_reverse_mode(False)
         B.sdtw_set_schedule(0)
+        B.sdtw_set_schedule_tail(-1, 0)
     assert torch.equal(v0, v1) and torch.equal(g0, g1) and torch.equal(v0, v2) and torch.equal(g0, g2)
     assert torch.isfinite(g0).all()
 
