@@ -490,6 +490,93 @@ int oracle_barycenter_ex_f32(const float *Z0, int64_t m, int d, const float *X, 
     return rc_all;
 }
 
+/* ---- gradient descent with a backtracking (Armijo) line search on the barycenter objective of eq. 7 -- the
+ * stand-in for the off-the-shelf optimiser of Table 1 (reading C22): it
+ * removes the step-size fragility of the fixed-step loop with value-only evaluations and vector operations.
+ *   f(Z) = sum_k w_k Soft-DTW(Z, x_k),  G = grad f.     Z(0) = Z0 promoted to double.
+ *   iteration it:  t = step0;  up to max_trials times:  Zt = Z - t G;  accept if f(Zt) <= f(Z) - c1 t ||G||^2,
+ *                  else t = shrink t.   Accepted: Z = Zt, steps[it] = t.  None accepted: steps[it] = 0 and the
+ *                  descent stops (remaining entries of steps / trials are 0, objective repeats the last value).
+ *   objective[it] = f(Z(it)) for it = 0..iters (iters + 1 entries),  trials[it] = evaluations of f spent. ---- */
+int oracle_barycenter_backtracking_f32(const float *Z0, int64_t m, int d, const float *X, const int64_t *offsets, int N,
+                                       double gamma, const double *weights, int64_t band, int iters, double step0,
+                                       double shrink, double c1, int max_trials, double *Z_out, double *values,
+                                       double *objective, double *steps, int32_t *trials, int mode, int nthreads) {
+    if (!Z0 || !X || !offsets || !Z_out || !objective || !steps || !trials || m < 1 || d < 1 || N < 1 ||
+        !(gamma > 0.0) || iters < 0 || !(step0 > 0.0) || !(shrink > 0.0 && shrink < 1.0) || !(c1 >= 0.0) || max_trials < 1)
+        return ORACLE_ERR_ARG;
+    const int64_t md = m * d;
+    double *G = (double *)malloc((size_t)md * sizeof(double));
+    double *Zt = (double *)malloc((size_t)md * sizeof(double));
+    double *vals = (double *)malloc((size_t)N * sizeof(double));
+    if (!G || !Zt || !vals) { free(G); free(Zt); free(vals); return ORACLE_ERR_MEM; }
+    for (int64_t t = 0; t < md; ++t) Z_out[t] = (double)Z0[t];
+    for (int it = 0; it < iters; ++it) { steps[it] = 0.0; trials[it] = 0; }
+    /* EVAL: f (and G) at a double-precision Z, pair by pair, summed in k order like oracle_barycenter_ex_f32 */
+    int rc = ORACLE_OK;
+    double f = 0.0;
+#define EVAL(Zptr, want_g, fout)                                                                                       \
+    do {                                                                                                               \
+        double *gk_ = (double *)calloc((size_t)N * (size_t)md, sizeof(double));                                        \
+        if (!gk_) { rc = ORACLE_ERR_MEM; break; }                                                                      \
+        _Pragma("omp parallel for schedule(dynamic, 1)") for (int k = 0; k < N; ++k) {                                 \
+            const int64_t n_ = offsets[k + 1] - offsets[k];                                                            \
+            double *x_ = (double *)malloc((size_t)(n_ * d) * sizeof(double));                                          \
+            for (int64_t t_ = 0; t_ < n_ * d; ++t_) x_[t_] = (double)X[offsets[k] * d + t_];                           \
+            double *g_ = (want_g) ? gk_ + (size_t)k * (size_t)md : NULL;                                               \
+            if (mode == 1) oracle_pair_checkpointed_banded(x_, n_, (Zptr), m, d, gamma, band, &vals[k], g_);           \
+            else oracle_pair_full_banded(x_, n_, (Zptr), m, d, gamma, band, &vals[k], g_, NULL, NULL);                 \
+            free(x_);                                                                                                  \
+        }                                                                                                              \
+        double o_ = 0.0;                                                                                               \
+        for (int k = 0; k < N; ++k) o_ += (weights ? weights[k] : 1.0) * vals[k];                                      \
+        (fout) = o_;                                                                                                   \
+        if (want_g)                                                                                                    \
+            for (int64_t t_ = 0; t_ < md; ++t_) {                                                                      \
+                double a_ = 0.0;                                                                                       \
+                for (int k = 0; k < N; ++k) a_ += (weights ? weights[k] : 1.0) * gk_[(size_t)k * (size_t)md + t_];     \
+                G[t_] = a_;                                                                                            \
+            }                                                                                                          \
+        free(gk_);                                                                                                     \
+    } while (0)
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+    EVAL(Z_out, 1, f);
+    objective[0] = f;
+    if (values) memcpy(values, vals, (size_t)N * sizeof(double));
+    int stopped = 0;
+    for (int it = 0; it < iters && rc == ORACLE_OK; ++it) {
+        if (stopped) { objective[it + 1] = f; continue; }
+        double gg = 0.0;
+        for (int64_t t = 0; t < md; ++t) gg += G[t] * G[t];
+        double step = step0;
+        int accepted = 0;
+        for (int tr = 0; tr < max_trials && rc == ORACLE_OK; ++tr) {
+            for (int64_t t = 0; t < md; ++t) Zt[t] = Z_out[t] - step * G[t];
+            double ft = 0.0;
+            EVAL(Zt, 0, ft);
+            trials[it] = tr + 1;
+            if (ft <= f - c1 * step * gg) {
+                memcpy(Z_out, Zt, (size_t)md * sizeof(double));
+                steps[it] = step;
+                EVAL(Z_out, 1, f);                       /* gradient (and the same f) at the accepted point */
+                if (values) memcpy(values, vals, (size_t)N * sizeof(double));
+                accepted = 1;
+                break;
+            }
+            step *= shrink;
+        }
+        if (!accepted) stopped = 1;
+        objective[it + 1] = f;
+    }
+#undef EVAL
+    free(G); free(Zt); free(vals);
+    return rc;
+}
+
 /* ---- Def. 4 / eq. 1: classic DTW by the min-plus dynamic programme (eq. 5 with gamma = 0),
  * squared-Euclidean delta.  Used by the gamma -> 0 pin. ---- */
 int oracle_dtw(const double *x, int64_t n, const double *z, int64_t m, int d, double *value) {

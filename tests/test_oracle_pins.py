@@ -565,3 +565,33 @@ def test_subdtw_embedded_copy_ties_and_batch(oracle):
         lo, hi = data["offsets"][k], data["offsets"][k + 1]
         vk, ak, bk = oracle.subdtw_f32(data["Z0"], data["X"][lo:hi], np.array([0, hi - lo]))
         assert (vk[0], ak[0], bk[0]) == (v[k], a[k], b[k])
+
+
+# ----------------------------------------------------------------------------- backtracking descent (NEXT-3, reading C22)
+def test_backtracking_descent_armijo_conditions(oracle):
+    data = synth.make(1)
+    cfg = data["cfg"]
+    Z0, X, off = data["Z0"], data["X"], data["offsets"]
+    step0, shrink, c1, iters = 0.64, 0.5, 1e-4, 5
+    Z, vals, obj, steps, trials = oracle.barycenter_backtracking(Z0, X, off, cfg.gamma, iters, step0, shrink, c1)
+    assert np.all(np.diff(obj) < 0) and len(obj) == iters + 1 and np.all(trials >= 1)
+    # replay the first iteration with independent value_grad calls: every rejected step violates the Armijo
+    # condition, the accepted one satisfies it, and Z moved by exactly that step (float32 Z0 is exact in float64)
+    v0, G0 = oracle.value_grad(Z0, X, off, cfg.gamma)
+    f0, gg = v0.sum(), float((G0 ** 2).sum())
+    assert abs(obj[0] - f0) < 1e-12 * abs(f0)
+    t = step0
+    for tr in range(trials[0]):
+        Zt = Z0.astype(np.float64) - t * G0
+        Z1, _, o1 = oracle.barycenter(Z0, X, off, cfg.gamma, 2, t)      # o1[1] = f(Z0 - t G0), evaluated in float64
+        ok = o1[1] <= f0 - c1 * t * gg
+        assert ok == (tr == trials[0] - 1), (tr, t, o1[1], f0)
+        if ok:
+            assert t == steps[0] and abs(o1[1] - obj[1]) < 1e-12 * abs(f0)
+        t *= shrink
+    # a step that is always accepted reproduces the fixed-step loop bit for bit; a hopeless one stops the descent
+    Zf, _, of = oracle.barycenter(Z0, X, off, cfg.gamma, 3, 0.01)
+    Zb, _, ob, sb, tb = oracle.barycenter_backtracking(Z0, X, off, cfg.gamma, 3, 0.01, shrink, 0.0)
+    assert np.array_equal(Zf, Zb) and np.array_equal(of, ob[:3]) and np.all(sb == 0.01) and np.all(tb == 1)
+    Zs, _, os_, ss, ts = oracle.barycenter_backtracking(Z0, X, off, cfg.gamma, 3, 50.0, shrink, c1, max_trials=1)
+    assert np.array_equal(Zs, Z0.astype(np.float64)) and np.all(ss == 0) and ts[0] == 1 and np.all(os_ == os_[0])
