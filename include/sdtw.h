@@ -95,6 +95,27 @@ int sdtw_barycenter_ex(float* Z_inout, int64_t m, int32_t d, const float* X_conc
                        float* out_objective, void* stream);
 
 /*
+ * sdtw_barycenter_backtracking -- gradient descent on eq. 7's objective f(Z) = sum_k w_k Soft-DTW(Z, x_k) with an Armijo
+ * backtracking line search: the stand-in for the off-the-shelf optimiser of Table 1 (l.320-332; C22).  It
+ * removes the step-size fragility of the fixed-step loop with value-only evaluations and vector operations.
+ *   iteration it:  t = step0;  up to max_trials times:  Zt = Z - t G;  accept if f(Zt) <= f(Z) - c1 t ||G||^2, else
+ *                  t = shrink t.  Accepted: Z = Zt.  None accepted: the descent stops (later iterations do nothing).
+ *   weights, band       as in sdtw_value_grad_ex (NULL / -1 for the plain problem)
+ *   step0 > 0, 0 < shrink < 1, c1 >= 0, max_trials >= 1, iters >= 0
+ *   out_values          dev  [N]  value_k at the final Z; may be NULL
+ *   out_objective       HOST [iters + 1] float64, f at Z(0), ..., Z(iters)            (required)
+ *   out_steps           HOST [iters] float32, the accepted step of each iteration (0 = none accepted)
+ *   out_trials          HOST [iters] int32, evaluations of f spent in each iteration
+ * A rejected trial costs one forward sweep, an accepted one a forward and a reverse sweep.  The accept / reject test is
+ * taken on the host in float64 on the kernel's objective, so this call BLOCKS: it synchronises `stream` once per
+ * trial (two 8-byte device-to-host copies).  The objective is summed in float64 from the float32 per-pair values.
+ */
+int sdtw_barycenter_backtracking(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets,
+                                 int32_t N, float gamma, const float* weights, int64_t band, int32_t iters, float step0,
+                                 float shrink, float c1, int32_t max_trials, float* out_values, double* out_objective,
+                                 float* out_steps, int32_t* out_trials, void* stream);
+
+/*
  * sdtw_dtw_score -- Step 3 of the paper (section 3.4, Def. 8 / eq. 8, l.233-242): the classic DTW of eq. 1 (l.123-127;
  * eq. 5 with gamma = 0, squared-Euclidean delta) between the prototype Z and each cycle x_k, the number of cells
  * |pi_k| of the optimal alignment path, and the similarity score d_score = DTW / |pi|.  When several paths attain the

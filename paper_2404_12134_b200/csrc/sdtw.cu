@@ -47,7 +47,7 @@ struct Layout {
     long long items = 0;
     size_t off_stats = 0;
     size_t off_counters = 0, off_prog_b = 0, off_VP = 0, off_Xs = 0, off_Zs = 0, off_VS = 0, off_ES = 0, off_CK = 0,
-           off_Gk = 0;
+           off_Gk = 0, off_G = 0, off_Zt = 0, off_Vt = 0, off_scal = 0;   // last four: line-search scratch
     size_t sync_bytes = 0;      // counters + stats + prog_b: cleared before every evaluation
     size_t vs_bytes = 0;        // VS: preset to the sentinel pattern before every evaluation
     size_t total = 0;
@@ -101,6 +101,10 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
         L.off_ES = o;   o += L.vs_bytes;
         L.off_CK = o;   o += align_up((size_t)ck_floats * 4, 256);
         L.off_Gk = o;   o += align_up((size_t)N * (size_t)m * (size_t)d * 4, 256);
+        L.off_G = o;    o += align_up((size_t)m * (size_t)d * 4, 256);
+        L.off_Zt = o;   o += align_up((size_t)m * (size_t)d * 4, 256);
+        L.off_Vt = o;   o += align_up((size_t)N * 4, 256);
+        L.off_scal = o; o += 256;
     }
     L.total = o;
     return SDTW_OK;
@@ -310,7 +314,10 @@ bool finite_pos(float g) { return std::isfinite(g) && g > 0.f; }
 
 // one evaluation: values (+ gradient) at Z.  If Z_update != nullptr the descent step is fused into the reduction.
 int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, const float* X, float gamma, int band,
-             float* out_values, float* out_objective, float* out_grad, float* Z_update, float step, cudaStream_t stream) {
+             float* out_values, float* out_objective, float* out_grad, float* Z_update, float step, cudaStream_t stream,
+             int phase = 3, double* out_objective64 = nullptr) {
+    // phase bit 0: clears, input scaling, forward sweep, values / objective.  bit 1: reverse sweep, reduction over
+    // pairs (+ descent step).  The line search runs the two halves separately (a rejected trial needs no reverse pass).
     const Layout& L = pl.L;
     Params P{};
     float* Xs = reinterpret_cast<float*>(ws + L.off_Xs);
@@ -339,6 +346,8 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     ProfRec pr{};
     if (g_profile) for (auto& e : pr.e) CUDA_TRY(cudaEventCreate(&e));
     if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[0], stream));
+    int rc = SDTW_OK;
+    if (phase & 1) {
     CUDA_TRY(cudaMemsetAsync(ws + L.off_counters, 0, L.sync_bytes, stream));
     // every word of the strip-boundary columns starts as the sentinel the consumers poll for (sdtw_kernels.cuh)
     CUDA_TRY(cudaMemsetAsync(ws + L.off_VS, 0xFF, L.vs_bytes, stream));
@@ -350,20 +359,22 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
         CUDA_TRY(cudaGetLastError());
     }
     if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[1], stream));
-    int rc = dispatch_forward(pl.d, P, pl.want_grad, di.sms, stream);
+    rc = dispatch_forward(pl.d, P, pl.want_grad, di.sms, stream);
     if (rc) return rc;
+    } else if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[1], stream));
     if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[2], stream));
-    if (pl.want_grad) {
+    if (pl.want_grad && (phase & 2)) {
         rc = dispatch_backward(pl.d, P, di.sms, stream);
         if (rc) return rc;
     }
     if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[3], stream));
-    if (out_values || out_objective) {
-        finalize_values_kernel<<<1, 256, 0, stream>>>(P.VP, pl.d_pm, P.wts, pl.N, L.NS, inv_kappa, out_values, out_objective);
+    if ((phase & 1) && (out_values || out_objective || out_objective64)) {
+        finalize_values_kernel<<<1, 256, 0, stream>>>(P.VP, pl.d_pm, P.wts, pl.N, L.NS, inv_kappa, out_values, out_objective,
+                                                      out_objective64);
         ++g_launches;
         CUDA_TRY(cudaGetLastError());
     }
-    if (pl.want_grad) {
+    if (pl.want_grad && (phase & 2)) {
         const long long md = (long long)pl.m * pl.d;
         const int blocks = (int)((md + 255) / 256);
         reduce_pairs_kernel<<<blocks, 256, 0, stream>>>(P.Gk, P.wts, pl.N, md, out_grad, Z_update, step);
@@ -505,6 +516,86 @@ int sdtw_barycenter_ex(float* Z_inout, int64_t m, int32_t d, const float* X_conc
         float* obj = out_objective ? out_objective + it : nullptr;
         rc = evaluate(*pl, ws.ptr, di, Z_inout, X_concat, gamma, band_eff, vals, obj, nullptr, Z_inout, step, stream);
         if (rc) return rc;
+    }
+    return SDTW_OK;
+}
+
+int sdtw_barycenter_backtracking(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets,
+                                 int32_t N, float gamma, const float* weights, int64_t band, int32_t iters, float step0,
+                                 float shrink, float c1, int32_t max_trials, float* out_values, double* out_objective,
+                                 float* out_steps, int32_t* out_trials, void* stream_) {
+    int rc = check_common(Z_inout, m, d, X_concat, offsets, N, gamma);
+    if (rc) return rc;
+    if (iters < 0 || !(std::isfinite(step0) && step0 > 0.f) || !(shrink > 0.f && shrink < 1.f) ||
+        !(std::isfinite(c1) && c1 >= 0.f) || max_trials < 1 || !out_objective || (iters > 0 && (!out_steps || !out_trials)))
+        return SDTW_ERR_INVALID_ARG;
+    int band_eff = -1;
+    rc = check_ex(m, offsets, N, weights, band, &band_eff);
+    if (rc) return rc;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    DeviceInfo di;
+    rc = get_device(di);
+    if (rc) return rc;
+    Plan* pl = nullptr;
+    rc = get_plan(di.dev, m, d, offsets, N, weights, true, stream, &pl);
+    if (rc) return rc;
+    Workspace ws;
+    rc = ws.acquire(pl->L.total, di.dev, stream);
+    if (rc) return rc;
+    const Layout& L = pl->L;
+    float* G = reinterpret_cast<float*>(ws.ptr + L.off_G);
+    float* Zt = reinterpret_cast<float*>(ws.ptr + L.off_Zt);
+    float* Vt = reinterpret_cast<float*>(ws.ptr + L.off_Vt);
+    double* scal = reinterpret_cast<double*>(ws.ptr + L.off_scal);      // [0] objective, [1] ||G||^2
+    const long long md = (long long)m * d;
+    const int blocks = (int)((md + 255) / 256);
+    double h[2] = {0.0, 0.0};
+    auto read_scalars = [&]() -> int {
+        CUDA_TRY(cudaMemcpyAsync(h, scal, sizeof(h), cudaMemcpyDeviceToHost, stream));
+        CUDA_TRY(cudaStreamSynchronize(stream));
+        return SDTW_OK;
+    };
+    auto gradient_norm = [&]() -> int {
+        sqnorm_kernel<<<1, 1024, 0, stream>>>(G, md, scal + 1);
+        ++g_launches;
+        CUDA_TRY(cudaGetLastError());
+        return SDTW_OK;
+    };
+    // f, values and G at Z0
+    rc = evaluate(*pl, ws.ptr, di, Z_inout, X_concat, gamma, band_eff, out_values, nullptr, G, nullptr, 0.f, stream, 3, scal);
+    if (rc || (rc = gradient_norm()) || (rc = read_scalars())) return rc;
+    double f = h[0], gg = h[1];
+    out_objective[0] = f;
+    bool stopped = false;
+    for (int it = 0; it < iters; ++it) {
+        out_steps[it] = 0.f; out_trials[it] = 0;
+        if (!stopped) {
+            double t = step0;
+            bool accepted = false;
+            for (int tr = 0; tr < max_trials; ++tr) {
+                trial_point_kernel<<<blocks, 256, 0, stream>>>(Zt, Z_inout, G, md, (float)t);
+                ++g_launches;
+                CUDA_TRY(cudaGetLastError());
+                // forward sweep only (with checkpoints: an accepted trial goes straight on to its reverse sweep)
+                rc = evaluate(*pl, ws.ptr, di, Zt, X_concat, gamma, band_eff, Vt, nullptr, nullptr, nullptr, 0.f, stream, 1, scal);
+                if (rc || (rc = read_scalars())) return rc;
+                out_trials[it] = tr + 1;
+                if (h[0] <= f - (double)c1 * t * gg) {                 // Armijo condition, on the host in double
+                    CUDA_TRY(cudaMemcpyAsync(Z_inout, Zt, (size_t)md * 4, cudaMemcpyDeviceToDevice, stream));
+                    if (out_values) CUDA_TRY(cudaMemcpyAsync(out_values, Vt, (size_t)N * 4, cudaMemcpyDeviceToDevice, stream));
+                    rc = evaluate(*pl, ws.ptr, di, Zt, X_concat, gamma, band_eff, nullptr, nullptr, G, nullptr, 0.f, stream, 2);
+                    if (rc || (rc = gradient_norm()) || (rc = read_scalars())) return rc;
+                    f = h[0]; gg = h[1];
+                    out_steps[it] = (float)t;
+                    accepted = true;
+                    break;
+                }
+                t *= (double)shrink;
+            }
+            if (!accepted) stopped = true;
+        }
+        out_objective[it + 1] = f;
     }
     return SDTW_OK;
 }

@@ -740,7 +740,8 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
 // small kernels: per-pair values from the item partials, objective, reduction over pairs, descent step
 __global__ void finalize_values_kernel(const double* __restrict__ VP, const PairMeta* __restrict__ pm,
                                        const float* __restrict__ wts, int N, int NS,
-                                       double inv_kappa, float* __restrict__ out_values, float* __restrict__ out_objective) {
+                                       double inv_kappa, float* __restrict__ out_values, float* __restrict__ out_objective,
+                                       double* __restrict__ out_objective64) {
     __shared__ double red[256];
     double local = 0.0;
     for (int ps = threadIdx.x; ps < N; ps += blockDim.x) {
@@ -758,6 +759,7 @@ __global__ void finalize_values_kernel(const double* __restrict__ VP, const Pair
         __syncthreads();
     }
     if (threadIdx.x == 0 && out_objective) *out_objective = (float)red[0];
+    if (threadIdx.x == 0 && out_objective64) *out_objective64 = red[0];
 }
 
 // G[e] = sum over pairs (schedule order, fp64 accumulator: deterministic, no atomics); optional descent step
@@ -771,6 +773,25 @@ __global__ void reduce_pairs_kernel(const float* __restrict__ Gk, const float* _
     const float gsum = (float)acc;
     if (out_grad) out_grad[e] = gsum;
     if (Z) Z[e] = Z[e] - step * gsum;
+}
+
+// line-search helpers: the trial point Zt = Z - t G, and ||G||^2 by a fixed-shape tree (one block; deterministic)
+__global__ void trial_point_kernel(float* __restrict__ Zt, const float* __restrict__ Z, const float* __restrict__ G,
+                                   long long count, float t) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < count) Zt[e] = Z[e] - t * G[e];
+}
+__global__ void sqnorm_kernel(const float* __restrict__ G, long long count, double* __restrict__ out) {
+    __shared__ double red[1024];
+    double acc = 0.0;
+    for (long long e = threadIdx.x; e < count; e += blockDim.x) acc += (double)G[e] * (double)G[e];
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = red[0];
 }
 
 __global__ void gd_update_kernel(float* __restrict__ Z, const float* __restrict__ G, long long count, float step) {

@@ -614,3 +614,46 @@ def test_segment_cycles_loop_matches_oracle_driven_loop(B, oracle):
         assert inside, (s, e, truth)
         hit.add(inside[0])
     assert len(hit) >= 5
+
+
+# ------------------------------------------------------------------------------------------- NEXT-3: line-search descent
+@pytest.mark.parametrize("idx,scale,N,iters,step0", [(1, 1.0, 8, 6, 0.64), (2, 1.0, 16, 5, 0.04), (4, 0.1, 8, 4, 0.02),
+                                                     (3, 0.05, 4, 4, 0.4)])
+def test_backtracking_descent_matches_oracle(B, oracle, idx, scale, N, iters, step0):
+    """sdtw_barycenter_backtracking against the float64 oracle of the same algorithm: step0 is several times too large
+    for the fixed-step loop, so the line search has to cut it; accepted steps, trial counts, objective history and the
+    final barycenter must agree (the accept test compares the same quantities on both sides; the margins on these
+    inputs are far above float32 round-off, which the test checks)."""
+    cfg = synth.scaled(synth.CONFIGS[idx], scale, N=N) if (scale != 1.0 or N != synth.CONFIGS[idx].N) else synth.CONFIGS[idx]
+    data = synth.make(cfg)
+    Z, vals, obj, steps, trials = B.sdtw_barycenter_backtracking(_dev(data["Z0"]), _dev(data["X"]), data["offsets"],
+                                                                 cfg.gamma, iters, step0)
+    Zo, vo, oo, so, to = oracle.barycenter_backtracking(data["Z0"], data["X"], data["offsets"], cfg.gamma, iters, step0,
+                                                        mode="checkpointed")
+    print(f"[{cfg.name}] steps {steps.tolist()} (oracle {so.tolist()}), trials {trials.tolist()}, objective {obj.tolist()}")
+    assert np.array_equal(trials, to) and np.allclose(steps, so, rtol=1e-6)
+    assert trials.max() > 1 and np.all(np.diff(obj) < 0)                  # the search did cut the step; monotone descent
+    scale_f = np.sum(cfg.gamma * (data["lengths"] + cfg.m))
+    assert np.all(np.abs(obj - oo) <= 1e-4 * np.maximum(np.abs(oo), scale_f))
+    e = rel_l2(Z.cpu().numpy(), Zo)
+    moved = np.linalg.norm(Z.cpu().numpy() - Zo) / np.linalg.norm(Zo - data["Z0"])
+    print(f"[{cfg.name}] barycenter rel L2 {e:.3e}, relative to distance moved {moved:.3e}")
+    assert e <= BARY_TOL and moved <= 5e-2
+    check_values(vals.cpu().numpy(), vo, data["lengths"], cfg, f"{cfg.name} values at the final Z")
+
+
+def test_backtracking_equals_fixed_step_when_always_accepted(B):
+    import torch
+    data = synth.make(1)
+    cfg = data["cfg"]
+    Zf, vf, of = B.sdtw_barycenter(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, 3, cfg.step)
+    Zb, vb, ob, sb, tb = B.sdtw_barycenter_backtracking(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, 3,
+                                                        cfg.step, c1=0.0)
+    assert torch.equal(Zf, Zb) and np.all(tb == 1) and np.allclose(sb, cfg.step)
+    assert np.allclose(ob[:3], of.cpu().numpy(), rtol=1e-6)
+    # hopeless first step, one trial allowed: nothing moves
+    Zs, _, os_, ss, ts = B.sdtw_barycenter_backtracking(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, 2,
+                                                        50.0, max_trials=1)
+    assert torch.equal(Zs.cpu(), torch.from_numpy(data["Z0"])) and np.all(ss == 0) and os_[0] == os_[2]
+    with pytest.raises(B.SdtwError):
+        B.sdtw_barycenter_backtracking(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, 2, 0.1, shrink=1.5)
