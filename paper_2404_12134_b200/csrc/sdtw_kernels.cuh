@@ -198,6 +198,7 @@ __device__ __forceinline__ float ex2_fma(float x) {
 // (mask A: the even row of a step, mask B: the odd row).  The MUFU pipe is the forward kernel's bound and its issue
 // slots are 60 % busy, so moving a quarter of the ex2 work to the FMA pipe shortens the sweep.  The reverse kernel is
 // latency bound and keeps MUFU for all three (a 12-instruction chain instead of one would lengthen its critical path).
+// d >= 3: the cost arithmetic already fills the issue slots, so the polynomial is not used there either.
 #ifndef SDTW_POLY_MASK_A
 #define SDTW_POLY_MASK_A 2
 #endif
@@ -400,7 +401,7 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
                     if (j0 + w - i == band) h[w] = BIG;
                     if (i - (j0 + w) == band) v = BIG;
                 }
-                cell<false, (D > 1)>(tl, acc, h[w], v, dummy0, dummy1, (((i & 1) ? SDTW_POLY_MASK_B : SDTW_POLY_MASK_A) >> w) & 1);
+                cell<false, (D > 1)>(tl, acc, h[w], v, dummy0, dummy1, D <= 2 && ((((i & 1) ? SDTW_POLY_MASK_B : SDTW_POLY_MASK_A) >> w) & 1));
                 if (w == 0) vfirst = v;
             }
             if ((unsigned)(i - r_v0 - 1) < (unsigned)(r_v1 - r_v0)) vacc += vfirst_sel ? vfirst : v;
@@ -422,9 +423,9 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
                 for (int w = 0; w < W; ++w) {              // cell (A, w+1) and cell (A+1, w) are independent
                     float tl, acc;
                     sqdist2<D>(xa, z[w], tl, acc);
-                    cell<false, (D > 1)>(tl, acc, h[w], va, dummy0, dummy1, (SDTW_POLY_MASK_A >> w) & 1);
+                    cell<false, (D > 1)>(tl, acc, h[w], va, dummy0, dummy1, D <= 2 && ((SDTW_POLY_MASK_A >> w) & 1));
                     sqdist2<D>(xb, z[w], tl, acc);
-                    cell<false, (D > 1)>(tl, acc, h[w], vb, dummy0, dummy1, (SDTW_POLY_MASK_B >> w) & 1);
+                    cell<false, (D > 1)>(tl, acc, h[w], vb, dummy0, dummy1, D <= 2 && ((SDTW_POLY_MASK_B >> w) & 1));
                 }
                 vp0 = va; vp1 = vb;
             } else {
@@ -666,25 +667,41 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
             if (lane == 0) eout_s[t] = make_float2(msg0_prev, msg1_prev);
         };
 
+        // Progress word of an item: chunks completed from the top (C - c after chunk c); when the item is done,
+        // FIN | z: every message of its chunks [0, z) is an implicit +0 (they were never visited).
+        constexpr unsigned FIN = 0x80000000u;
         unsigned seen = 0;
         int pf = (cl + 1) * BPC - 1;                           // block whose checkpoint (ph, pv) currently holds
         unsigned long long skipped = 0;
+        bool terminated = false;
         for (int c = cl; c >= cf; --c) {
+            unsigned lbits = __float_as_uint(msg0_prev) | __float_as_uint(msg1_prev) | __float_as_uint(cdf_prev);
+#pragma unroll
+            for (int w = 0; w < W; ++w) lbits |= __float_as_uint(A[w]);
+            const bool local_nz = __any_sync(FULL, lbits != 0u);     // flow already inside this strip
             if (has_right) {                                   // right strip must have finished chunks >= max(c-LAGC, 0)
                 const unsigned need = (unsigned)(C - max(c - LAGC, 0));
                 while (seen < need) { seen = ld_acquire(p.prog_b + item + 1); if (seen < need) __nanosleep(64); }
             }
+            const bool rfin = (seen & FIN) != 0u;
+            const int zr = (int)(seen & ~FIN);                 // valid when rfin
+            // Early exit: nothing flows inside this strip and nothing will ever arrive from the right (there is no right
+            // strip, or it is done and its remaining messages are implicit zeros): every chunk from here down is a skip.
+            if (!p.dense_reverse && !local_nz && (!has_right || (rfin && c < zr))) {
+                __syncwarp();
+                if (lane == 0) st_release(p.prog_b + item, FIN | (unsigned)(c + 1));
+                skipped += (unsigned long long)(c - cf + 1);
+                terminated = true;
+                break;
+            }
             // lane 31 works on rows c CROWS - SKEW + 2t (+1) at step t; lane t fetches its message pair
             const int erow = c * CROWS - SKEW + 2 * lane;
-            const float2 ein = (has_right && lane < CH && erow >= 0) ? *reinterpret_cast<const float2*>(ESnext + erow)
-                                                                     : make_float2(0.f, 0.f);
+            const float2 ein = (has_right && lane < CH && erow >= 0 && !(rfin && erow / CROWS < zr))
+                                   ? *reinterpret_cast<const float2*>(ESnext + erow) : make_float2(0.f, 0.f);
             // Exact skip: every flow that could enter this chunk's cells is +0 (E underflows to zero off the
             // alignment band), so every product and sum below would be +0 and g would not change.
-            if (!p.dense_reverse) {
-                unsigned bits = __float_as_uint(ein.x) | __float_as_uint(ein.y) | __float_as_uint(msg0_prev) |
-                                __float_as_uint(msg1_prev) | __float_as_uint(cdf_prev);
-#pragma unroll
-                for (int w = 0; w < W; ++w) bits |= __float_as_uint(A[w]);
+            if (!p.dense_reverse && !local_nz) {
+                const unsigned bits = __float_as_uint(ein.x) | __float_as_uint(ein.y);
                 if (!__any_sync(FULL, bits != 0u)) {
                     if (J > 0 && lane < CH) *reinterpret_cast<float2*>(ESme + c * CROWS + 2 * lane) = make_float2(0.f, 0.f);
                     __syncwarp();
@@ -736,15 +753,10 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
             __syncwarp();                                      // orders every lane's ES store before lane 0's release
             if (lane == 0) st_release(p.prog_b + item, (unsigned)(C - c));
         }
-        if (cf > 0) {
-            // chunks above the band: no flow reaches them.  The left strip's band starts up to SW rows higher, so it
-            // still reads this strip's messages for a few of those chunks: publish zeros, then report everything done.
-            if (J > 0) {
-                const int r0 = max(0, cf - SW / CROWS - 2) * CROWS, r1 = cf * CROWS;
-                for (int r = r0 + 2 * lane; r < r1; r += 64) *reinterpret_cast<float2*>(ESme + r) = make_float2(0.f, 0.f);
-            }
+        // done: the chunks below cf (above the band) were never visited, their messages are implicit zeros
+        if (!terminated) {
             __syncwarp();
-            if (lane == 0) st_release(p.prog_b + item, (unsigned)C);
+            if (lane == 0) st_release(p.prog_b + item, FIN | (unsigned)cf);
         }
         skipped += (unsigned long long)(C - 1 - cl + cf);
         if (lane == 0 && p.stats) { atomicAdd(p.stats + 0, (unsigned long long)C); atomicAdd(p.stats + 1, skipped); }
