@@ -351,6 +351,7 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     CUDA_TRY(cudaMemsetAsync(ws + L.off_counters, 0, L.sync_bytes, stream));
     // every word of the strip-boundary columns starts as the sentinel the consumers poll for (sdtw_kernels.cuh)
     CUDA_TRY(cudaMemsetAsync(ws + L.off_VS, 0xFF, L.vs_bytes, stream));
+    if (pl.want_grad) CUDA_TRY(cudaMemsetAsync(ws + L.off_ES, 0xFF, L.vs_bytes, stream));   // same protocol in reverse
     {
         const long long nx = (long long)pl.offsets[pl.N] * pl.d, nz = (long long)pl.m * pl.d;
         const int blocks = (int)std::min<long long>((nx + nz + 255) / 256, (long long)di.sms * 8);

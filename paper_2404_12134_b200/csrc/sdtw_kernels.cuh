@@ -116,6 +116,9 @@ __device__ __forceinline__ float2 ld_relaxed_f2(const float* p) {
 __device__ __forceinline__ void st_relaxed_f2(float* p, float2 v) {
     asm volatile("st.relaxed.gpu.global.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v.x), "f"(v.y) : "memory");
 }
+__device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {
+    unsigned v; asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
+}
 __device__ __forceinline__ bool is_sentinel(float x) { return __float_as_uint(x) == SENTINEL; }
 
 template <int BYTES>
@@ -670,7 +673,25 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
         // Progress word of an item: chunks completed from the top (C - c after chunk c); when the item is done,
         // FIN | z: every message of its chunks [0, z) is an implicit +0 (they were never visited).
         constexpr unsigned FIN = 0x80000000u;
-        unsigned seen = 0;
+        // Strip-to-strip exchange of the reverse pass, without flags or fences on the way (as in the forward kernel): ES is
+        // preset to the sentinel pattern, the right strip writes its messages with relaxed stores, this strip polls the
+        // DATA words, one chunk ahead of use.  Only the end of an item is published with a release: its progress word
+        // becomes FIN | z, "done, and every message of my chunks [0, z) is an implicit +0 (never written)".
+        unsigned finw = 0;                                     // the right strip's progress word as last seen
+        auto poll_fin = [&]() {
+            if (has_right && !(finw & FIN)) {
+                unsigned f = 0;
+                if (lane == 0) f = ld_acquire(p.prog_b + item + 1);
+                finw = __shfl_sync(FULL, f, 0);
+            }
+        };
+        auto load_msg = [&](const int c) {                     // lane t: the message pair of lane 31's step t of chunk c
+            const int r = c * CROWS - SKEW + 2 * lane;
+            return (has_right && lane < CH && r >= 0) ? ld_relaxed_f2(ESnext + r) : make_float2(0.f, 0.f);
+        };
+        auto peek_fin = [&]() { return (has_right && lane == 0) ? ld_relaxed_u32(p.prog_b + item + 1) : 0u; };
+        float2 ereg = load_msg(cl);
+        unsigned freg = peek_fin();                            // prefetched with the messages; a stale value only delays
         int pf = (cl + 1) * BPC - 1;                           // block whose checkpoint (ph, pv) currently holds
         unsigned long long skipped = 0;
         bool terminated = false;
@@ -679,12 +700,25 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
 #pragma unroll
             for (int w = 0; w < W; ++w) lbits |= __float_as_uint(A[w]);
             const bool local_nz = __any_sync(FULL, lbits != 0u);     // flow already inside this strip
-            if (has_right) {                                   // right strip must have finished chunks >= max(c-LAGC, 0)
-                const unsigned need = (unsigned)(C - max(c - LAGC, 0));
-                while (seen < need) { seen = ld_acquire(p.prog_b + item + 1); if (seen < need) __nanosleep(64); }
+            // lane 31 works on rows c CROWS - SKEW + 2t (+1) at step t; lane t holds its message pair in ereg
+            const int erow = c * CROWS - SKEW + 2 * lane;
+            float2 ein = ereg;
+            if (has_right) {
+                bool bad = is_sentinel(ein.x) || is_sentinel(ein.y);
+                if (__shfl_sync(FULL, freg, 0) & FIN) poll_fin();        // the right strip is done: make that official (acquire)
+                while (__any_sync(FULL, bad)) {
+                    // not published yet -- or never will be: the right strip is done and these rows lie in chunks it
+                    // did not visit (after the acquire in poll_fin every row it did write is visible)
+                    if (bad) {
+                        ein = ld_relaxed_f2(ESnext + erow);
+                        bad = is_sentinel(ein.x) || is_sentinel(ein.y);
+                        if (bad && (finw & FIN) && erow / CROWS < (int)(finw & ~FIN)) { ein = make_float2(0.f, 0.f); bad = false; }
+                    }
+                    if (__any_sync(FULL, bad)) { __nanosleep(64); poll_fin(); }
+                }
             }
-            const bool rfin = (seen & FIN) != 0u;
-            const int zr = (int)(seen & ~FIN);                 // valid when rfin
+            const bool rfin = (finw & FIN) != 0u;
+            const int zr = (int)(finw & ~FIN);                 // valid when rfin
             // Early exit: nothing flows inside this strip and nothing will ever arrive from the right (there is no right
             // strip, or it is done and its remaining messages are implicit zeros): every chunk from here down is a skip.
             if (!p.dense_reverse && !local_nz && (!has_right || (rfin && c < zr))) {
@@ -694,18 +728,13 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
                 terminated = true;
                 break;
             }
-            // lane 31 works on rows c CROWS - SKEW + 2t (+1) at step t; lane t fetches its message pair
-            const int erow = c * CROWS - SKEW + 2 * lane;
-            const float2 ein = (has_right && lane < CH && erow >= 0 && !(rfin && erow / CROWS < zr))
-                                   ? *reinterpret_cast<const float2*>(ESnext + erow) : make_float2(0.f, 0.f);
+            if (c > cf) { ereg = load_msg(c - 1); freg = peek_fin(); }   // prefetch for the next chunk
             // Exact skip: every flow that could enter this chunk's cells is +0 (E underflows to zero off the
             // alignment band), so every product and sum below would be +0 and g would not change.
             if (!p.dense_reverse && !local_nz) {
                 const unsigned bits = __float_as_uint(ein.x) | __float_as_uint(ein.y);
                 if (!__any_sync(FULL, bits != 0u)) {
-                    if (J > 0 && lane < CH) *reinterpret_cast<float2*>(ESme + c * CROWS + 2 * lane) = make_float2(0.f, 0.f);
-                    __syncwarp();
-                    if (lane == 0) st_release(p.prog_b + item, (unsigned)(C - c));
+                    if (J > 0 && lane < CH) st_relaxed_f2(ESme + c * CROWS + 2 * lane, make_float2(0.f, 0.f));
                     ++skipped;
                     continue;
                 }
@@ -749,9 +778,7 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
             }
             __syncwarp();
             // lane 0 worked on rows 64c + 2t (+1) at step t
-            if (J > 0 && lane < CH) *reinterpret_cast<float2*>(ESme + c * CROWS + 2 * lane) = eout_s[lane];
-            __syncwarp();                                      // orders every lane's ES store before lane 0's release
-            if (lane == 0) st_release(p.prog_b + item, (unsigned)(C - c));
+            if (J > 0 && lane < CH) st_relaxed_f2(ESme + c * CROWS + 2 * lane, eout_s[lane]);
         }
         // done: the chunks below cf (above the band) were never visited, their messages are implicit zeros
         if (!terminated) {
