@@ -39,7 +39,7 @@ MUFU_PER_CLK_PER_SM = 16
 ALGO_MUFU_FWD, ALGO_MUFU_BWD = 3, 3          # algorithmic special-function evaluations per cell (2 ex2 + lg2; 3 ex2)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the named kernel at the named config, from the
 # ncu --set full capture summarised in profiles/ (null for workloads without a capture)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {("forward_kernel", 4): 2281825000 + 36702691000}   # profiles/r1c_forward_kernel_cfg4_full.txt
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {("forward_kernel", 4): 2095106000 + 36700662000}   # profiles/r1d_forward_kernel_cfg4_full.txt
 
 
 def workload_string(cfg):
@@ -72,6 +72,13 @@ class ClockSampler:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
         sm, mx, reasons = [], [], set()
+        if not self.lines:                      # timed region shorter than the sampling period: one sample right after it
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=20).stdout
+                self.lines = [l.strip() for l in out.splitlines() if l.strip()]
+            except (OSError, subprocess.SubprocessError):
+                pass
         for ln in self.lines:
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
