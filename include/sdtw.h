@@ -27,7 +27,8 @@
  *     the stream has drained.  Results are bitwise reproducible run to run for fixed inputs (no atomics on data).
  *   - Return value: SDTW_OK (0) or a negative SDTW_ERR_* code.  No exception crosses the ABI.  On an argument error
  *     nothing is enqueued and outputs are untouched.  NaN/Inf in the DATA is not scanned for (it propagates).
- *   - d is supported for 1 <= d <= SDTW_MAX_D (compiled maximum); 1 <= n_k, m < 2^30; 1 <= N < 2^24.
+ *   - d is supported for 1 <= d <= SDTW_MAX_D (compiled maximum; SDTW_DTW_MAX_D for sdtw_dtw_score / sdtw_subdtw);
+ *     1 <= n_k, m < 2^30; 1 <= N < 2^24.
  *   - There is no CPU fallback: on a device that is not compute capability 10.x the calls return SDTW_ERR_UNSUPPORTED.
  */
 #ifndef SDTW_H_
@@ -47,6 +48,7 @@ extern "C" {
 #define SDTW_ERR_CUDA (-4)        /* a CUDA runtime call failed; see sdtw_last_cuda_error()                      */
 
 #define SDTW_MAX_D 4
+#define SDTW_DTW_MAX_D 9 /* sdtw_dtw_score / sdtw_subdtw: the paper's Step 1 aligns all 9 robot variables at once (l.300) */
 
 /*
  * sdtw_value_grad -- eq. 5 and eq. 6 for N pairs (x_k, Z), summed over k.

@@ -55,11 +55,12 @@ struct Layout {
 };
 
 int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, Layout& L, int vs_words = 1) {
+    const int max_d = (vs_words == 2) ? SDTW_DTW_MAX_D : SDTW_MAX_D;   // vs_words == 2: the DTW / Sub-DTW kernels
     if (!offsets || m < 1 || d < 1 || N < 1) return SDTW_ERR_INVALID_ARG;
     if (offsets[0] != 0) return SDTW_ERR_INVALID_ARG;
     for (int k = 0; k < N; ++k)
         if (offsets[k + 1] <= offsets[k]) return SDTW_ERR_INVALID_ARG;
-    if (d > SDTW_MAX_D || m >= (1LL << 30) || N >= (1 << 24)) return SDTW_ERR_UNSUPPORTED;
+    if (d > max_d || m >= (1LL << 30) || N >= (1 << 24)) return SDTW_ERR_UNSUPPORTED;
     for (int k = 0; k < N; ++k)
         if (offsets[k + 1] - offsets[k] >= (1LL << 30)) return SDTW_ERR_UNSUPPORTED;
     L.NS = (int)((m + SW - 1) / SW);
@@ -306,6 +307,11 @@ int dispatch_dtw(int d, const DtwParams& P, int sms, cudaStream_t s) {
         case 2: return launch_dtw<2, SUB>(P, sms, s);
         case 3: return launch_dtw<3, SUB>(P, sms, s);
         case 4: return launch_dtw<4, SUB>(P, sms, s);
+        case 5: return launch_dtw<5, SUB>(P, sms, s);
+        case 6: return launch_dtw<6, SUB>(P, sms, s);
+        case 7: return launch_dtw<7, SUB>(P, sms, s);
+        case 8: return launch_dtw<8, SUB>(P, sms, s);
+        case 9: return launch_dtw<9, SUB>(P, sms, s);
     }
     return SDTW_ERR_UNSUPPORTED;
 }
@@ -389,12 +395,13 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     return SDTW_OK;
 }
 
-int check_common(const void* Z, int64_t m, int32_t d, const void* X, const int64_t* offsets, int32_t N, float gamma) {
+int check_common(const void* Z, int64_t m, int32_t d, const void* X, const int64_t* offsets, int32_t N, float gamma,
+                 int max_d = SDTW_MAX_D) {
     if (!Z || !X || !offsets || m < 1 || d < 1 || N < 1 || !finite_pos(gamma)) return SDTW_ERR_INVALID_ARG;
     if (offsets[0] != 0) return SDTW_ERR_INVALID_ARG;
     for (int k = 0; k < N; ++k)
         if (offsets[k + 1] <= offsets[k]) return SDTW_ERR_INVALID_ARG;
-    if (d > SDTW_MAX_D) return SDTW_ERR_UNSUPPORTED;
+    if (d > max_d) return SDTW_ERR_UNSUPPORTED;
     return SDTW_OK;
 }
 
@@ -609,7 +616,7 @@ int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat,
 
 static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets,
                       int32_t N, float* out_val, int32_t* out_i0, float* out_score, int32_t* out_i1, void* stream_) {
-    int rc = check_common(Z, m, d, X_concat, offsets, N, 1.0f);
+    int rc = check_common(Z, m, d, X_concat, offsets, N, 1.0f, SDTW_DTW_MAX_D);
     if (rc) return rc;
     std::lock_guard<std::mutex> lock(g_mutex);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);

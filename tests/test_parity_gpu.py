@@ -657,3 +657,17 @@ def test_backtracking_equals_fixed_step_when_always_accepted(B):
     assert torch.equal(Zs.cpu(), torch.from_numpy(data["Z0"])) and np.all(ss == 0) and os_[0] == os_[2]
     with pytest.raises(B.SdtwError):
         B.sdtw_barycenter_backtracking(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, 2, 0.1, shrink=1.5)
+
+
+@pytest.mark.parametrize("d", [5, 7, 9])
+def test_dtw_and_subdtw_up_to_nine_channels(B, oracle, d):
+    """The paper's Step 1 aligns all 9 robot variables at once: sdtw_dtw_score / sdtw_subdtw accept
+    d <= SDTW_DTW_MAX_D = 9; the Soft-DTW calls stay at d <= 4."""
+    cfg = dataclasses.replace(synth.CONFIGS[2], N=5, n_lo=500, n_hi=640, m=300, d=d, name=f"d{d}")
+    data = synth.make(cfg, seed=d)
+    _check_dtw(B, oracle, data, cfg.name)
+    _check_subdtw(B, oracle, data["Z0"], data["X"], data["offsets"], cfg.name)
+    if d == 9:
+        with pytest.raises(B.SdtwError) as ei:
+            B.sdtw_value_grad(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], 0.1)
+        assert ei.value.status == B.SDTW_ERR_UNSUPPORTED
