@@ -311,7 +311,9 @@ def run_ours(args):
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": {"workload": workload_string(cfg), "cells_per_step": cells_job, "workspace_gb": ws_bytes / 1e9,
-                       "l2": "no flush: every step streams its checkpoints (workspace) through HBM, far above the 126 MB L2",
+                       "l2": ("no flush: every step streams its checkpoints (workspace) through HBM, far above the 126 MB L2"
+                              if ws_bytes > 4 * 126e6 else
+                              "no flush: small configuration, the working set fits in the 126 MB L2 (latency-bound; not a roofline case)"),
                        "parallelism": f"pairs sharded over {world} GPU(s); all-reduce of m*d gradient" if world > 1 else "single GPU",
                        "tile": B.sdtw_tile_info()},
             "barycenter_iter_s": ms_step * 1e-3,
