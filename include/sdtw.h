@@ -128,6 +128,7 @@ int sdtw_barycenter_backtracking(float* Z_inout, int64_t m, int32_t d, const flo
  *   out_pathlen  dev [N] int32, |pi_k|  (max(n_k, m) <= |pi_k| <= n_k + m - 1); may be NULL
  *   out_score    dev [N] float32, out_dtw[k] / out_pathlen[k]; may be NULL
  * Forward only, full matrix (no band), no special functions; same argument / stream / workspace conventions.
+ * n_k + m must stay below 2^24 (SDTW_ERR_UNSUPPORTED otherwise; the same holds for sdtw_subdtw).
  */
 int sdtw_dtw_score(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
                    float* out_dtw, int32_t* out_pathlen, float* out_score, void* stream);

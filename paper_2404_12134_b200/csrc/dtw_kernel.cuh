@@ -20,6 +20,12 @@
 namespace sdtw {
 
 constexpr int DTW_WARPS = 8;
+#ifndef SDTW_DTW_W
+#define SDTW_DTW_W 4
+#endif
+// columns per thread of the DTW kernels: wider than the Soft-DTW tile (fewer shuffles / boundary words per cell; the cell
+// is cheap and has no special functions to hide); narrower at many channels, where z[DW][D] would spill
+template <int D> __host__ __device__ constexpr int dtw_w() { return D <= 2 ? SDTW_DTW_W : 4; }
 constexpr unsigned F_INF = 0x7f800000u;
 
 struct DtwParams {
@@ -36,7 +42,7 @@ struct DtwParams {
     unsigned num_items;
 };
 
-struct RL { float r; int l; };
+struct RL { float r; float l; };   // l: path length / start row kept as a float (exact below 2^24): its +1 then runs on the FMA pipe, not the ALU pipe that bounds this kernel
 
 __device__ __forceinline__ uint4 ld_relaxed_u4(const unsigned* p) {
     uint4 v;
@@ -52,19 +58,19 @@ template <int D> __host__ __device__ constexpr int dtw_smem_floats() { return 2 
 // one cell: (rd, ld) diagonal, (ru, lu) up [in: old row value of this column; out: this cell], (rl, ll) left [in/out]
 // SUB (Sub-DTW, eq. 2): the integer carried with the minimum is the path's first row (copied), not its length (+1)
 template <int D, bool SUB>
-__device__ __forceinline__ void dtw_cell(const XRow<D>& x, const float (&z)[D], float& rd, int& ld, float& ru, int& lu,
-                                         float& rl, int& ll) {
+__device__ __forceinline__ void dtw_cell(const XRow<D>& x, const float (&z)[D], float& rd, float& ld, float& ru, float& lu,
+                                         float& rl, float& ll) {
     float t = __fsub_rn(x.c[0], z[0]);
     float dist = __fmul_rn(t, t);
 #pragma unroll
     for (int c = 1; c < D; ++c) { t = __fsub_rn(x.c[c], z[c]); dist = __fadd_rn(dist, __fmul_rn(t, t)); }
     const float mn = fminf(fminf(rd, ru), rl);
-    int lsel;                              // first of (diagonal, up, left) that attains the minimum; branch-free
-    asm("{\n\t.reg .pred p, q;\n\t.reg .s32 t;\n\t"
+    float lsel;                            // first of (diagonal, up, left) that attains the minimum; branch-free
+    asm("{\n\t.reg .pred p, q;\n\t.reg .f32 t;\n\t"
         "setp.eq.f32 p, %1, %2;\n\tsetp.eq.f32 q, %3, %2;\n\t"
-        "selp.s32 t, %4, %5, q;\n\tselp.s32 %0, %6, t, p;\n\t}"
-        : "=r"(lsel) : "f"(rd), "f"(mn), "f"(ru), "r"(lu), "r"(ll), "r"(ld));
-    const int l1 = SUB ? lsel : lsel + 1;
+        "selp.f32 t, %4, %5, q;\n\tselp.f32 %0, %6, t, p;\n\t}"
+        : "=f"(lsel) : "f"(rd), "f"(mn), "f"(ru), "f"(lu), "f"(ll), "f"(ld));
+    const float l1 = SUB ? lsel : __fadd_rn(lsel, 1.0f);
     const float rn = __fadd_rn(dist, mn);
     rd = ru; ld = lu;                      // this column's old row value is the next column's diagonal
     ru = rn; lu = l1;
@@ -75,6 +81,7 @@ __device__ __forceinline__ void dtw_cell(const XRow<D>& x, const float (&z)[D], 
 // X_concat) have free ends: r_i0 = 0 for every i, value = min_i r_im, b* = the smallest such i, a* = the path's first row.
 template <int D, bool SUB>
 __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) {
+    constexpr int W = dtw_w<D>();                                    // shadows sdtw::W inside this kernel
     extern __shared__ __align__(16) float smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float* xs0 = smem + warp * dtw_smem_floats<D>();                 // [2][XWIN][D]
@@ -95,20 +102,19 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
         unsigned* VSme = p.VS + pm.vs_off + (long long)J * pm.vs_stride + 2 * VS_PAD;   // word 2 row
         const unsigned* VSprev = VSme - pm.vs_stride;
 
-        float z[W][D], ru[W];
-        int lu[W];
+        float z[W][D], ru[W], lu[W];
 #pragma unroll
         for (int w = 0; w < W; ++w) {
             const int j = j0 + w;
 #pragma unroll
             for (int c = 0; c < D; ++c) z[w][c] = (j < m) ? __ldg(p.Z + (long long)j * D + c) : 0.f;
-            ru[w] = INF; lu[w] = 0;                          // virtual row 0: r_0j = +inf
+            ru[w] = INF; lu[w] = 0.f;                          // virtual row 0: r_0j = +inf
         }
-        RL oA{INF, 0}, oB{INF, 0};                           // this lane's last column, rows 2(s-l) and 2(s-l)+1
-        RL dprev{(J == 0 && lane == 0) ? 0.f : INF, 0};      // diagonal of the first column's upper row; r_00 = 0
+        RL oA{INF, 0.f}, oB{INF, 0.f};                           // this lane's last column, rows 2(s-l) and 2(s-l)+1
+        RL dprev{(J == 0 && lane == 0) ? 0.f : INF, 0.f};      // diagonal of the first column's upper row; r_00 = 0
         const float* xs_lane = xs0;
         const bool last_strip = (J == p.NS - 1);
-        float best = INF; int best_a = 0, best_b = 0;        // Sub-DTW: running min over rows of r in column m - 1
+        float best = INF, best_a = 0.f; int best_b = 0;        // Sub-DTW: running min over rows of r in column m - 1
         auto track = [&](const int i) {
 #pragma unroll
             for (int w = 0; w < W; ++w)
@@ -121,27 +127,27 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
             RL inB{__shfl_up_sync(FULL, oB.r, 1), __shfl_up_sync(FULL, oB.l, 1)};
             if (lane == 0) {
                 const uint4 qv = vin_s[t];
-                inA.r = __uint_as_float(qv.x); inA.l = (int)qv.y; inB.r = __uint_as_float(qv.z); inB.l = (int)qv.w;
+                inA.r = __uint_as_float(qv.x); inA.l = __uint_as_float(qv.y); inB.r = __uint_as_float(qv.z); inB.l = __uint_as_float(qv.w);
             }
             XRow<D> xa, xb;
             load_x2<D>(xs_lane, 2 * t, xa, xb);
             const int i0 = RP * (c * CH + t - lane);
             if (!slow || (unsigned)i0 < (unsigned)n) {
-                float rd = dprev.r, rl = inA.r; int ld = dprev.l, ll = inA.l;
+                float rd = dprev.r, rl = inA.r, ld = dprev.l, ll = inA.l;
 #pragma unroll
                 for (int w = 0; w < W; ++w) dtw_cell<D, SUB>(xa, z[w], rd, ld, ru[w], lu[w], rl, ll);
                 oA.r = rl; oA.l = ll;
                 if (SUB && last_strip) track(i0);
             }
             if (!slow || (unsigned)(i0 + 1) < (unsigned)n) {
-                float rd = inA.r, rl = inB.r; int ld = inA.l, ll = inB.l;
+                float rd = inA.r, rl = inB.r, ld = inA.l, ll = inB.l;
 #pragma unroll
                 for (int w = 0; w < W; ++w) dtw_cell<D, SUB>(xb, z[w], rd, ld, ru[w], lu[w], rl, ll);
                 oB.r = rl; oB.l = ll;
                 if (SUB && last_strip) track(i0 + 1);
             }
             dprev = inB;
-            if (lane == 31) vout_s[t] = make_uint4(__float_as_uint(oA.r), (unsigned)oA.l, __float_as_uint(oB.r), (unsigned)oB.l);
+            if (lane == 31) vout_s[t] = make_uint4(__float_as_uint(oA.r), __float_as_uint(oA.l), __float_as_uint(oB.r), __float_as_uint(oB.l));
         };
 
         stage_x_async<D>(xs0, p.X, pm.x_off, n, 0, lane);
@@ -149,7 +155,7 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
         // column 0 of the border: r_i0 = +inf; Sub-DTW: r_i0 = 0, and a path that enters row i from it starts at row i
         // (the entry of row r is the diagonal predecessor of row r + 1, so it carries r + 1)
         auto border = [&](const int r) {
-            return SUB ? make_uint4(0u, (unsigned)(r + 1), 0u, (unsigned)(r + 2)) : make_uint4(F_INF, 0u, F_INF, 0u);
+            return SUB ? make_uint4(0u, __float_as_uint((float)(r + 1)), 0u, __float_as_uint((float)(r + 2))) : make_uint4(F_INF, 0u, F_INF, 0u);
         };
         uint4 vreg = border(2 * vlane);
         if (J > 0) vreg = ld_relaxed_u4(VSprev + 2 * (2 * vlane));
@@ -191,12 +197,12 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
             if (j0 + w == m - 1) {
                 if (SUB) {
                     if (p.out_dtw) p.out_dtw[pm.k] = best;
-                    if (p.out_len) p.out_len[pm.k] = best_a;
+                    if (p.out_len) p.out_len[pm.k] = (int)best_a;
                     if (p.out_b) p.out_b[pm.k] = best_b;
                 } else {
                     if (p.out_dtw) p.out_dtw[pm.k] = ru[w];
-                    if (p.out_len) p.out_len[pm.k] = lu[w];
-                    if (p.out_score) p.out_score[pm.k] = __fdiv_rn(ru[w], (float)lu[w]);
+                    if (p.out_len) p.out_len[pm.k] = (int)lu[w];
+                    if (p.out_score) p.out_score[pm.k] = __fdiv_rn(ru[w], lu[w]);
                 }
             }
         }

@@ -63,7 +63,8 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
     if (d > max_d || m >= (1LL << 30) || N >= (1 << 24)) return SDTW_ERR_UNSUPPORTED;
     for (int k = 0; k < N; ++k)
         if (offsets[k + 1] - offsets[k] >= (1LL << 30)) return SDTW_ERR_UNSUPPORTED;
-    L.NS = (int)((m + SW - 1) / SW);
+    const int strip_cols = (vs_words == 2) ? 32 * ((d <= 2) ? dtw_w<1>() : dtw_w<4>()) : SW;   // DTW kernels: dtw_kernel.cuh
+    L.NS = (int)((m + strip_cols - 1) / strip_cols);
     L.items = (long long)N * L.NS;
     if (L.items >= (1LL << 31)) return SDTW_ERR_UNSUPPORTED;
     // schedule order: longest cycle first (stable), so the shortest sweeps fill the tail
@@ -618,6 +619,8 @@ static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const floa
                       int32_t N, float* out_val, int32_t* out_i0, float* out_score, int32_t* out_i1, void* stream_) {
     int rc = check_common(Z, m, d, X_concat, offsets, N, 1.0f, SDTW_DTW_MAX_D);
     if (rc) return rc;
+    for (int k = 0; k < N; ++k)          // path lengths / start rows are carried as floats, exact below 2^24
+        if (offsets[k + 1] - offsets[k] + m >= (1LL << 24)) return SDTW_ERR_UNSUPPORTED;
     std::lock_guard<std::mutex> lock(g_mutex);
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     DeviceInfo di;
