@@ -249,8 +249,12 @@ __device__ __forceinline__ float sqdist(const XRow<D>& x, const float (&z)[D]) {
     return acc;
 }
 
-struct FastTag { static constexpr bool slow = false; };
-struct SlowTag { static constexpr bool slow = true; };
+struct FastTag { static constexpr bool slow = false; static constexpr bool val = false; };
+struct SlowTag { static constexpr bool slow = true; static constexpr bool val = true; };
+// fast arithmetic (no bounds / band tests) plus the bookkeeping of the value staircase: the chunks a warp's staircase
+// crosses sit at a different height in every strip, so a slow path there adds its delay to EVERY strip's hand-over and
+// lengthens the whole dependency chain of a pair (it did: 48 instead of 30 us per strip on a cfg-4 pair)
+struct FastValTag { static constexpr bool slow = false; static constexpr bool val = true; };
 
 // chunk c (steps c CH .. c CH + CH-1, rows c CROWS - SKEW .. c CROWS + CROWS-1 over the 32 lanes) touches only valid rows
 __device__ __forceinline__ bool interior_chunk(int c, int n) { return c * CROWS >= SKEW && c * CROWS + CROWS <= n; }
@@ -421,14 +425,22 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
             XRow<D> xa, xb;
             load_x2<D>(xs_lane, 2 * t, xa, xb);
             if constexpr (!slow) {
+                constexpr bool val = decltype(tag)::val;
+                const int i0 = RP * (c * CH + t - lane);   // used by the staircase bookkeeping only
                 float dummy0, dummy1;
 #pragma unroll
                 for (int w = 0; w < W; ++w) {              // cell (A, w+1) and cell (A+1, w) are independent
                     float tl, acc;
                     sqdist2<D>(xa, z[w], tl, acc);
                     cell<false, (D > 1)>(tl, acc, h[w], va, dummy0, dummy1, D <= 2 && ((SDTW_POLY_MASK_A >> w) & 1));
+                    if (val && i0 == r_h && j0 + w >= jlo && j0 + w <= jhi) hsum += h[w];
                     sqdist2<D>(xb, z[w], tl, acc);
                     cell<false, (D > 1)>(tl, acc, h[w], vb, dummy0, dummy1, D <= 2 && ((SDTW_POLY_MASK_B >> w) & 1));
+                    if (val && i0 + 1 == r_h && j0 + w >= jlo && j0 + w <= jhi) hsum += h[w];
+                }
+                if (val) {                                 // same additions, in the same order, as the general row
+                    if ((unsigned)(i0 - r_v0 - 1) < (unsigned)(r_v1 - r_v0)) vacc += va;
+                    if ((unsigned)(i0 - r_v0) < (unsigned)(r_v1 - r_v0)) vacc += vb;
                 }
                 vp0 = va; vp1 = vb;
             } else {
@@ -494,11 +506,19 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
                 if (J > 0) vreg = ld_relaxed_f2(VSprev + rbase + CROWS);
             }
             xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;    // rows of step t: xs_lane[2t], [2t+1]
-            if (interior_chunk(c, n) && (c < c_v0 || c > c_v1) && band_clear(c, J, band)) {
+            const bool inside = interior_chunk(c, n) && band_clear(c, J, band);
+            if (inside && (c < c_v0 || c > c_v1)) {
 #pragma unroll 1
                 for (int b = 0; b < CH / TR; ++b) {
 #pragma unroll
                     for (int u = 0; u < TR; ++u) step(c, b * TR + u, FastTag{});
+                    if (CKPT) checkpoint(c * (CH / TR) + b + 1);
+                }
+            } else if (inside && Tfull > 0) {              // on this warp's value staircase
+#pragma unroll 1
+                for (int b = 0; b < CH / TR; ++b) {
+#pragma unroll
+                    for (int u = 0; u < TR; ++u) step(c, b * TR + u, FastValTag{});
                     if (CKPT) checkpoint(c * (CH / TR) + b + 1);
                 }
             } else {
