@@ -386,8 +386,12 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
         bool vfirst_sel = false;
         if (Tfull == 0 && T == 0) { r_h = n - 1; jlo = 1; jhi = m - 1; r_v0 = 0; r_v1 = n - 1; vfirst_sel = true; }
         else if (T < Tfull) {
-            const int rho_prev = (T == 0) ? 0 : (int)min((long long)(n - 1), (long long)T * W * n / m);
-            const int rho_cur = (T == Tfull - 1) ? n - 1 : (int)min((long long)(n - 1), (long long)(T + 1) * W * n / m);
+            // staircase rows are ODD rows (the second row of a step) wherever possible: a thread's h[] then holds exactly
+            // that row after the step, so the fast path needs no bookkeeping inside its cell loop.  Row n - 1 may be even;
+            // it never lies in an interior chunk, so only the general step meets it.
+            auto rho = [&](const long long Tq) { return min(n - 1, (int)min((long long)(n - 1), Tq * W * n / m) | 1); };
+            const int rho_prev = (T == 0) ? 0 : rho(T);
+            const int rho_cur = (T == Tfull - 1) ? n - 1 : rho(T + 1);
             r_h = rho_prev; jlo = max(1, j0); jhi = j0 + W - 1; r_v0 = rho_prev; r_v1 = rho_cur;
         } else { r_h = n - 1; jlo = j0; jhi = m - 1; r_v0 = r_v1 = n - 1; }
         float vacc = 0.f, hsum = 0.f;
@@ -433,14 +437,16 @@ __global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params 
                     float tl, acc;
                     sqdist2<D>(xa, z[w], tl, acc);
                     cell<false, (D > 1)>(tl, acc, h[w], va, dummy0, dummy1, D <= 2 && ((SDTW_POLY_MASK_A >> w) & 1));
-                    if (val && i0 == r_h && j0 + w >= jlo && j0 + w <= jhi) hsum += h[w];
                     sqdist2<D>(xb, z[w], tl, acc);
                     cell<false, (D > 1)>(tl, acc, h[w], vb, dummy0, dummy1, D <= 2 && ((SDTW_POLY_MASK_B >> w) & 1));
-                    if (val && i0 + 1 == r_h && j0 + w >= jlo && j0 + w <= jhi) hsum += h[w];
                 }
                 if (val) {                                 // same additions, in the same order, as the general row
                     if ((unsigned)(i0 - r_v0 - 1) < (unsigned)(r_v1 - r_v0)) vacc += va;
                     if ((unsigned)(i0 - r_v0) < (unsigned)(r_v1 - r_v0)) vacc += vb;
+                    if (i0 + 1 == r_h) {                   // r_h is odd inside an interior chunk: h[] is that row now
+#pragma unroll
+                        for (int w = 0; w < W; ++w) if (j0 + w >= jlo && j0 + w <= jhi) hsum += h[w];
+                    }
                 }
                 vp0 = va; vp1 = vb;
             } else {
