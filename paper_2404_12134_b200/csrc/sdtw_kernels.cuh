@@ -306,7 +306,7 @@ constexpr int UNIT_RING = 16;
 struct RollCtl { int popped; int lock; int uid[UNIT_RING]; int seen[32]; };
 
 template <int D, bool CKPT, int FW>
-__global__ void __launch_bounds__(FW * 32, 32 / FW) forward_kernel(const Params p) {
+__global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kernel(const Params p) {
     extern __shared__ __align__(16) float smem[];
     __shared__ RollCtl ctl;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
