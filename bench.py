@@ -39,7 +39,7 @@ MUFU_PER_CLK_PER_SM = 16
 ALGO_MUFU_FWD, ALGO_MUFU_BWD = 3, 3          # algorithmic special-function evaluations per cell (2 ex2 + lg2; 3 ex2)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the named kernel at the named config, from the
 # ncu --set full capture summarised in profiles/ (null for workloads without a capture)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {("forward_kernel", 4): 2438845000 + 36700962000}   # profiles/r1e_forward_kernel_cfg4_full.txt
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {("forward_kernel", 4): 2563222000 + 36700025000}   # profiles/r1e_forward_kernel_cfg4_full.txt
 
 
 def workload_string(cfg):
