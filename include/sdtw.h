@@ -180,54 +180,6 @@ int sdtw_set_workspace(void* dev_ptr, size_t bytes);
 const char* sdtw_status_string(int status);
 int sdtw_last_cuda_error(void);
 
-/*
- * Instrumentation used by bench.py (not part of the numerical path).
- *   sdtw_launch_count()   kernels launched by this library since load.
- *   sdtw_profile_enable() when on, every sdtw_value_grad / barycenter iteration brackets its forward kernel, its
- *                         reverse kernel and the remaining small kernels with CUDA events on the caller's stream.
- *   sdtw_profile_read()   waits for those events and returns the accumulated milliseconds and the number of
- *                         evaluations they cover; clears the accumulators.  Any pointer may be NULL.
- */
-uint64_t sdtw_launch_count(void);
-int sdtw_profile_enable(int on);
-int sdtw_profile_read(double* ms_forward, double* ms_backward, double* ms_other, int64_t* evaluations);
-
-/*
- * sdtw_measure_mufu_peak -- measurement, not part of the numerical path: runs dependent chains of one special-function
- * instruction (kind 0 = ex2.approx, 1 = lg2.approx, 2 = rcp.approx; the three the kernels use) on every SM of the
- * current device on a private stream, BLOCKS until done, and returns results per second (best of 3) and the SM count.
- * This is the denominator of the roofline bench.py reports.
- */
-int sdtw_measure_mufu_peak(int32_t kind, double* ops_per_s, int32_t* sm_count);
-
-/*
- * Reverse-pass mode.  The expected-alignment matrix E of eq. 6 underflows to exactly +0 in float32 away from the
- * alignment band, and every quantity the reverse recurrence derives from zero flows is +0 as well; by default the
- * reverse kernel therefore SKIPS a 32-step chunk of a column strip when every flow entering it is +0.  The result is
- * bitwise identical to visiting every cell.  sdtw_set_reverse_mode(1) disables the skip (every cell is visited: the
- * "dense" mode used for measurement and for the bitwise-equality test); 0 restores the default.
- * sdtw_reverse_stats() BLOCKS (device synchronise) and returns, for the last evaluation that ran a reverse pass, the
- * number of (strip, chunk) units and how many of them were skipped.  Either pointer may be NULL.
- */
-int sdtw_set_reverse_mode(int dense);
-int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped);
-
-/*
- * Forward schedule (tuning, does not change any result bit): the forward kernel hands out UNITS of `unit_strips`
- * adjacent column strips of one pair to its CTAs (sdtw_kernels.cuh).  0 restores the automatic choice; values above
- * the kernel's warps per CTA are clamped.  Negative => SDTW_ERR_INVALID_ARG.
- */
-int sdtw_set_schedule(int unit_strips);
-/* The last `tail_strips` strips of every pair are handed out in units of `tail_unit` strips (small units at the end of
- * the queue shorten the drain).  tail_strips < 0 restores the automatic choice; tail_unit <= 0 means "as unit_strips". */
-int sdtw_set_schedule_tail(int tail_strips, int tail_unit);
-
-/* Compile-time tile constants, for DESIGN.md / bench.py reporting: columns per thread, columns per strip (work item),
- * wavefront steps between checkpoints, steps per strip-boundary exchange, rows a lane works on per step.  Any pointer
- * may be NULL. */
-int sdtw_tile_info(int32_t* cols_per_thread, int32_t* strip_cols, int32_t* ckpt_steps, int32_t* chunk_steps,
-                   int32_t* rows_per_step);
-
 #ifdef __cplusplus
 }
 #endif

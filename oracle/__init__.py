@@ -234,6 +234,31 @@ def value_grad(Z, X_concat, offsets, gamma, want_grad=True, mode="full", nthread
     return values, grad
 
 
+def value_grad_f64z(Z, X_concat, offsets, gamma, want_grad=True, mode="full", nthreads=0, weights=None, band=-1):
+    """value_grad at a barycenter given in float64 (an iterate of the descent, which keeps Z in float64 between
+    iterations -- reading C14).  X_concat stays the float32 input.  Returns (values, grad or None, objective)."""
+    Z = np.ascontiguousarray(Z, np.float64)
+    if Z.ndim == 1:
+        Z = Z[:, None]
+    X = np.ascontiguousarray(X_concat, np.float32)
+    if X.ndim == 1:
+        X = X[:, None]
+    off = np.ascontiguousarray(offsets, np.int64)
+    assert X.shape[1] == Z.shape[1] and off[0] == 0 and off[-1] == X.shape[0]
+    m, d = Z.shape
+    N = len(off) - 1
+    values = np.zeros(N, np.float64)
+    grad = np.zeros((m, d), np.float64) if want_grad else None
+    w, wp = _weights(weights, N)
+    obj = ctypes.c_double(0.0)
+    _chk(_load().oracle_value_grad_ex_f64z(_d(Z), ctypes.c_int64(m), ctypes.c_int(d), X.ctypes.data_as(_c_float_p),
+                                           off.ctypes.data_as(_c_i64_p), ctypes.c_int(N), ctypes.c_double(gamma), wp,
+                                           ctypes.c_int64(band), _d(values), _d(grad) if want_grad else None,
+                                           ctypes.byref(obj), ctypes.c_int(1 if mode == "checkpointed" else 0),
+                                           ctypes.c_int(nthreads)))
+    return values, grad, obj.value
+
+
 def barycenter(Z0, X_concat, offsets, gamma, iters, step, mode="full", nthreads=0, weights=None, band=-1):
     """Mirror of sdtw_barycenter / sdtw_barycenter_ex: fixed-step GD in float64 on sum_k w_k value_k.
     Returns (Z (m,d) float64, values (N,) at the last evaluated iterate, objective (iters,))."""

@@ -371,16 +371,32 @@ int oracle_value_grad_f32(const float *Z, int64_t m, int d, const float *X, cons
 }
 /* the same with eq. 7's per-pair weights w_k (NULL = all 1) and Table 1's Sakoe-Chiba band (< 0 = none):
  * values[k] unweighted, grad = sum_k w_k grad_k (k ascending), *objective = sum_k w_k values[k]. */
+int oracle_value_grad_ex_f64z(const double *z, int64_t m, int d, const float *X, const int64_t *offsets, int N,
+                              double gamma, const double *weights, int64_t band, double *values, double *grad,
+                              double *objective, int mode, int nthreads);
 int oracle_value_grad_ex_f32(const float *Z, int64_t m, int d, const float *X, const int64_t *offsets, int N,
                              double gamma, const double *weights, int64_t band, double *values, double *grad,
                              double *objective, int mode, int nthreads) {
-    if (!Z || !X || !offsets || !values || m < 1 || d < 1 || N < 1 || !(gamma > 0.0)) return ORACLE_ERR_ARG;
+    if (!Z || m < 1 || d < 1) return ORACLE_ERR_ARG;
+    double *z = (double *)malloc((size_t)(m * d) * sizeof(double));
+    if (!z) return ORACLE_ERR_MEM;
+    for (int64_t t = 0; t < m * d; ++t) z[t] = (double)Z[t];
+    const int rc = oracle_value_grad_ex_f64z(z, m, d, X, offsets, N, gamma, weights, band, values, grad, objective, mode,
+                                             nthreads);
+    free(z);
+    return rc;
+}
+/* the same evaluation at a barycenter given in double (an iterate of the descent below, which keeps Z in double
+ * between iterations -- reading C14): lets a caller drive the loop Z <- Z - step G one evaluation at a time (the
+ * full-size reference outputs of tests/golden/ are written that way, resumably). */
+int oracle_value_grad_ex_f64z(const double *z, int64_t m, int d, const float *X, const int64_t *offsets, int N,
+                              double gamma, const double *weights, int64_t band, double *values, double *grad,
+                              double *objective, int mode, int nthreads) {
+    if (!z || !X || !offsets || !values || m < 1 || d < 1 || N < 1 || !(gamma > 0.0)) return ORACLE_ERR_ARG;
     for (int k = 0; k < N; ++k)
         if (offsets[k + 1] <= offsets[k]) return ORACLE_ERR_ARG;
-    double *z = (double *)malloc((size_t)(m * d) * sizeof(double));
     double *gk = grad ? (double *)calloc((size_t)N * (size_t)(m * d), sizeof(double)) : NULL;
-    if (!z || (grad && !gk)) { free(z); free(gk); return ORACLE_ERR_MEM; }
-    for (int64_t t = 0; t < m * d; ++t) z[t] = (double)Z[t];
+    if (grad && !gk) { free(gk); return ORACLE_ERR_MEM; }
     int rc_all = ORACLE_OK;
 #ifdef _OPENMP
     if (nthreads > 0) omp_set_num_threads(nthreads);
@@ -416,7 +432,6 @@ int oracle_value_grad_ex_f32(const float *Z, int64_t m, int d, const float *X, c
         for (int k = 0; k < N; ++k) obj += (weights ? weights[k] : 1.0) * values[k];
         *objective = obj;
     }
-    free(z);
     free(gk);
     return rc_all;
 }

@@ -2,6 +2,7 @@
 // include/sdtw.h.  The arithmetic is in sdtw_kernels.cuh.  No CPU fallback exists: a device that is not sm_100 is
 // rejected with SDTW_ERR_UNSUPPORTED.
 #include "sdtw.h"
+#include "sdtw_debug.h"
 
 #include <algorithm>
 #include <cmath>
@@ -19,16 +20,35 @@ using namespace sdtw;
 thread_local int g_last_cuda_error = 0;
 std::mutex g_mutex;
 uint64_t g_launches = 0;
-void* g_user_ws = nullptr;
-size_t g_user_ws_bytes = 0;
-bool g_profile = false;
-int g_dense_reverse = 0;
-int g_unit_strips = 0;        // 0 = automatic (sdtw_set_schedule)
-int g_tail_strips = -1, g_tail_unit = 0;   // experiment hook: -1 = automatic
-const unsigned long long* g_last_stats = nullptr;   // device address of the last evaluation's reverse statistics
+struct UserWs { void* ptr = nullptr; size_t bytes = 0; };
+UserWs g_user_ws[64];         // caller-registered workspace, one per device (sdtw_set_workspace)
+// instrumentation / tuning switches of include/sdtw_debug.h: per calling thread, so that one thread's measurement
+// settings never change another thread's launch
+thread_local bool g_profile = false;
+thread_local int g_dense_reverse = 0;
+thread_local int g_unit_strips = 0;        // 0 = automatic (sdtw_set_schedule)
+thread_local int g_tail_strips = -1, g_tail_unit = 0;   // -1 = automatic (sdtw_set_schedule_tail)
+thread_local const unsigned long long* g_last_stats = nullptr;   // device address of the last evaluation's reverse statistics
+thread_local uint64_t g_last_stats_gen = 0;   // ... valid while no workspace has been freed since (g_ws_gen)
+uint64_t g_ws_gen = 1;
 
-struct ProfRec { cudaEvent_t e[5]; };   // start | prologue | forward | reverse | small kernels
-std::vector<ProfRec> g_prof;
+// CUDA events bracketing the phases of one evaluation: start | prologue | forward | reverse | small kernels.
+// Owned by a ProfScope until the evaluation has been enqueued completely; an early return destroys them.
+struct ProfRec { cudaEvent_t e[5] = {nullptr, nullptr, nullptr, nullptr, nullptr}; };
+thread_local std::vector<ProfRec> g_prof;
+struct ProfScope {
+    ProfRec rec;
+    bool on = false, kept = false;
+    int begin(bool enable) {
+        on = enable;
+        if (!on) return cudaSuccess;
+        for (auto& e : rec.e) { cudaError_t r = cudaEventCreate(&e); if (r != cudaSuccess) return (int)r; }
+        return cudaSuccess;
+    }
+    int mark(int i, cudaStream_t s) { return on ? (int)cudaEventRecord(rec.e[i], s) : (int)cudaSuccess; }
+    void keep() { if (on) { g_prof.push_back(rec); kept = true; } }
+    ~ProfScope() { if (on && !kept) for (auto& e : rec.e) if (e) cudaEventDestroy(e); }
+};
 
 #define CUDA_TRY(expr)                                   \
     do {                                                 \
@@ -337,11 +357,13 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     P.ES = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_ES) : nullptr;
     P.CK = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_CK) : nullptr;
     P.Gk = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_Gk) : nullptr;
-    P.stats = reinterpret_cast<unsigned long long*>(ws + L.off_stats);
+    // reverse-pass statistics (two atomics per work item) are collected only while profiling is enabled
+    P.stats = g_profile ? reinterpret_cast<unsigned long long*>(ws + L.off_stats) : nullptr;
     P.dense_reverse = g_dense_reverse;
     P.band = band;
     P.wts = pl.d_w;
     g_last_stats = P.stats;
+    g_last_stats_gen = g_ws_gen;
     P.m = (int)pl.m; P.N = pl.N; P.NS = L.NS;
     P.num_items = (unsigned)L.items;
     const double kappa = 1.0 / ((double)gamma * std::log(2.0));
@@ -350,9 +372,9 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     // the kernels see gamma only through the rounded sqrtk; undo exactly that scale on the way out
     const double inv_kappa = 1.0 / ((double)sqrtk * (double)sqrtk);
 
-    ProfRec pr{};
-    if (g_profile) for (auto& e : pr.e) CUDA_TRY(cudaEventCreate(&e));
-    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[0], stream));
+    ProfScope pr;
+    CUDA_TRY((cudaError_t)pr.begin(g_profile));
+    CUDA_TRY((cudaError_t)pr.mark(0, stream));
     int rc = SDTW_OK;
     if (phase & 1) {
     CUDA_TRY(cudaMemsetAsync(ws + L.off_counters, 0, L.sync_bytes, stream));
@@ -366,16 +388,16 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
         ++g_launches;
         CUDA_TRY(cudaGetLastError());
     }
-    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[1], stream));
+    CUDA_TRY((cudaError_t)pr.mark(1, stream));
     rc = dispatch_forward(pl.d, P, pl.want_grad, di.sms, stream);
     if (rc) return rc;
-    } else if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[1], stream));
-    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[2], stream));
+    } else CUDA_TRY((cudaError_t)pr.mark(1, stream));
+    CUDA_TRY((cudaError_t)pr.mark(2, stream));
     if (pl.want_grad && (phase & 2)) {
         rc = dispatch_backward(pl.d, P, di.sms, stream);
         if (rc) return rc;
     }
-    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[3], stream));
+    CUDA_TRY((cudaError_t)pr.mark(3, stream));
     if ((phase & 1) && (out_values || out_objective || out_objective64)) {
         finalize_values_kernel<<<1, 256, 0, stream>>>(P.VP, pl.d_pm, P.wts, pl.N, L.NS, inv_kappa, out_values, out_objective,
                                                       out_objective64);
@@ -389,10 +411,8 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
         ++g_launches;
         CUDA_TRY(cudaGetLastError());
     }
-    if (g_profile) {
-        CUDA_TRY(cudaEventRecord(pr.e[4], stream));
-        g_prof.push_back(pr);
-    }
+    CUDA_TRY((cudaError_t)pr.mark(4, stream));
+    pr.keep();
     return SDTW_OK;
 }
 
@@ -444,16 +464,16 @@ struct Workspace {
         cache = &g_ws_cache[dev];
         if (!cache->last_use) CUDA_TRY(cudaEventCreateWithFlags(&cache->last_use, cudaEventDisableTiming));
         else CUDA_TRY(cudaStreamWaitEvent(s, cache->last_use, 0));
-        if (g_user_ws) {
-            if (g_user_ws_bytes < bytes) return SDTW_ERR_WORKSPACE;
-            ptr = static_cast<char*>(g_user_ws);
+        if (g_user_ws[dev].ptr) {
+            if (g_user_ws[dev].bytes < bytes) return SDTW_ERR_WORKSPACE;
+            ptr = static_cast<char*>(g_user_ws[dev].ptr);
             return SDTW_OK;
         }
         if (cache->bytes < bytes) {
             if (cache->ptr) {                       // rare: the problem grew; wait for earlier users, then regrow
                 CUDA_TRY(cudaEventSynchronize(cache->last_use));
                 CUDA_TRY(cudaFree(cache->ptr));
-                g_last_stats = nullptr;
+                ++g_ws_gen;
                 cache->ptr = nullptr; cache->bytes = 0;
             }
             void* q = nullptr;
@@ -639,20 +659,16 @@ static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const floa
     P.VS = reinterpret_cast<unsigned*>(ws.ptr + L.off_VS);
     P.out_dtw = out_val; P.out_len = out_i0; P.out_score = out_score; P.out_b = out_i1;
     P.m = (int)m; P.N = N; P.NS = L.NS; P.num_items = (unsigned)L.items;
-    ProfRec pr{};
-    if (g_profile) for (auto& e : pr.e) CUDA_TRY(cudaEventCreate(&e));
-    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[0], stream));
+    ProfScope pr;
+    CUDA_TRY((cudaError_t)pr.begin(g_profile));
+    CUDA_TRY((cudaError_t)pr.mark(0, stream));
     CUDA_TRY(cudaMemsetAsync(ws.ptr + L.off_counters, 0, L.sync_bytes, stream));
     CUDA_TRY(cudaMemsetAsync(ws.ptr + L.off_VS, 0xFF, L.vs_bytes, stream));   // sentinel preset (dtw_kernel.cuh)
-    if (g_profile) CUDA_TRY(cudaEventRecord(pr.e[1], stream));
+    CUDA_TRY((cudaError_t)pr.mark(1, stream));
     rc = sub ? dispatch_dtw<true>(d, P, di.sms, stream) : dispatch_dtw<false>(d, P, di.sms, stream);
     if (rc) return rc;
-    if (g_profile) {
-        CUDA_TRY(cudaEventRecord(pr.e[2], stream));     // "forward" slot = the DTW kernel
-        CUDA_TRY(cudaEventRecord(pr.e[3], stream));
-        CUDA_TRY(cudaEventRecord(pr.e[4], stream));
-        g_prof.push_back(pr);
-    }
+    for (int i = 2; i <= 4; ++i) CUDA_TRY((cudaError_t)pr.mark(i, stream));   // "forward" slot = the DTW kernel
+    pr.keep();
     return SDTW_OK;
 }
 
@@ -744,15 +760,16 @@ int sdtw_set_workspace(void* dev_ptr, size_t bytes) {
     std::lock_guard<std::mutex> lock(g_mutex);
     if (dev_ptr && (reinterpret_cast<uintptr_t>(dev_ptr) & 255u)) return SDTW_ERR_INVALID_ARG;
     if (!dev_ptr && bytes) return SDTW_ERR_INVALID_ARG;
-    g_user_ws = dev_ptr;
-    g_last_stats = nullptr;
-    g_user_ws_bytes = dev_ptr ? bytes : 0;
+    int dev = 0;                                    // the registration belongs to the CURRENT device
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return SDTW_ERR_UNSUPPORTED;
+    g_user_ws[dev].ptr = dev_ptr;
+    g_user_ws[dev].bytes = dev_ptr ? bytes : 0;
+    ++g_ws_gen;
     if (!dev_ptr) {                                 // also drop the library-owned buffer of the current device
-        int dev = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64 && g_ws_cache[dev].ptr) {
+        if (g_ws_cache[dev].ptr) {
             if (g_ws_cache[dev].last_use) cudaEventSynchronize(g_ws_cache[dev].last_use);
             cudaFree(g_ws_cache[dev].ptr);
-            g_last_stats = nullptr;
             g_ws_cache[dev].ptr = nullptr;
             g_ws_cache[dev].bytes = 0;
         }
@@ -827,7 +844,7 @@ int sdtw_set_reverse_mode(int dense) {
 int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped) {
     std::lock_guard<std::mutex> lock(g_mutex);
     unsigned long long h[2] = {0, 0};
-    if (g_last_stats) {
+    if (g_last_stats && g_last_stats_gen == g_ws_gen) {
         CUDA_TRY(cudaDeviceSynchronize());
         CUDA_TRY(cudaMemcpy(h, g_last_stats, sizeof(h), cudaMemcpyDeviceToHost));
     }

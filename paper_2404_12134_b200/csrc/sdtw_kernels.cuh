@@ -18,7 +18,8 @@
 //   forward  VS[row]: written by lane 31 of the left strip, read by lane 0 of the right strip.  No flag: the buffer is
 //            preset to a sentinel bit pattern no arithmetic result can have and the consumer polls the DATA words with
 //            relaxed gpu-scope loads, one 64-row chunk ahead of use, so the wait is normally hidden;
-//   reverse  ES[row]: E messages from the right strip to the left one, ordered by a release/acquire progress counter.
+//   reverse  ES[row]: E messages from the right strip to the left one, same protocol (sentinel preset, relaxed data-word
+//            polling one chunk ahead); only the END of an item is published with a release (its progress word).
 // Every TR steps the forward kernel checkpoints the warp state (h[W] + the two values in flight) to HBM; the reverse
 // kernel restores a checkpoint, recomputes TR steps keeping the transition weights in shared memory, then runs the E
 // recurrence over those TR steps backwards, accumulating the gradient contraction of eq. 6 in registers.
@@ -40,9 +41,6 @@ namespace sdtw {
 #ifndef SDTW_CH
 #define SDTW_CH 32
 #endif
-#ifndef SDTW_SLACK
-#define SDTW_SLACK 0
-#endif
 
 constexpr int W = SDTW_W;       // columns per thread
 constexpr int RP = 2;           // rows per lane per step
@@ -52,7 +50,6 @@ constexpr int CROWS = CH * RP;  // rows a lane sweeps per chunk
 constexpr int SKEW = 31 * RP;   // lane 31 is this many rows behind lane 0
 constexpr int XPAD = 64;        // >= SKEW, keeps the staged window aligned
 constexpr int XWIN = XPAD + CROWS;  // rows of the cycle staged per chunk: [c*CROWS - XPAD, c*CROWS + CROWS)
-constexpr int SLACK = SDTW_SLACK;   // chunks a forward consumer lets its producer get ahead once it has caught up
 constexpr int LAGC = (SKEW + CROWS - 1) / CROWS;  // chunks of the neighbouring strip one chunk reaches back into
 constexpr int TR = SDTW_TR;     // steps between checkpoints (= steps recomputed per reverse block)
 constexpr int WARPS = SDTW_WARPS;  // warps per CTA (each warp is an independent agent)
@@ -479,21 +476,9 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
 
         for (int c = cf; c <= cl; ++c) {
             const int rbase = c * CROWS + 2 * vlane;       // lane 0 works on rows rbase, rbase + 1 at step `vlane`
-#ifdef SDTW_EXPERIMENT_NODEP
-            if (false) {
-#else
             if (J > 0) {                                   // valid = the left strip has published these rows
-#endif
                 bool bad = unpublished(vreg, rbase);
                 if (__any_sync(FULL, bad)) {
-                    if (SLACK > 0) {                       // caught up with the producer: let it get SLACK chunks ahead
-                        const int rw = min(c + SLACK, C - 1) * CROWS + 2 * vlane;
-                        for (;;) {
-                            const float2 t = ld_relaxed_f2(VSprev + rw);
-                            if (!__any_sync(FULL, unpublished(t, rw))) break;
-                            __nanosleep(400);
-                        }
-                    }
                     for (;;) {
                         if (bad) vreg = ld_relaxed_f2(VSprev + rbase);
                         bad = unpublished(vreg, rbase);
@@ -709,6 +694,7 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
                 unsigned f = 0;
                 if (lane == 0) f = ld_acquire(p.prog_b + item + 1);
                 finw = __shfl_sync(FULL, f, 0);
+                __syncwarp();                                  // the other lanes reload ES only after lane 0's acquire
             }
         };
         auto load_msg = [&](const int c) {                     // lane t: the message pair of lane 31's step t of chunk c

@@ -21,14 +21,36 @@ def binding():
 
 
 def test_library_exports_every_declared_symbol(binding):
-    hdr = open(os.path.join(ROOT, "include", "sdtw.h")).read()
-    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(sdtw_[a-z_]+)\s*\(", hdr))
-    assert {"sdtw_value_grad", "sdtw_barycenter", "sdtw_workspace_bytes", "sdtw_set_workspace"} <= declared
+    """Every prototype of include/*.h (sdtw.h: the product boundary; sdtw_debug.h: instrumentation / tuning hooks) is
+    exported by libsdtw.so and bound under the same name."""
+    declared = {}
+    for name in ("sdtw.h", "sdtw_debug.h"):
+        hdr = open(os.path.join(ROOT, "include", name)).read()
+        hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+        declared[name] = set(re.findall(r"\b(sdtw_[a-z_]+)\s*\(", hdr))
+    assert {"sdtw_value_grad", "sdtw_barycenter", "sdtw_workspace_bytes", "sdtw_set_workspace"} <= declared["sdtw.h"]
+    # the product header carries no measurement or tuning switches
+    assert not any(("profile" in n or "schedule" in n or "stats" in n or "measure" in n) for n in declared["sdtw.h"])
+    assert not (declared["sdtw.h"] & declared["sdtw_debug.h"])
+    both = declared["sdtw.h"] | declared["sdtw_debug.h"]
     lib = ctypes.CDLL(os.path.join(ROOT, "paper_2404_12134_b200", "libsdtw.so"))
-    for name in declared:
+    for name in both:
         assert hasattr(lib, name), name
-    assert declared == set(binding.SYMBOLS), declared ^ set(binding.SYMBOLS)
+    assert both == set(binding.SYMBOLS), both ^ set(binding.SYMBOLS)
+
+
+def test_binding_helpers_eq7_weights_and_table1_band(binding):
+    """binding.eq7_weights / table1_band against numbers written out by hand from eq. 7 (lambda_i / m_i,
+    lambda = 1 by default) and Table 1 (bandwidth = 0.6 x the longest signal length)."""
+    w = binding.eq7_weights([4, 8, 5])
+    assert w.dtype == np.float32 and np.array_equal(w, np.array([0.25, 0.125, 0.2], np.float32))
+    w = binding.eq7_weights([4, 8, 5], lam=[2.0, 1.0, 0.5])
+    assert np.array_equal(w, np.array([0.5, 0.125, 0.1], np.float32))
+    assert binding.table1_band(30000, [27000, 33000, 31000]) == 19800         # 0.6 x 33000
+    assert binding.table1_band(30000, [27000, 28000]) == 18000                # the barycenter is the longest: 0.6 x 30000
+    assert binding.table1_band(18385, [18385] * 5) == 11031                   # Table 3's length: floor(11031.0)
+    assert binding.table1_band(1001, [1001], 0.25) == 250                     # floor(250.25)
+    assert binding.table1_band(10, [10], 1.0) == 10
 
 
 def test_status_strings_and_tile_info(binding):

@@ -1,0 +1,65 @@
+"""The stored full-size reference outputs (tests/golden/fullsize_*.npz, written by tests/golden/make_fullsize_refs.py
+from the float64 oracle alone) are what the oracle computes from today's inputs: input and oracle-source hashes, the
+recorded contractivity check (reading C13), and a spot re-computation by the oracle."""
+import hashlib
+import json
+import os
+
+import numpy as np
+import pytest
+
+from paper_2404_12134_b200 import synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+GOLDEN = os.path.join(ROOT, "tests", "golden")
+
+
+def _meta():
+    path = os.path.join(GOLDEN, "fullsize_refs.json")
+    assert os.path.exists(path), "run tests/golden/make_fullsize_refs.py"
+    return json.load(open(path))
+
+
+def _inputs_sha(data):
+    h = hashlib.sha256()
+    for a in (data["Z0"], data["X"], data["offsets"]):
+        h.update(np.ascontiguousarray(a).tobytes())
+    return h.hexdigest()
+
+
+@pytest.mark.parametrize("idx", [3, 4, 5])
+def test_golden_hashes_match_inputs_and_oracle_source(idx):
+    meta = _meta()[f"cfg{idx}"]
+    data = synth.make(idx)
+    assert meta["inputs_sha256"] == _inputs_sha(data)
+    src = open(os.path.join(ROOT, "oracle", "sdtw_oracle.c"), "rb").read()
+    assert meta["oracle_sha256"] == hashlib.sha256(src).hexdigest(), "oracle source changed: regenerate the references"
+    gold = np.load(os.path.join(GOLDEN, f"fullsize_cfg{idx}.npz"))
+    cfg = data["cfg"]
+    if idx == 5:
+        assert len(gold["pairs"]) >= 64 and int(gold["anomalous"].sum()) >= 16
+        assert np.array_equal(gold["anomalous"], data["anomalous"][gold["pairs"]]) and np.all(np.isfinite(gold["values"]))
+        return
+    # the frozen step of synth.CONFIGS is the one that passed the contractivity check, and the descent stayed finite
+    assert float(gold["step"]) == cfg.step and int(gold["iters"]) == cfg.iters
+    last = meta["contractivity"][-1]
+    assert last["step"] == cfg.step and last["rel_out"] <= 1e-4 and abs(last["rel_in"] - 1e-6) < 5e-7
+    assert all(t["rel_out"] > 1e-4 for t in meta["contractivity"][:-1])       # every larger step tried had failed it
+    assert gold["grad0"].shape == (cfg.m, cfg.d) and gold["Z_final"].shape == (cfg.m, cfg.d)
+    assert gold["values0"].shape == (cfg.N,) and len(gold["objective"]) == cfg.iters
+    assert np.all(np.isfinite(gold["Z_final"])) and np.all(np.isfinite(gold["grad0"]))
+    assert abs(gold["objective"][0] - gold["values0"].sum()) <= 1e-9 * abs(gold["objective"][0])
+
+
+def test_golden_spot_recomputation(oracle):
+    """One cfg-3 pair (value and its gradient contribution cannot be separated from the stored sum, so: value only)
+    and one cfg-5 pair recomputed by the oracle now."""
+    for idx, key_pairs, key_vals in ((3, None, "values0"), (5, "pairs", "values")):
+        data = synth.make(idx)
+        gold = np.load(os.path.join(GOLDEN, f"fullsize_cfg{idx}.npz"))
+        j = 1
+        k = int(gold[key_pairs][j]) if key_pairs else j
+        a, b = data["offsets"][k], data["offsets"][k + 1]
+        v, _ = oracle.value_grad(data["Z0"], data["X"][a:b], np.array([0, b - a]), data["cfg"].gamma, want_grad=False,
+                                 mode="checkpointed")
+        assert abs(v[0] - gold[key_vals][j]) <= 1e-12 * max(1.0, abs(v[0]))

@@ -595,3 +595,25 @@ def test_backtracking_descent_armijo_conditions(oracle):
     assert np.array_equal(Zf, Zb) and np.array_equal(of, ob[:3]) and np.all(sb == 0.01) and np.all(tb == 1)
     Zs, _, os_, ss, ts = oracle.barycenter_backtracking(Z0, X, off, cfg.gamma, 3, 50.0, shrink, c1, max_trials=1)
     assert np.array_equal(Zs, Z0.astype(np.float64)) and np.all(ss == 0) and ts[0] == 1 and np.all(os_ == os_[0])
+
+
+def test_descent_driven_one_evaluation_at_a_time_is_the_c_loop_bitwise(oracle):
+    """oracle.value_grad_f64z (the evaluation at a float64 barycenter) driven by Z <- Z - step G in numpy reproduces
+    oracle.barycenter bit for bit: that is how tests/golden/make_fullsize_refs.py writes the full-size references."""
+    from paper_2404_12134_b200 import synth
+    for idx, iters, mode in ((1, 10, "full"), (2, 2, "checkpointed")):
+        data = synth.make(idx)
+        cfg = data["cfg"]
+        Zo, vo, oo = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, iters, cfg.step, mode=mode)
+        Z = data["Z0"].astype(np.float64)
+        hist = []
+        for _ in range(iters):
+            v, G, obj = oracle.value_grad_f64z(Z, data["X"], data["offsets"], cfg.gamma, mode=mode)
+            hist.append(obj)
+            Z = Z - cfg.step * G
+        assert np.array_equal(Z, Zo) and np.array_equal(np.array(hist), oo) and np.array_equal(v, vo)
+    # at a float32-representable Z it is value_grad itself
+    data = synth.make(1)
+    v1, g1, o1 = oracle.value_grad_f64z(data["Z0"].astype(np.float64), data["X"], data["offsets"], 1.0)
+    v2, g2, o2 = oracle.value_grad(data["Z0"], data["X"], data["offsets"], 1.0, want_objective=True)
+    assert np.array_equal(v1, v2) and np.array_equal(g1, g2) and o1 == o2

@@ -1,9 +1,14 @@
 """Parity of the CUDA path (through the C ABI of include/sdtw.h) with the float64 oracle.
 
 Tolerances (BASELINE.json north_star):
-  per-pair values : |v - v*| <= 1e-4 * max(|v*|, gamma (n_k + m))      (reading C10; the strict |v*| ratio is printed)
-  summed gradient : ||G - G*||_2 <= 2e-3 ||G*||_2
-  barycenter      : ||Z - Z*||_2 <= 2e-3 ||Z*||_2  after the configured iterations
+  per-pair values : |v - v*| <= 1e-4 * max(|v*|, gamma (n_k + m))      (reading C10), and the strict ratio
+                    |v - v*| <= 1e-4 |v*| wherever |v*| is not tiny (|v*| >= 0.05 gamma (n_k + m): value = path cost
+                    minus gamma x entropy, two terms of that size that cancel -- below that the strict ratio measures
+                    the cancellation, not the arithmetic)
+  summed gradient : ||G - G*||_2 <= 2e-3 ||G*||_2, and max_j |G_j - G*_j| <= 2e-3 max_j |G*_j| (a fault confined to
+                    one strip-boundary column is invisible to the L2 norm); the worst column modulo 128 is printed
+  barycenter      : ||Z - Z*||_2 <= 2e-3 ||Z*||_2 after the configured iterations, and ||Z - Z*|| <= 5e-2 ||Z* - Z0||
+                    (error relative to the distance moved; the first one is nearly vacuous when Z barely moves)
 """
 import dataclasses
 import os
@@ -16,6 +21,9 @@ from paper_2404_12134_b200 import synth
 pytestmark = pytest.mark.gpu
 
 VAL_TOL, GRAD_TOL, BARY_TOL = 1e-4, 2e-3, 2e-3
+GRAD_MAX_TOL = 2e-3          # max-norm companion of the gradient bar
+MOVED_TOL = 5e-2             # barycenter error relative to the distance moved
+STRICT_FLOOR = 0.05          # strict value ratio asserted where |v*| >= STRICT_FLOOR * gamma (n + m)
 
 
 @pytest.fixture(scope="module")
@@ -37,11 +45,39 @@ def rel_l2(a, b):
 
 def check_values(v, ov, lengths, cfg, tag=""):
     v = np.asarray(v, np.float64)
-    den = np.maximum(np.abs(ov), cfg.gamma * (np.asarray(lengths) + cfg.m))
+    scale = cfg.gamma * (np.asarray(lengths) + cfg.m)
+    den = np.maximum(np.abs(ov), scale)
     err = np.abs(v - ov) / den
     strict = np.abs(v - ov) / np.maximum(np.abs(ov), 1e-300)
-    print(f"[{tag}] values: C10 rel max {err.max():.3e}, strict rel max {strict.max():.3e}")
+    big = np.abs(ov) >= STRICT_FLOOR * scale
+    print(f"[{tag}] values: C10 rel max {err.max():.3e}, strict rel max {strict.max():.3e} "
+          f"(asserted on {int(big.sum())} of {len(ov)}: max {strict[big].max() if big.any() else 0.0:.3e})")
     assert err.max() <= VAL_TOL, (tag, err.max())
+    assert (not big.any()) or strict[big].max() <= VAL_TOL, (tag, strict[big].max())
+
+
+def check_grad(G, oG, tag=""):
+    """relative L2 and max-norm; prints the column of the largest deviation modulo 128 (the strip width: a fault at a
+    strip boundary shows up as 0 or 127)."""
+    G = np.asarray(G, np.float64).reshape(oG.shape)
+    e = rel_l2(G, oG)
+    dev = np.abs(G - oG)
+    emax = float(dev.max() / max(np.abs(oG).max(), 1e-300))
+    j = int(np.unravel_index(np.argmax(dev), dev.shape)[0])
+    print(f"[{tag}] gradient rel L2 {e:.3e}, max-norm {emax:.3e} (worst column {j}, {j % 128} mod 128)")
+    assert e <= GRAD_TOL, (tag, e)
+    assert emax <= GRAD_MAX_TOL, (tag, emax, j)
+    return e, emax
+
+
+def check_barycenter(Z, Zo, Z0, tag=""):
+    Z = np.asarray(Z, np.float64).reshape(Zo.shape)
+    e = rel_l2(Z, Zo)
+    moved = float(np.linalg.norm(Z - Zo) / max(np.linalg.norm(Zo - np.asarray(Z0, np.float64).reshape(Zo.shape)), 1e-300))
+    print(f"[{tag}] barycenter rel L2 {e:.3e}, relative to distance moved {moved:.3e}")
+    assert e <= BARY_TOL, (tag, e)
+    assert moved <= MOVED_TOL, (tag, moved)
+    return e, moved
 
 
 def run_value_grad(B, oracle, data, tag, mode="checkpointed"):
@@ -54,9 +90,7 @@ def run_value_grad(B, oracle, data, tag, mode="checkpointed"):
     ov, oG = oracle.value_grad(data["Z0"], data["X"], data["offsets"], cfg.gamma, mode=mode)
     check_values(vals.cpu().numpy(), ov, data["lengths"], cfg, tag)
     assert none is None and torch.equal(vals, vals_f)            # forward-only sweep computes the same values
-    e = rel_l2(G.cpu().numpy(), oG)
-    print(f"[{tag}] gradient rel L2 {e:.3e}")
-    assert e <= GRAD_TOL, (tag, e)
+    check_grad(G.cpu().numpy(), oG, tag)
     return vals, G
 
 
@@ -67,9 +101,7 @@ def test_cfg1_tiny_value_grad_and_barycenter(B, oracle):
     run_value_grad(B, oracle, data, "cfg1", mode="full")
     Z, vals, obj = B.sdtw_barycenter(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, cfg.iters, cfg.step)
     Zo, vo, oo = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, cfg.iters, cfg.step)
-    assert rel_l2(Z.cpu().numpy(), Zo) <= BARY_TOL
-    moved = np.linalg.norm(Z.cpu().numpy() - Zo) / np.linalg.norm(Zo - data["Z0"])
-    print(f"[cfg1] barycenter rel L2 {rel_l2(Z.cpu().numpy(), Zo):.3e}, relative to distance moved {moved:.3e}")
+    e, moved = check_barycenter(Z.cpu().numpy(), Zo, data["Z0"], "cfg1")
     assert moved <= 1e-2
     check_values(vals.cpu().numpy(), vo, data["lengths"], cfg, "cfg1 bary values")
     assert np.allclose(obj.cpu().numpy(), oo, rtol=1e-5)
@@ -81,10 +113,7 @@ def test_cfg2_medium_value_grad_and_barycenter(B, oracle):
     run_value_grad(B, oracle, data, "cfg2")
     Z, vals, obj = B.sdtw_barycenter(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, cfg.iters, cfg.step)
     Zo, vo, oo = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, cfg.iters, cfg.step, mode="checkpointed")
-    e = rel_l2(Z.cpu().numpy(), Zo)
-    moved = np.linalg.norm(Z.cpu().numpy() - Zo) / np.linalg.norm(Zo - data["Z0"])
-    print(f"[cfg2] barycenter rel L2 {e:.3e}, relative to distance moved {moved:.3e}; objective {oo[0]:.2f} -> {oo[-1]:.2f}")
-    assert e <= BARY_TOL
+    check_barycenter(Z.cpu().numpy(), Zo, data["Z0"], f"cfg2, objective {oo[0]:.2f} -> {oo[-1]:.2f}")
     assert np.allclose(obj.cpu().numpy(), oo, rtol=1e-4)
     check_values(vals.cpu().numpy(), vo, data["lengths"], cfg, "cfg2 bary values")
 
@@ -99,9 +128,7 @@ def test_scaled_multichannel_and_full_length(B, oracle, idx, scale, N, iters):
         step = 0.08 / N * 0.25
         Z, vals, obj = B.sdtw_barycenter(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, iters, step)
         Zo, vo, oo = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, iters, step, mode="checkpointed")
-        e = rel_l2(Z.cpu().numpy(), Zo)
-        print(f"[{cfg.name}] barycenter rel L2 {e:.3e}; objective {oo}")
-        assert e <= BARY_TOL
+        check_barycenter(Z.cpu().numpy(), Zo, data["Z0"], f"{cfg.name}, objective {oo}")
 
 
 def test_scaled_scoring_sweep_forward_only(B, oracle):
@@ -158,6 +185,7 @@ def test_reverse_zero_skip_is_bitwise_exact(B):
         data = synth.make(cfg)
         Z, X = _dev(data["Z0"]), _dev(data["X"])
         try:
+            B.sdtw_profile_enable(True)                      # the reverse statistics are collected only while profiling
             B.sdtw_set_reverse_mode(True)
             vd, gd = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
             chunks_d, skipped_d = B.sdtw_reverse_stats()
@@ -166,6 +194,8 @@ def test_reverse_zero_skip_is_bitwise_exact(B):
             chunks_s, skipped_s = B.sdtw_reverse_stats()
         finally:
             B.sdtw_set_reverse_mode(False)
+            B.sdtw_profile_read()
+            B.sdtw_profile_enable(False)
         assert torch.equal(vd, vs) and torch.equal(gd, gs), cfg.name
         assert skipped_d == 0 and chunks_d == chunks_s > 0
         print(f"[{cfg.name}] reverse chunks {chunks_s}, skipped {skipped_s} ({100.0 * skipped_s / chunks_s:.1f} %)")
@@ -269,51 +299,101 @@ def test_additivity_and_pair_order(B):
     assert rel_l2(G.cpu().numpy(), acc.cpu().numpy()) < 1e-6
 
 
-# ------------------------------------------------------------------------------------------- full sizes (sampled)
-@pytest.mark.timeout(1500)
-def test_full_size_cfg3_cfg4_cfg5_sampled_against_oracle(B, oracle):
-    """BASELINE.json's full sizes in the launch configuration bench.py times (all pairs in one call).  The oracle
-    computes a sample of pairs one by one: their values must match the full call's values; the gradient of the
-    sampled pairs alone (separable per pair) is checked at full length; properties cover the rest."""
+# ------------------------------------------------------------------------------------------- full sizes
+# The acceptance test of BASELINE.json's north_star at cfg 3-5: the oracle's outputs at full size take hours of CPU time,
+# so they are computed once by tests/golden/make_fullsize_refs.py (which calls only oracle/ and the input generator)
+# and stored under tests/golden/ with the SHA-256 of the inputs and of the oracle source.
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _golden(idx, data):
+    import hashlib
+    import json
+    path = os.path.join(GOLDEN, f"fullsize_cfg{idx}.npz")
+    assert os.path.exists(path), f"{path} is missing: run tests/golden/make_fullsize_refs.py --cfg {idx}"
+    meta = json.load(open(os.path.join(GOLDEN, "fullsize_refs.json")))[f"cfg{idx}"]
+    h = hashlib.sha256()
+    for a in (data["Z0"], data["X"], data["offsets"]):
+        h.update(np.ascontiguousarray(a).tobytes())
+    assert h.hexdigest() == meta["inputs_sha256"], "the stored reference outputs were computed from other inputs"
+    return np.load(path), meta
+
+
+def _full_descent_config(B, idx):
+    """Summed value + gradient at Z0 over ALL pairs, then the configured descent (iterations and step of
+    synth.CONFIGS, which passed the contractivity check C13 in the oracle), in the launch configuration bench.py times."""
     import torch
-    ncpu = os.cpu_count() or 1
-    for idx, nsample in ((3, 2), (4, 2), (5, 3)):
+    data = synth.make(idx)
+    cfg = data["cfg"]
+    gold, meta = _golden(idx, data)
+    assert float(gold["step"]) == cfg.step and int(gold["iters"]) == cfg.iters, "synth.CONFIGS was re-frozen: regenerate"
+    last = meta["contractivity"][-1]
+    assert last["step"] == cfg.step and last["rel_out"] <= 1e-4
+    tag = f"cfg{idx} full size, all {cfg.N} pairs"
+    Z0, X = _dev(data["Z0"]), _dev(data["X"])
+    vals, G = B.sdtw_value_grad(Z0, X, data["offsets"], cfg.gamma)
+    torch.cuda.synchronize()
+    check_values(vals.cpu().numpy(), gold["values0"], data["lengths"], cfg, tag)
+    check_grad(G.cpu().numpy(), gold["grad0"].astype(np.float64), tag)
+    Z, vals_last, obj = B.sdtw_barycenter(Z0.clone(), X, data["offsets"], cfg.gamma, cfg.iters, cfg.step)
+    torch.cuda.synchronize()
+    check_barycenter(Z.cpu().numpy(), gold["Z_final"], data["Z0"], f"{tag}, {cfg.iters} iterations at step {cfg.step:g}")
+    check_values(vals_last.cpu().numpy(), gold["values_last"], data["lengths"], cfg, tag + ", values at the last evaluated iterate")
+    scale = float(np.sum(cfg.gamma * (data["lengths"] + cfg.m)))
+    oo = gold["objective"]
+    print(f"[{tag}] objective {obj.cpu().numpy().tolist()} (oracle {oo.tolist()})")
+    assert np.all(np.abs(obj.cpu().numpy() - oo) <= VAL_TOL * np.maximum(np.abs(oo), scale))
+    return data, vals, G
+
+
+@pytest.mark.timeout(1500)
+def test_cfg3_full_all_pairs_gradient_and_descent(B):
+    _full_descent_config(B, 3)
+
+
+@pytest.mark.timeout(1500)
+def test_cfg4_full_all_pairs_gradient_and_descent(B):
+    _full_descent_config(B, 4)
+
+
+@pytest.mark.timeout(1500)
+def test_cfg5_64_pairs_16_anomalous_full_size(B):
+    """cfg 5 (1000 cycles of 20-40k samples against m = 30000, forward only) in one call; 64 seeded pairs, 16 of them
+    anomalous, against the stored oracle values."""
+    import torch
+    data = synth.make(5)
+    cfg = data["cfg"]
+    gold, _ = _golden(5, data)
+    ks = gold["pairs"]
+    assert len(ks) >= 64 and int(data["anomalous"][ks].sum()) >= 16 and np.array_equal(gold["anomalous"], data["anomalous"][ks])
+    vals, G = B.sdtw_value_grad(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, want_grad=False)
+    torch.cuda.synchronize()
+    assert G is None and torch.isfinite(vals).all()
+    v = vals.cpu().numpy()
+    check_values(v[ks], gold["values"], data["lengths"][ks], cfg, f"cfg5 full size, {len(ks)} pairs")
+    assert np.median(v[data["anomalous"]]) > np.median(v[~data["anomalous"]])
+
+
+@pytest.mark.timeout(1500)
+def test_full_size_batch_equals_single_pair_calls(B):
+    """Schedule validation (the CUDA path against itself, not parity): at full size the batch call -- work queue,
+    units, reduction over pairs -- gives each pair the bits it gets alone, and the summed gradient is the sum of the
+    single-pair gradients (pair independence)."""
+    import torch
+    for idx in (3, 4):
         data = synth.make(idx)
         cfg = data["cfg"]
         Z, X = _dev(data["Z0"]), _dev(data["X"])
-        want_grad = cfg.iters > 0
-        vals, G = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=want_grad)
-        torch.cuda.synchronize()
-        assert torch.isfinite(vals).all()
-        rng = np.random.default_rng(idx)
-        ks = np.sort(rng.choice(cfg.N, size=nsample, replace=False))
-        if idx == 5:                                    # make sure an anomalous cycle is in the sample
-            ks[0] = int(np.flatnonzero(data["anomalous"])[0])
-            ks = np.unique(ks)
-        from paper_2404_12134_b200.dist import take_pairs
-        Xs, offs = take_pairs(data["X"], data["offsets"], ks)
-        ov, oG = oracle.value_grad(data["Z0"], Xs, offs, cfg.gamma, want_grad=want_grad, mode="checkpointed",
-                                   nthreads=min(ncpu, len(ks)))
-        sub = dataclasses.replace(cfg)
-        check_values(vals.cpu().numpy()[ks], ov, data["lengths"][ks], sub, f"cfg{idx} full size, pairs {ks.tolist()}")
-        if want_grad:
-            vs, Gs = B.sdtw_value_grad(Z, _dev(Xs), offs, cfg.gamma)
-            assert torch.equal(vs.cpu(), vals.cpu()[torch.from_numpy(ks)])       # same bits alone or inside the batch
-            e = rel_l2(Gs.cpu().numpy(), oG)
-            print(f"[cfg{idx} full size] gradient of pairs {ks.tolist()} rel L2 {e:.3e}")
-            assert e <= GRAD_TOL
-            assert torch.isfinite(G).all()
-            # the batch call (work queue, strip-major schedule, reduction over pairs) against the sum of single-pair
-            # calls over ALL pairs (pair independence, PAPER.md:196)
-            acc = torch.zeros_like(G, dtype=torch.float64)
-            for k in range(cfg.N):
-                a, b = int(data["offsets"][k]), int(data["offsets"][k + 1])
-                vk, gk = B.sdtw_value_grad(Z, X[a:b], np.array([0, b - a]), cfg.gamma)
-                assert vk.item() == vals[k].item()
-                acc += gk.double()
-            e = rel_l2(G.cpu().numpy(), acc.cpu().numpy())
-            print(f"[cfg{idx} full size] batch gradient vs sum of {cfg.N} single-pair calls: rel L2 {e:.3e}")
-            assert e <= 1e-5
+        vals, G = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+        acc = torch.zeros_like(G, dtype=torch.float64)
+        for k in range(cfg.N):
+            a, b = int(data["offsets"][k]), int(data["offsets"][k + 1])
+            vk, gk = B.sdtw_value_grad(Z, X[a:b], np.array([0, b - a]), cfg.gamma)
+            assert vk.item() == vals[k].item()
+            acc += gk.double()
+        e = rel_l2(G.cpu().numpy(), acc.cpu().numpy())
+        print(f"[cfg{idx} full size] batch gradient vs sum of {cfg.N} single-pair calls: rel L2 {e:.3e}")
+        assert e <= 1e-5 and torch.isfinite(G).all()
         del Z, X, vals, G
         torch.cuda.empty_cache()
 
@@ -328,19 +408,20 @@ def test_band_and_weights_value_grad(B, oracle, idx, scale, N, frac):
     cfg = synth.scaled(synth.CONFIGS[idx], scale, N=N)
     data = synth.make(cfg)
     lens = data["lengths"]
-    band = B.table1_band(cfg.m, lens, frac)
+    band = int(np.floor(frac * max(cfg.m, int(lens.max()))))     # Table 1: a fraction of the longest length
+    assert band == B.table1_band(cfg.m, lens, frac)
     assert band >= np.abs(lens - cfg.m).max() and band < min(cfg.m, lens.min()) - 1      # feasible, and it excludes cells
     rng = np.random.default_rng(idx)
-    w = B.eq7_weights(lens, lam=rng.uniform(0.5, 2.0, size=N))
+    lam = rng.uniform(0.5, 2.0, size=N)
+    w = (lam / lens).astype(np.float32)                           # eq. 7: lambda_k / n_k
+    assert np.array_equal(w, B.eq7_weights(lens, lam=lam))
     Z, X = _dev(data["Z0"]), _dev(data["X"])
     vals, G, obj = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, weights=w, band=band)
     torch.cuda.synchronize()
     ov, oG, oobj = oracle.value_grad(data["Z0"], data["X"], data["offsets"], cfg.gamma, mode="checkpointed",
                                      weights=w.astype(np.float64), band=band, want_objective=True)
     check_values(vals.cpu().numpy(), ov, lens, cfg, f"{cfg.name} band {band}")
-    e = rel_l2(G.cpu().numpy(), oG)
-    print(f"[{cfg.name} band {band} ({frac} x longest), weighted] gradient rel L2 {e:.3e}; objective {obj.item():.6f} vs {oobj:.6f}")
-    assert e <= GRAD_TOL
+    check_grad(G.cpu().numpy(), oG, f"{cfg.name} band {band} ({frac} x longest), weighted; objective {obj.item():.6f} vs {oobj:.6f}")
     assert abs(obj.item() - oobj) <= 1e-4 * max(abs(oobj), float(np.sum(np.abs(w) * cfg.gamma * (lens + cfg.m))))
     # the band changes the result (it is not silently ignored), and a band that excludes nothing changes no bit
     v_free, g_free = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
@@ -357,18 +438,16 @@ def test_band_barycenter_weighted_descent(B, oracle):
     cfg = synth.scaled(synth.CONFIGS[4], 0.1, N=8)
     data = synth.make(cfg)
     lens = data["lengths"]
-    band = B.table1_band(cfg.m, lens, 0.6)
-    w = B.eq7_weights(lens)
+    band = int(np.floor(0.6 * max(cfg.m, int(lens.max()))))      # Table 1 / eq. 7 restated here, not taken from the binding
+    w = (1.0 / lens).astype(np.float32)
+    assert band == B.table1_band(cfg.m, lens, 0.6) and np.array_equal(w, B.eq7_weights(lens))
     step = 0.02 / cfg.N * float(np.mean(lens))                # eq. 7 divides by n_k: rescale the step accordingly
     iters = 3
     Z, vals, obj = B.sdtw_barycenter_ex(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, iters, step,
                                         weights=w, band=band)
     Zo, vo, oo = oracle.barycenter(data["Z0"], data["X"], data["offsets"], cfg.gamma, iters, step, mode="checkpointed",
                                    weights=w.astype(np.float64), band=band)
-    e = rel_l2(Z.cpu().numpy(), Zo)
-    moved = np.linalg.norm(Z.cpu().numpy() - Zo) / np.linalg.norm(Zo - data["Z0"])
-    print(f"[{cfg.name} band {band}, eq. 7 weights] barycenter rel L2 {e:.3e}, relative to distance moved {moved:.3e}; objective {oo}")
-    assert e <= BARY_TOL and moved <= 5e-2
+    check_barycenter(Z.cpu().numpy(), Zo, data["Z0"], f"{cfg.name} band {band}, eq. 7 weights; objective {oo}")
     assert np.allclose(obj.cpu().numpy(), oo, rtol=1e-4, atol=1e-4 * cfg.gamma * 2)
     check_values(vals.cpu().numpy(), vo, lens, cfg, "banded weighted barycenter values")
 
@@ -414,9 +493,8 @@ def test_band_that_matters(B, oracle, n_lo, n_hi, m, d, gamma, band):
     den = np.maximum(np.abs(ov), gamma * (lens + m))
     assert (np.abs(ov - ov_free) / den).max() > 5 * VAL_TOL             # the band matters on this input
     check_values(vals.cpu().numpy(), ov, lens, cfg, cfg.name)
-    e = rel_l2(G.cpu().numpy(), oG)
-    print(f"[{cfg.name}] gradient rel L2 {e:.3e} (unbanded oracle differs by {rel_l2(oG_free, oG):.3e}, band+1 by {rel_l2(oG_off, oG):.3e})")
-    assert e <= GRAD_TOL and rel_l2(oG_free, oG) > 10 * GRAD_TOL
+    check_grad(G.cpu().numpy(), oG, f"{cfg.name} (unbanded oracle differs by {rel_l2(oG_free, oG):.3e}, band+1 by {rel_l2(oG_off, oG):.3e})")
+    assert rel_l2(oG_free, oG) > 10 * GRAD_TOL
     assert rel_l2(oG_off, oG) > 2 * GRAD_TOL                            # ... and so does a one-cell shift of its edge
 
 
@@ -635,10 +713,7 @@ def test_backtracking_descent_matches_oracle(B, oracle, idx, scale, N, iters, st
     assert trials.max() > 1 and np.all(np.diff(obj) < 0)                  # the search did cut the step; monotone descent
     scale_f = np.sum(cfg.gamma * (data["lengths"] + cfg.m))
     assert np.all(np.abs(obj - oo) <= 1e-4 * np.maximum(np.abs(oo), scale_f))
-    e = rel_l2(Z.cpu().numpy(), Zo)
-    moved = np.linalg.norm(Z.cpu().numpy() - Zo) / np.linalg.norm(Zo - data["Z0"])
-    print(f"[{cfg.name}] barycenter rel L2 {e:.3e}, relative to distance moved {moved:.3e}")
-    assert e <= BARY_TOL and moved <= 5e-2
+    check_barycenter(Z.cpu().numpy(), Zo, data["Z0"], cfg.name)
     check_values(vals.cpu().numpy(), vo, data["lengths"], cfg, f"{cfg.name} values at the final Z")
 
 
