@@ -37,9 +37,26 @@ UNIT = "cells/s"
 # roofline constants: MUFU (ex2/lg2/rcp) results per clock per SM on sm_100, SM count, max clock
 MUFU_PER_CLK_PER_SM = 16
 ALGO_MUFU_FWD, ALGO_MUFU_BWD = 3, 3          # algorithmic special-function evaluations per cell (2 ex2 + lg2; 3 ex2)
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the named kernel at the named config, from the
-# ncu --set full capture summarised in profiles/ (null for workloads without a capture)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {("forward_kernel", 4): 2563222000 + 36700025000}   # profiles/r1e_forward_kernel_cfg4_full.txt
+PROFILE_ROUNDS = ("r2", "r1e")                # newest first: profiles/<round>_<kernel>_cfg<idx>[_<variant>]_full.txt
+
+
+def ncu_traffic(kernel, cfg_index, variant=""):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of `kernel` on config `cfg_index`, read from the
+    header of the committed `ncu --set full` summary under profiles/ (the "# raw:" lines); (None, None) when no
+    capture of that kernel / workload is committed."""
+    for rnd in PROFILE_ROUNDS:
+        path = os.path.join(ROOT, "profiles", f"{rnd}_{kernel}_cfg{cfg_index}{'_' + variant if variant else ''}_full.txt")
+        if not os.path.exists(path):
+            continue
+        tot, seen = 0.0, 0
+        for ln in open(path):
+            f = ln.split()
+            if len(f) == 5 and f[:2] == ["#", "raw:"] and f[2] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                tot += float(f[4]) * {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}[f[3]]
+                seen += 1
+        if seen == 2:
+            return int(tot), os.path.relpath(path, ROOT)
+    return None, None
 
 
 def workload_string(cfg):
@@ -99,7 +116,7 @@ def oracle_sample(data, cores):
     """Bounded sample of the workload for the CPU legs: the first 2*cores cycles cut to their first 6000 samples,
     against the first 6000 points of Z0 (same generator, same gamma; ~3.6e7 cells per pair)."""
     cfg = data["cfg"]
-    P = min(cfg.N, 2 * cores)
+    P = min(len(data["lengths"]), 2 * cores)
     L = min(6000, cfg.m)
     chunks = [data["X"][data["offsets"][k]:data["offsets"][k] + min(L, data["lengths"][k])] for k in range(P)]
     off = np.zeros(P + 1, np.int64)
@@ -119,8 +136,21 @@ def time_oracle(data, reps=1):
         oracle.value_grad(Z, X, off, data["cfg"].gamma, mode="checkpointed", nthreads=cores)
         dt = time.perf_counter() - t
         best = dt if best is None else min(best, dt)
-    return {"value": ncells / best, "unit": UNIT, "cores": min(cores, oracle.num_threads()), "kind": "oracle",
-            "sample": what, "seconds": best}
+    out = {"value": ncells / best, "unit": UNIT, "cores": min(cores, oracle.num_threads()), "kind": "oracle",
+           "sample": what, "seconds": best}
+    # the same oracle at FULL length (row-checkpointed mode, the one the full-size references are made with): one
+    # whole cycle per core against the whole Z0, forward recurrence only (value), so that the leg stays near 30 s
+    cfg = data["cfg"]
+    if cfg.m >= 20000:
+        P = min(len(data["lengths"]), cores)
+        off = data["offsets"]
+        t = time.perf_counter()
+        oracle.value_grad(data["Z0"], data["X"][:off[P]], off[:P + 1], cfg.gamma, want_grad=False, mode="checkpointed",
+                          nthreads=cores)
+        dt = time.perf_counter() - t
+        out["full_length"] = {"value": float(off[P]) * cfg.m / dt, "unit": "forward cells/s", "seconds": dt,
+                              "sample": f"first {P} whole cycles vs the whole Z0 (m = {cfg.m}), value only, float64"}
+    return out
 
 
 def run_reference(args):
@@ -150,11 +180,20 @@ def run_reference(args):
 
 
 # ---------------------------------------------------------------------------------------------- our arm
+def table3_config(pairs):
+    """The shape of the paper's Table 3 (Table 1): `pairs` univariate cycles of
+    up to 18385 samples against a barycenter of 18385 points, gamma = 1, Sakoe-Chiba band 0.6, eq. 7 weights."""
+    from dataclasses import replace
+    return replace(synth.CONFIGS[4], name=f"table3_N{pairs}", N=pairs, n_lo=16500, n_hi=18385, m=18385, gamma=1.0,
+                   iters=1, step=0.0)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
+    from dataclasses import replace
     from paper_2404_12134_b200 import binding as B
-    from paper_2404_12134_b200.dist import allreduce_sum_
+    from paper_2404_12134_b200 import dist as D
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -166,40 +205,68 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
-    base = synth.CONFIGS[args.config]
-    data = synth.make(base, seed=synth.BASE_SEED + base.index + 1000 * rank)     # rank 0 == the canonical draw
+    table3 = args.shape == "table3"
+    base = table3_config(args.pairs) if table3 else synth.CONFIGS[args.config]
+    if args.gamma is not None:
+        base = replace(base, gamma=float(args.gamma))
+    strong = args.scaling == "strong" and world > 1
+    # weak scaling: every rank draws its own cycles (rank 0 = the canonical draw); strong scaling: ONE problem (the
+    # canonical draw), its pairs partitioned over the ranks by dist.partition_pairs
+    data = synth.make(base, seed=synth.BASE_SEED + base.index + (0 if strong else 1000 * rank))
     cfg = data["cfg"]
+    if strong:
+        mine = D.partition_pairs(data["lengths"], world)[rank]
+        Xl, offl = D.take_pairs(data["X"], data["offsets"], mine)
+        data = dict(data, X=Xl, offsets=offl, lengths=data["lengths"][mine])
     ncells_local = synth.cells(data)
     Z0 = torch.from_numpy(data["Z0"]).to(dev)
     X = torch.from_numpy(data["X"]).to(dev)
     offsets = data["offsets"]
+    Nl = len(offsets) - 1
     forward_only = cfg.iters == 0
+    iters_cfg = max(cfg.iters, 1)
     ws_bytes = B.sdtw_workspace_bytes(cfg.m, cfg.d, offsets, not forward_only)
+    dense = args.reverse == "dense"
+    B.sdtw_set_reverse_mode(dense)
+    if table3:
+        weights = B.eq7_weights(data["lengths"])
+        band = B.table1_band(cfg.m, data["lengths"])
 
     Z = Z0.clone()
     G = torch.empty_like(Z)
-    vals = torch.empty(cfg.N, dtype=torch.float32, device=dev)
-    obj = torch.zeros(1, dtype=torch.float32, device=dev)
+    vals = torch.empty(Nl, dtype=torch.float32, device=dev)
+    obj_hist = torch.zeros(max(args.steps, args.warmup, 1), dtype=torch.float32, device=dev)
 
-    def step():
-        if forward_only:
-            B.sdtw_value_grad(Z, X, offsets, cfg.gamma, out_values=vals, want_grad=False)
-        elif world == 1:
-            B.sdtw_barycenter(Z, X, offsets, cfg.gamma, 1, cfg.step, out_values=vals, out_objective=obj)
-        else:
-            B.sdtw_value_grad(Z, X, offsets, cfg.gamma, out_values=vals, out_grad=G)
-            allreduce_sum_(G)
-            B.sdtw_gd_update(Z, G, cfg.step)
+    def run_steps(count):
+        """`count` steps.  A step = one pass of the hot path; for the descent configs the steps are the iterations of
+        the CONFIGURED descent (cfg.iters iterations from Z0 at cfg.step), restarted from Z0 when it is complete."""
+        done = 0
+        while done < count:
+            if forward_only:
+                B.sdtw_value_grad(Z, X, offsets, cfg.gamma, out_values=vals, want_grad=False)
+                k = 1
+            elif table3:
+                B.sdtw_value_grad_ex(Z, X, offsets, cfg.gamma, weights=weights, band=band, out_values=vals, out_grad=G)
+                k = 1
+            else:
+                k = min(iters_cfg, count - done)
+                Z.copy_(Z0)
+                if world == 1:
+                    B.sdtw_barycenter(Z, X, offsets, cfg.gamma, k, cfg.step, out_values=vals, out_objective=obj_hist[done:done + k])
+                else:
+                    for _ in range(k):
+                        B.sdtw_value_grad(Z, X, offsets, cfg.gamma, out_values=vals, out_grad=G)
+                        D.allreduce_sum_(G)
+                        B.sdtw_gd_update(Z, G, cfg.step)
+            done += k
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
-        step()
+    run_steps(args.warmup)
     barrier()
-    Z.copy_(Z0)                                    # time the first K iterations of the configured descent
     B.sdtw_profile_enable(True)
     B.sdtw_profile_read()
     sampler = ClockSampler(local)
@@ -208,15 +275,20 @@ def run_ours(args):
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    for _ in range(args.steps):
-        step()
+    run_steps(args.steps)
     e1.record()
     barrier()
     ms_total = e0.elapsed_time(e1)
     launches = B.sdtw_launch_count() - launches0
     prof = B.sdtw_profile_read()
+    rev_chunks, rev_skipped = B.sdtw_reverse_stats() if not forward_only else (0, 0)
     B.sdtw_profile_enable(False)
     clocks = sampler.stop()
+    # what was timed stayed finite (the step passed the contractivity check of tests/golden/make_fullsize_refs.py)
+    finite = bool(torch.isfinite(Z).all().item() and torch.isfinite(vals).all().item())
+    if not finite:
+        raise SystemExit("bench.py: non-finite barycenter or values after the timed steps")
+    objective = obj_hist[:min(args.steps, iters_cfg)].cpu().tolist() if not (forward_only or table3 or world > 1) else None
     t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -233,29 +305,38 @@ def run_ours(args):
     if not args.skip_e2e:
         Xh = torch.from_numpy(data["X"]).pin_memory()
         Zh = torch.from_numpy(data["Z0"].copy()).pin_memory()
+        Gh = torch.zeros_like(Zh).pin_memory()
         objh = torch.zeros(1, dtype=torch.float32).pin_memory()
-        valh = torch.zeros(cfg.N, dtype=torch.float32).pin_memory()
-        e2e_steps = max(1, min(args.steps, 3))
+        valh = torch.zeros(Nl, dtype=torch.float32).pin_memory()
+        e2e_steps = max(1, args.steps)
+        cur = torch.cuda.current_stream().cuda_stream
 
-        def e2e_step():
-            if world == 1 and not forward_only:
-                B.sdtw_barycenter_host(Zh, Xh, offsets, cfg.gamma, 1, cfg.step, valh, objh,
-                                       stream=torch.cuda.current_stream().cuda_stream)
-            elif world == 1:
-                B.sdtw_value_grad_host(Zh, Xh, offsets, cfg.gamma, valh, None, stream=torch.cuda.current_stream().cuda_stream)
+        def e2e_step(i):
+            if world == 1 and not forward_only and not table3:
+                if i % iters_cfg == 0:
+                    Zh.copy_(torch.from_numpy(data["Z0"]))
+                B.sdtw_barycenter_host(Zh, Xh, offsets, cfg.gamma, 1, cfg.step, valh, objh, stream=cur)
+            elif world == 1 and forward_only:
+                B.sdtw_value_grad_host(Zh, Xh, offsets, cfg.gamma, valh, None, stream=cur)
             else:
                 X.copy_(Xh, non_blocking=True)
                 Z.copy_(Zh, non_blocking=True)
-                step()
-                Zh.copy_(Z, non_blocking=True)
+                if table3:
+                    run_steps(1)
+                    Gh.copy_(G, non_blocking=True)
+                else:
+                    B.sdtw_value_grad(Z, X, offsets, cfg.gamma, out_values=vals, out_grad=G)
+                    D.allreduce_sum_(G)
+                    B.sdtw_gd_update(Z, G, cfg.step)
+                    Zh.copy_(Z, non_blocking=True)
                 valh.copy_(vals, non_blocking=True)
                 torch.cuda.synchronize()
 
-        e2e_step()
+        e2e_step(0)
         barrier()
         t0 = time.perf_counter()
-        for _ in range(e2e_steps):
-            e2e_step()
+        for i in range(e2e_steps):
+            e2e_step(i)
         barrier()
         t_e2e = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device=dev)
         if world > 1:
@@ -264,8 +345,9 @@ def run_ours(args):
         h2d = int(Xh.numel() * 4 + Zh.numel() * 4)
         d2h = int(valh.numel() * 4 + (0 if forward_only else Zh.numel() * 4 + 4))
         e2e = {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-               "steps": e2e_steps, "api": "sdtw_barycenter_host" if world == 1 and not forward_only else
-               ("sdtw_value_grad_host" if world == 1 else "pinned copies + sdtw_value_grad + all_reduce + sdtw_gd_update")}
+               "steps": e2e_steps, "api": "sdtw_barycenter_host" if world == 1 and not forward_only and not table3 else
+               ("sdtw_value_grad_host" if world == 1 and forward_only else
+                "pinned copies + sdtw_value_grad(_ex) (+ all_reduce + sdtw_gd_update)")}
 
     # ---- measured special-function issue rate of this device (the roofline denominator)
     mufu = {}
@@ -276,52 +358,82 @@ def run_ours(args):
     if rank == 0:
         sm_max_hz = (clocks.get("sm_max_mhz") or 1965.0) * 1e6
         sms = torch.cuda.get_device_properties(local).multi_processor_count
-        mufu_peak = MUFU_PER_CLK_PER_SM * sms * sm_max_hz
+        mufu_derived = MUFU_PER_CLK_PER_SM * sms * sm_max_hz
+        mufu_peak = min(mufu.values())                 # live: dependent ex2 / lg2 / rcp chains on every SM (mufu_peak.cu)
         n_eval = max(prof["evaluations"], 1)
         t_fwd, t_bwd = prof["ms_forward"] / n_eval * 1e-3, prof["ms_backward"] / n_eval * 1e-3
-        # the dominant kernel is the one with the longest measured duration (the reverse kernel skips chunks whose
-        # incoming E flow is +0, so it usually is the forward kernel)
+        # reverse pass: cells it visited (a visited (strip, chunk) unit = 32 steps x 32 lanes x 2 x 4 cells; the other
+        # units carry E = +0 exactly and are skipped)
+        cells_per_chunk = 32 * 32 * 2 * 4
+        tile = B.sdtw_tile_info()
+        cells_per_chunk = tile["chunk_steps"] * 32 * tile["rows_per_step"] * tile["cols_per_thread"]
+        visited_cells = (rev_chunks - rev_skipped) * cells_per_chunk
+        reverse = None
+        if not forward_only:
+            reverse = {"mode": args.reverse, "units": int(rev_chunks), "skipped_frac": (rev_skipped / rev_chunks) if rev_chunks else None,
+                       "visited_cells": int(visited_cells), "visited_frac_of_cells": visited_cells / ncells_local,
+                       "ms": t_bwd * 1e3,
+                       "frac_on_visited": (ALGO_MUFU_BWD * visited_cells / t_bwd) / mufu_peak if t_bwd > 0 else None,
+                       "note": "algorithmic 3 ex2 per VISITED cell / reverse kernel time / MUFU peak; with the exact +0 skip "
+                               "the pass is a per-pair latency chain, not a throughput kernel"}
+        # the dominant kernel is the one with the longest measured duration
         if forward_only or t_bwd <= t_fwd:
-            dom, t_dom, algo = "forward_kernel", t_fwd, ALGO_MUFU_FWD
+            dom, t_dom, achieved = "forward_kernel", t_fwd, ALGO_MUFU_FWD * ncells_local / t_fwd
         else:
-            dom, t_dom, algo = "backward_kernel", t_bwd, ALGO_MUFU_BWD
-        achieved = algo * ncells_local / t_dom
+            dom, t_dom, achieved = "backward_kernel", t_bwd, ALGO_MUFU_BWD * visited_cells / t_bwd
+        variant = ("dense" if dense else "") if not args.gamma else f"gamma{args.gamma:g}"
+        traffic, traffic_src = (None, None) if (world > 1 or table3) else ncu_traffic(dom, cfg.index, variant)
         algo_total = ALGO_MUFU_FWD + (0 if forward_only else ALGO_MUFU_BWD)
         roofline = {
             "bound": "alu", "kernel": dom, "achieved": achieved / 1e9, "peak": mufu_peak / 1e9, "unit": "GMUFU-op/s",
             "frac": achieved / mufu_peak,
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get((dom, args.config)) if world == 1 else None,
+            "traffic": traffic, "traffic_source": traffic_src,
             "algorithmic_bytes": None if forward_only else int(ncells_local * 0.375 + ncells_local * 4 / 128),
-            "peak_source": f"derived: {MUFU_PER_CLK_PER_SM} MUFU results/clk/SM x {sms} SMs x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm); "
-                           "MEASURED_PEAKS.json holds no ALU figure (DESIGN.md section 8)",
+            "algorithmic_bytes_note": "checkpoint records (0.375 B/cell) + strip-boundary column (4/128 B/cell) written by one "
+                                      "forward launch: this design's checkpoint volume (DESIGN.md 5.5)",
+            "peak_source": "measured live: dependent ex2 / lg2 / rcp chains on every SM (sdtw_measure_mufu_peak), the slowest "
+                           "of the three; MEASURED_PEAKS.json holds no ALU figure (DESIGN.md section 8)",
+            "peak_derived": mufu_derived / 1e9,
+            "peak_derived_source": f"{MUFU_PER_CLK_PER_SM} MUFU results/clk/SM x {sms} SMs x {sm_max_hz / 1e6:.0f} MHz (clocks.max.sm)",
             "mufu_measured_gops": {k: v / 1e9 for k, v in mufu.items()},
             "algorithmic_per_cell": {"forward": ALGO_MUFU_FWD, "reverse": ALGO_MUFU_BWD},
-            "note": "achieved counts the special-function evaluations the method needs (3 per forward cell); the forward "
-                    "kernel issues 2.625 of them on the MUFU pipe and evaluates 3 in 8 of the second exponentials with "
-                    "an FMA-pipe polynomial, so frac can exceed the MUFU-only bound (DESIGN.md 5.2)",
+            "note": "achieved counts the special-function evaluations the method needs (3 per forward cell, 3 per visited "
+                    "reverse cell); the forward kernel issues 2.625 per cell on the MUFU pipe and evaluates 3 in 8 of the "
+                    "second exponentials with an FMA-pipe polynomial, so the MUFU-only fraction can pass 1 (DESIGN.md 5.2)",
             "kernel_ms": {"forward": t_fwd * 1e3, "reverse": t_bwd * 1e3, "other": prof["ms_other"] / n_eval},
             "forward_frac": (ALGO_MUFU_FWD * ncells_local / t_fwd) / mufu_peak if t_fwd > 0 else None,
-            "step_frac_of_cell_rate_roofline": (value / world) / (mufu_peak / algo_total),
-            "checkpoint_hbm_gbs": None if forward_only else
-                (2 * ws_bytes) / max(t_fwd + t_bwd, 1e-9) / 1e9,
+            "reverse": reverse,
+            "cells_per_s_rel_dense_bound": (value / world) / (mufu_peak / algo_total),
+            "cells_per_s_rel_dense_bound_note": "whole-step cells/s relative to the dense bound of 6 special functions per "
+                "cell (3 forward + 3 reverse); NOT a roofline fraction when the reverse pass skips cells: see reverse.visited_frac_of_cells",
+            "checkpoint_hbm_gbs": None if forward_only else (2 * ws_bytes) / max(t_fwd + t_bwd, 1e-9) / 1e9,
         }
         cpu = None if args.skip_cpu else time_oracle(data)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-            "data": "synthetic",
-            "config": {"workload": workload_string(cfg), "cells_per_step": cells_job, "workspace_gb": ws_bytes / 1e9,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_string(cfg) + ("; eq. 7 weights, Sakoe-Chiba band 0.6; step = one value+gradient evaluation" if table3 else ""),
+                       "cells_per_step": cells_job, "workspace_gb": ws_bytes / 1e9,
+                       "descent": None if (forward_only or table3) else
+                           f"steps are the iterations of the configured descent ({iters_cfg} iterations from Z0 at step {cfg.step:g}), "
+                           f"restarted from Z0 every {iters_cfg} steps (one 120 KB device copy inside the timed region)",
+                       "reverse_mode": None if forward_only else args.reverse,
                        "l2": ("no flush: every step streams its checkpoints (workspace) through HBM, far above the 126 MB L2"
                               if ws_bytes > 4 * 126e6 else
                               "no flush: small configuration, the working set fits in the 126 MB L2 (latency-bound; not a roofline case)"),
-                       "parallelism": f"pairs sharded over {world} GPU(s); all-reduce of m*d gradient" if world > 1 else "single GPU",
-                       "tile": B.sdtw_tile_info()},
+                       "parallelism": (f"pairs of ONE problem partitioned over {world} GPUs (LPT on n_k); " if strong else
+                                       f"every GPU its own {cfg.N} pairs; ") + "all-reduce of the m*d gradient per step"
+                                      if world > 1 else "single GPU",
+                       "tile": tile},
             "barycenter_iter_s": ms_step * 1e-3,
+            "objective": objective, "finite": finite,
             "roofline": roofline, "cpu_baseline": cpu,
             "e2e": e2e,
             "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(out))
+    B.sdtw_set_reverse_mode(False)
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -408,6 +520,14 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--op", choices=["barycenter", "score"], default="barycenter",
                     help="score = the Step-3 d_score kernel (extra; the headline is barycenter)")
+    ap.add_argument("--reverse", choices=["skip", "dense"], default="skip",
+                    help="dense = the reverse kernel visits every cell (no exact-zero skip): the throughput measurement")
+    ap.add_argument("--gamma", type=float, default=None, help="override the config's gamma (1.0 = the paper's default, Table 1)")
+    ap.add_argument("--shape", choices=["config", "table3"], default="config",
+                    help="table3 = the paper's Table 3 shape (--pairs cycles of <= 18385 samples, gamma 1, band 0.6, eq. 7 weights)")
+    ap.add_argument("--pairs", type=int, default=5, help="number of cycles for --shape table3 (the paper: 5, 10, 25)")
+    ap.add_argument("--scaling", choices=["weak", "strong"], default="weak",
+                    help="N > 1: weak = every rank its own pairs; strong = one problem partitioned by dist.partition_pairs")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs only: leave out the host-buffer leg")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs only: leave out the timed oracle leg")
     args = ap.parse_args()

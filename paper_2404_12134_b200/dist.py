@@ -39,10 +39,24 @@ def take_pairs(X_concat, offsets, idx):
 
 
 def allreduce_sum_(tensor, group=None):
-    """In-place sum over ranks (NCCL on GPUs, gloo on CPU); a no-op without an initialised process group."""
+    """In-place sum over ranks (NCCL on GPUs, gloo on CPU); a no-op without an initialised process group.
+
+    Bitwise reproducible and identical on every rank, whatever algorithm the collective library picks (SURVEY.md
+    8(e)): the partials are ALL-GATHERED and every rank adds them itself in rank order 0, 1, ..., R-1 (a fixed
+    left-to-right chain in the tensor's dtype), instead of trusting the reduction order of all_reduce.  The exchange
+    is m*d floats per rank (120 KB at m = 30000): latency bound either way."""
+    import torch
     import torch.distributed as dist
     if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
-        dist.all_reduce(tensor, op=dist.ReduceOp.SUM, group=group)
+        world = dist.get_world_size(group)
+        flat = tensor.contiguous().view(-1)
+        gathered = torch.empty(world * flat.numel(), dtype=flat.dtype, device=flat.device)
+        dist.all_gather_into_tensor(gathered, flat, group=group)
+        parts = gathered.view(world, flat.numel())
+        acc = parts[0].clone()
+        for r in range(1, world):
+            acc += parts[r]
+        tensor.copy_(acc.view_as(tensor))
     return tensor
 
 

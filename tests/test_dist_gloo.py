@@ -91,3 +91,31 @@ def test_two_rank_gloo_matches_single_process(tmp_path, oracle):
         Z = Z - cfg.step * g
     assert np.abs(np.load(tmp_path / "Z.npy") - Z).max() <= 1e-12
     assert np.allclose(np.load(tmp_path / "obj.npy"), objs, rtol=1e-12)
+
+
+def _reduce_worker(rank, world, port, out_dir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    rng = np.random.Generator(np.random.PCG64(77 + rank))
+    # magnitudes spread over 12 decades: the float32 sum depends on the order of the additions
+    x = torch.from_numpy((rng.standard_normal((1000, 3)) * 10.0 ** rng.uniform(-6, 6, size=(1000, 3))).astype(np.float32))
+    np.save(os.path.join(out_dir, f"part{rank}.npy"), x.numpy())
+    y = allreduce_sum_(x.clone())
+    np.save(os.path.join(out_dir, f"sum{rank}.npy"), y.numpy())
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.timeout(300)
+def test_allreduce_is_the_rank_ordered_chain_bit_for_bit(tmp_path):
+    """the reduction over ranks is an all-gather plus a fixed chain 0 + 1 + ... + R-1 in the tensor's
+    dtype, so every rank holds the same bits whatever the collective library does."""
+    world = 3
+    mp.spawn(_reduce_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    parts = [np.load(tmp_path / f"part{r}.npy") for r in range(world)]
+    expect = parts[0].copy()
+    for r in range(1, world):
+        expect = (expect + parts[r]).astype(np.float32)
+    for r in range(world):
+        assert np.array_equal(np.load(tmp_path / f"sum{r}.npy"), expect)
