@@ -47,6 +47,14 @@ int sdtw_measure_mufu_peak(int32_t kind, double* ops_per_s, int32_t* sm_count);
  */
 int sdtw_set_reverse_mode(int dense);
 int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped);
+/*
+ * The reverse pass has two kernels with the same arithmetic: 1 = reverse_kernel (a CTA of four warps per
+ * column strip; the recompute runs off the pair's dependency chain: the latency regime), 0 = backward_kernel (one warp
+ * per strip, four times as many strips in flight: the throughput regime, and the dense mode).  -1 (default) chooses by
+ * the number of pairs and the reverse mode.  Results agree to float32 round-off of the per-column sums (the order in
+ * which a column's rows are added differs); each kernel is bitwise reproducible.  Other values => SDTW_ERR_INVALID_ARG.
+ */
+int sdtw_set_reverse_kernel(int which);
 
 /*
  * Forward schedule (tuning, does not change any result bit): the forward kernel hands out UNITS of `unit_strips`

@@ -41,6 +41,7 @@ SYMBOLS = {
     "sdtw_profile_read": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double)] * 3 + [_i64p]),
     "sdtw_tile_info": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int32)] * 5),
     "sdtw_set_reverse_mode": (ctypes.c_int, [ctypes.c_int]),
+    "sdtw_set_reverse_kernel": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_schedule": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_schedule_tail": (ctypes.c_int, [ctypes.c_int, ctypes.c_int]),
     "sdtw_reverse_stats": (ctypes.c_int, [ctypes.POINTER(ctypes.c_uint64)] * 2),
@@ -374,6 +375,11 @@ def sdtw_measure_mufu_peak(kind: int = 0):
 def sdtw_set_reverse_mode(dense: bool):
     """dense=True visits every cell in the reverse pass; False (default) skips chunks whose incoming flow is +0."""
     _check(_lib.sdtw_set_reverse_mode(1 if dense else 0))
+
+
+def sdtw_set_reverse_kernel(which: int = -1):
+    """-1 automatic, 0 one warp per strip (throughput regime), 1 one CTA per strip (latency regime).  Same arithmetic."""
+    _check(_lib.sdtw_set_reverse_kernel(int(which)))
 
 
 def sdtw_set_schedule(unit_strips: int = 0):

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "sdtw_kernels.cuh"
+#include "sdtw_reverse.cuh"
 #include "dtw_kernel.cuh"
 
 namespace {
@@ -26,6 +27,7 @@ UserWs g_user_ws[64];         // caller-registered workspace, one per device (sd
 // settings never change another thread's launch
 thread_local bool g_profile = false;
 thread_local int g_dense_reverse = 0;
+thread_local int g_reverse_kernel = -1;    // -1 = automatic, 0 = backward_kernel, 1 = reverse_kernel (sdtw_set_reverse_kernel)
 thread_local int g_unit_strips = 0;        // 0 = automatic (sdtw_set_schedule)
 thread_local int g_tail_strips = -1, g_tail_unit = 0;   // -1 = automatic (sdtw_set_schedule_tail)
 thread_local const unsigned long long* g_last_stats = nullptr;   // device address of the last evaluation's reverse statistics
@@ -66,7 +68,7 @@ struct Layout {
     int NS = 0;                 // strips per pair
     long long items = 0;
     size_t off_stats = 0;
-    size_t off_counters = 0, off_prog_b = 0, off_VP = 0, off_Xs = 0, off_Zs = 0, off_VS = 0, off_ES = 0, off_CK = 0,
+    size_t off_counters = 0, off_prog_b = 0, off_hint_b = 0, off_VP = 0, off_Xs = 0, off_Zs = 0, off_VS = 0, off_ES = 0, off_CK = 0,
            off_Gk = 0, off_G = 0, off_Zt = 0, off_Vt = 0, off_scal = 0;   // last four: line-search scratch
     size_t sync_bytes = 0;      // counters + stats + prog_b: cleared before every evaluation
     size_t vs_bytes = 0;        // VS: preset to the sentinel pattern before every evaluation
@@ -113,6 +115,7 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
     L.off_counters = o; o += 128;
     L.off_stats = o;    o += 128;
     L.off_prog_b = o;   o += align_up((size_t)L.items * 4, 256);
+    L.off_hint_b = o;   o += align_up((size_t)L.items * 4, 256);
     L.sync_bytes = o;
     L.off_VP = o;       o += align_up((size_t)L.items * 8, 256);
     L.off_Xs = o;       o += align_up((size_t)offsets[N] * (size_t)d * 4, 256);
@@ -276,8 +279,32 @@ int launch_forward(const Params& P, bool ckpt, int sms, cudaStream_t stream) {
     return ckpt ? launch_forward_t<D, true>(P, sms, stream) : launch_forward_t<D, false>(P, sms, stream);
 }
 
+// Two reverse kernels, same arithmetic.  reverse_kernel (sdtw_reverse.cuh: a CTA of 4 warps per strip, the recompute off
+// the dependency chain) wins wherever a pair's chain of strips bounds the pass: few pairs, or most chunks skipped.
+// backward_kernel (one warp per strip, four times as many strips in flight) wins when the pass is bound by throughput:
+// the dense mode, or many more pairs than SMs.  Measured on a B200, reverse pass of one evaluation, new / old kernel:
+// N = 25 / 50 / 100 pairs of 30k: 6.7 / 8.0 / 9.4 ms against 12.1 / 12.7 / 13.5 ms; 200 pairs of 15k: 5.5 against 7.1 ms;
+// 400 pairs of 15k: 9.0 against 8.6 ms (gamma = 1: 15.8 against 11.7 ms); dense, 100 pairs of 30k: 184 against 138 ms.
+constexpr int LATENCY_KERNEL_MAX_PAIRS = 256;
+
+template <int D>
+int launch_reverse(const Params& P, int sms, cudaStream_t stream) {
+    const int smem = rev_smem_bytes<D>();
+    CUDA_TRY(cudaFuncSetAttribute(reverse_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    int occ = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, reverse_kernel<D>, RW * 32, smem));
+    if (occ < 1) return SDTW_ERR_UNSUPPORTED;
+    const int grid = (int)std::max(1LL, std::min((long long)P.num_items, (long long)sms * occ));
+    reverse_kernel<D><<<grid, RW * 32, smem, stream>>>(P);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    return SDTW_OK;
+}
+
 template <int D>
 int launch_backward(const Params& P, int sms, cudaStream_t stream) {
+    const bool latency = (g_reverse_kernel >= 0) ? (g_reverse_kernel == 1) : (!P.dense_reverse && P.N <= LATENCY_KERNEL_MAX_PAIRS);
+    if (latency) return launch_reverse<D>(P, sms, stream);
     const int smem = WARPS * bwd_smem_floats<D>() * 4;
     int grid = 1;
     int rc = persistent_grid(backward_kernel<D>, smem, sms, P.num_items, &grid);
@@ -352,6 +379,7 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     P.Zs = Zs; P.Xs = Xs; P.pm = pl.d_pm;
     P.counters = reinterpret_cast<unsigned*>(ws + L.off_counters);
     P.prog_b = reinterpret_cast<unsigned*>(ws + L.off_prog_b);
+    P.hint_b = reinterpret_cast<unsigned*>(ws + L.off_hint_b);
     P.VP = reinterpret_cast<double*>(ws + L.off_VP);
     P.VS = reinterpret_cast<float*>(ws + L.off_VS);
     P.ES = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_ES) : nullptr;
@@ -838,6 +866,13 @@ int sdtw_set_schedule(int unit_strips) {
 int sdtw_set_reverse_mode(int dense) {
     std::lock_guard<std::mutex> lock(g_mutex);
     g_dense_reverse = dense ? 1 : 0;
+    return SDTW_OK;
+}
+
+int sdtw_set_reverse_kernel(int which) {
+    if (which < -1 || which > 1) return SDTW_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    g_reverse_kernel = which;
     return SDTW_OK;
 }
 

@@ -79,7 +79,8 @@ struct Params {
     const float* Xs;      // sqrt(kappa) * X_concat
     const PairMeta* pm;
     unsigned* counters;   // [0] forward work queue, [1] reverse work queue
-    unsigned* prog_b;     // [N * NS] chunks completed by each reverse item
+    unsigned* prog_b;     // [N * NS] progress word of each reverse item: FIN | z when it is done
+    unsigned* hint_b;     // [N * NS] 1 + the first chunk the reverse item visited (0: none yet)
     float* VS;            // strip-boundary v columns, indexed by row
     float* ES;            // strip-boundary E messages, indexed by row
     float* CK;            // checkpoints
@@ -115,6 +116,9 @@ __device__ __forceinline__ void st_relaxed_f2(float* p, float2 v) {
 }
 __device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {
     unsigned v; asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
+}
+__device__ __forceinline__ void st_relaxed_u32(unsigned* p, unsigned v) {
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ bool is_sentinel(float x) { return __float_as_uint(x) == SENTINEL; }
 

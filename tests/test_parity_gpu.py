@@ -180,11 +180,14 @@ def test_reverse_zero_skip_is_bitwise_exact(B):
     result must be bit-for-bit the one obtained by visiting every cell, and the skip must actually fire on sharp
     (small gamma) problems and never on a problem whose E is nowhere zero."""
     import torch
-    for idx, scale, N, d_expect_skip in ((4, 0.1, 6, True), (3, 0.1, 3, True), (2, 1.0, 8, True), (1, 1.0, 8, False)):
+    import itertools
+    cases = ((4, 0.1, 6, True), (3, 0.1, 3, True), (2, 1.0, 8, True), (1, 1.0, 8, False))
+    for (idx, scale, N, d_expect_skip), kernel in itertools.product(cases, (0, 1)):     # both reverse kernels (sdtw_debug.h)
         cfg = synth.scaled(synth.CONFIGS[idx], scale, N=N)
         data = synth.make(cfg)
         Z, X = _dev(data["Z0"]), _dev(data["X"])
         try:
+            B.sdtw_set_reverse_kernel(kernel)
             B.sdtw_profile_enable(True)                      # the reverse statistics are collected only while profiling
             B.sdtw_set_reverse_mode(True)
             vd, gd = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
@@ -194,9 +197,10 @@ def test_reverse_zero_skip_is_bitwise_exact(B):
             chunks_s, skipped_s = B.sdtw_reverse_stats()
         finally:
             B.sdtw_set_reverse_mode(False)
+            B.sdtw_set_reverse_kernel(-1)
             B.sdtw_profile_read()
             B.sdtw_profile_enable(False)
-        assert torch.equal(vd, vs) and torch.equal(gd, gs), cfg.name
+        assert torch.equal(vd, vs) and torch.equal(gd, gs), (cfg.name, kernel)
         assert skipped_d == 0 and chunks_d == chunks_s > 0
         print(f"[{cfg.name}] reverse chunks {chunks_s}, skipped {skipped_s} ({100.0 * skipped_s / chunks_s:.1f} %)")
         assert (skipped_s > 0) == d_expect_skip, (cfg.name, skipped_s)
@@ -507,20 +511,42 @@ def test_band_dense_reverse_and_schedule_are_bitwise_neutral(B):
     data = synth.make(cfg)
     band = B.table1_band(cfg.m, data["lengths"], 0.3)
     Z, X = _dev(data["Z0"]), _dev(data["X"])
-    v0, g0, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
+    for kernel in (0, 1):
+        try:
+            B.sdtw_set_reverse_kernel(kernel)
+            v0, g0, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
+            B.sdtw_set_reverse_mode(True)
+            v1, g1, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
+            B.sdtw_set_reverse_mode(False)
+            B.sdtw_set_schedule(3)
+            B.sdtw_set_schedule_tail(7, 2)
+            v2, g2, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
+        finally:
+            B.sdtw_set_reverse_mode(False)
+            B.sdtw_set_reverse_kernel(-1)
+            B.sdtw_set_schedule(0)
+            B.sdtw_set_schedule_tail(-1, 0)
+        assert torch.equal(v0, v1) and torch.equal(g0, g1) and torch.equal(v0, v2) and torch.equal(g0, g2), kernel
+        assert torch.isfinite(g0).all()
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_both_reverse_kernels_against_the_oracle(B, oracle, kernel):
+    """The reverse pass has a latency-regime and a throughput-regime kernel (include/sdtw_debug.h,
+    sdtw_set_reverse_kernel); the library picks one by the number of pairs.  Each is held to the parity bar by itself,
+    with and without a band, on ragged shapes that span several strips and chunks."""
+    cases = [synth.make(1), synth.make(2), synth.make(synth.scaled(synth.CONFIGS[3], 0.06, N=5)),
+             synth.make(synth.scaled(synth.CONFIGS[4], 0.05, N=7))]
     try:
-        B.sdtw_set_reverse_mode(True)
-        v1, g1, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
-        B.sdtw_set_reverse_mode(False)
-        B.sdtw_set_schedule(3)
-        B.sdtw_set_schedule_tail(7, 2)
-        v2, g2, _ = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, band=band)
+        B.sdtw_set_reverse_kernel(kernel)
+        for data in cases:
+            cfg = data["cfg"]
+            vals, G = B.sdtw_value_grad(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma)
+            ov, oG = oracle.value_grad(data["Z0"], data["X"], data["offsets"], cfg.gamma)
+            check_values(vals.cpu().numpy(), ov, data["lengths"], cfg, f"{cfg.name}, reverse kernel {kernel}")
+            check_grad(G.cpu().numpy(), oG, f"{cfg.name}, reverse kernel {kernel}")
     finally:
-        B.sdtw_set_reverse_mode(False)
-        B.sdtw_set_schedule(0)
-        B.sdtw_set_schedule_tail(-1, 0)
-    assert torch.equal(v0, v1) and torch.equal(g0, g1) and torch.equal(v0, v2) and torch.equal(g0, g2)
-    assert torch.isfinite(g0).all()
+        B.sdtw_set_reverse_kernel(-1)
 
 
 # ------------------------------------------------------------------------------------------- Step 3 scoring: eq. 8
