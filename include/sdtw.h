@@ -172,8 +172,13 @@ int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_co
  * that share the buffer from different streams are ordered on it with an event, so they are safe but not concurrent.
  * sdtw_set_workspace(NULL, 0) unregisters the caller's buffer and frees the library-owned one of the current device.
  * The pointer must be 256-byte aligned.  sdtw_workspace_bytes returns 0 on invalid arguments.
+ * Forward-only calls (want_grad == 0) without a band keep O(chunks) boundary state per resident strip plus one
+ * boundary column per unit of strips; a forward-only call WITH a band that excludes cells keeps a
+ * full boundary column per strip: size its workspace with sdtw_workspace_bytes_ex(..., band).  The forward-only size
+ * depends on the SM count of the current device (148 is assumed when no device is current).
  */
 size_t sdtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad);
+size_t sdtw_workspace_bytes_ex(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad, int64_t band);
 int sdtw_set_workspace(void* dev_ptr, size_t bytes);
 
 /* Static description of a status code; the cudaError_t behind the last SDTW_ERR_CUDA on this thread. */

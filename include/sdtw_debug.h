@@ -55,6 +55,13 @@ int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped);
  * which a column's rows are added differs); each kernel is bitwise reproducible.  Other values => SDTW_ERR_INVALID_ARG.
  */
 int sdtw_set_reverse_kernel(int which);
+/*
+ * Forward-only calls without a band pass strip-boundary values through per-warp rings inside a unit of strips when
+ * the problem has more strips than resident warps (sdtw_kernels.cuh).  sdtw_set_forward_rings(0) makes them keep one
+ * boundary column per strip instead, as the gradient path does (the workspace then has to be sized with
+ * sdtw_workspace_bytes_ex and a band that excludes a cell); 1 restores the default.  The values are bitwise the same.
+ */
+int sdtw_set_forward_rings(int on);
 
 /*
  * Forward schedule (tuning, does not change any result bit): the forward kernel hands out UNITS of `unit_strips`

@@ -33,6 +33,7 @@ SYMBOLS = {
     "sdtw_value_grad_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_barycenter_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_workspace_bytes": (ctypes.c_size_t, [_i64, _i32, _i64p, _i32, ctypes.c_int]),
+    "sdtw_workspace_bytes_ex": (ctypes.c_size_t, [_i64, _i32, _i64p, _i32, ctypes.c_int, _i64]),
     "sdtw_set_workspace": (ctypes.c_int, [_vp, ctypes.c_size_t]),
     "sdtw_status_string": (ctypes.c_char_p, [ctypes.c_int]),
     "sdtw_last_cuda_error": (ctypes.c_int, []),
@@ -42,6 +43,7 @@ SYMBOLS = {
     "sdtw_tile_info": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int32)] * 5),
     "sdtw_set_reverse_mode": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_reverse_kernel": (ctypes.c_int, [ctypes.c_int]),
+    "sdtw_set_forward_rings": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_schedule": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_schedule_tail": (ctypes.c_int, [ctypes.c_int, ctypes.c_int]),
     "sdtw_reverse_stats": (ctypes.c_int, [ctypes.POINTER(ctypes.c_uint64)] * 2),
@@ -334,6 +336,11 @@ def sdtw_workspace_bytes(m, d, offsets, want_grad=True) -> int:
     return int(_lib.sdtw_workspace_bytes(int(m), int(d), offp, N, 1 if want_grad else 0))
 
 
+def sdtw_workspace_bytes_ex(m, d, offsets, want_grad=True, band=-1) -> int:
+    offp, N = _offsets(offsets)[1:]
+    return int(_lib.sdtw_workspace_bytes_ex(int(m), int(d), offp, N, 1 if want_grad else 0, int(band)))
+
+
 def sdtw_set_workspace(tensor_or_none):
     """Register a device byte buffer (torch uint8 CUDA tensor, kept alive by the caller) or None to unregister."""
     if tensor_or_none is None:
@@ -380,6 +387,11 @@ def sdtw_set_reverse_mode(dense: bool):
 def sdtw_set_reverse_kernel(which: int = -1):
     """-1 automatic, 0 one warp per strip (throughput regime), 1 one CTA per strip (latency regime).  Same arithmetic."""
     _check(_lib.sdtw_set_reverse_kernel(int(which)))
+
+
+def sdtw_set_forward_rings(on: bool = True):
+    """False: forward-only calls keep one boundary column per strip (the layout of the gradient path).  Same values."""
+    _check(_lib.sdtw_set_forward_rings(1 if on else 0))
 
 
 def sdtw_set_schedule(unit_strips: int = 0):

@@ -27,6 +27,7 @@ UserWs g_user_ws[64];         // caller-registered workspace, one per device (sd
 // settings never change another thread's launch
 thread_local bool g_profile = false;
 thread_local int g_dense_reverse = 0;
+thread_local int g_forward_rings = 1;       // 0: forward-only calls keep a boundary column per strip (sdtw_set_forward_rings)
 thread_local int g_reverse_kernel = -1;    // -1 = automatic, 0 = backward_kernel, 1 = reverse_kernel (sdtw_set_reverse_kernel)
 thread_local int g_unit_strips = 0;        // 0 = automatic (sdtw_set_schedule)
 thread_local int g_tail_strips = -1, g_tail_unit = 0;   // -1 = automatic (sdtw_set_schedule_tail)
@@ -68,6 +69,9 @@ struct Layout {
     int NS = 0;                 // strips per pair
     long long items = 0;
     size_t off_stats = 0;
+    int ring_units = 0;         // forward-only ring mode: strips per unit (0: one full boundary column per strip)
+    int ring_ctas = 0;          // CTAs the ring buffers are sized for
+    size_t off_ring = 0, off_ring_prog = 0;
     size_t off_counters = 0, off_prog_b = 0, off_hint_b = 0, off_VP = 0, off_Xs = 0, off_Zs = 0, off_VS = 0, off_ES = 0, off_CK = 0,
            off_Gk = 0, off_G = 0, off_Zt = 0, off_Vt = 0, off_scal = 0;   // last four: line-search scratch
     size_t sync_bytes = 0;      // counters + stats + prog_b: cleared before every evaluation
@@ -76,7 +80,15 @@ struct Layout {
     std::vector<PairMeta> pm;   // schedule order
 };
 
-int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, Layout& L, int vs_words = 1) {
+template <int D> constexpr int fwd_warps() { return D <= 2 ? 32 : 16; }   // warps per CTA of the forward kernel = strips per unit
+inline int fwd_warps_rt(int d) { return d <= 2 ? 32 : 16; }
+
+// ring_sms > 0: forward-only Soft-DTW call without a band on a device with that many SMs.  If the problem has more
+// strips than resident forward warps (the throughput regime), strip-boundary values travel through per-warp rings inside
+// a unit and only the unit boundaries keep a full column (sdtw_kernels.cuh, forward_kernel): O(chunks) live state per
+// resident strip instead of a column per strip ("skipped entirely when out_grad == NULL").
+int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, Layout& L, int vs_words = 1,
+                 int ring_sms = 0) {
     const int max_d = (vs_words == 2) ? SDTW_DTW_MAX_D : SDTW_MAX_D;   // vs_words == 2: the DTW / Sub-DTW kernels
     if (!offsets || m < 1 || d < 1 || N < 1) return SDTW_ERR_INVALID_ARG;
     if (offsets[0] != 0) return SDTW_ERR_INVALID_ARG;
@@ -95,6 +107,12 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
         return (offsets[a + 1] - offsets[a]) > (offsets[b + 1] - offsets[b]);
     });
+    if (ring_sms > 0 && !want_grad && vs_words == 1 && d <= SDTW_MAX_D &&
+        (long long)L.NS * N > (long long)ring_sms * fwd_warps_rt(d)) {
+        L.ring_units = fwd_warps_rt(d);
+        L.ring_ctas = ring_sms;
+    }
+    const int cols_per_pair = L.ring_units ? (L.NS + L.ring_units - 1) / L.ring_units - 1 : L.NS;   // boundary columns kept
     L.pm.resize(N);
     long long vs_floats = 0, ck_floats = 0;
     for (int ps = 0; ps < N; ++ps) {
@@ -106,7 +124,7 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
         pm.C = ((pm.n + RP - 1) / RP + 31 + CH - 1) / CH;
         pm.vs_stride = vs_words * (VS_PAD + pm.C * CROWS);   // 32-bit words per strip (the DTW kernel keeps 2 per row)
         pm.vs_off = vs_floats;
-        vs_floats += (long long)pm.vs_stride * L.NS;
+        vs_floats += (long long)pm.vs_stride * cols_per_pair;
         pm.ck_stride = (long long)(pm.C * (CH / TR) + 1) * CK_FLOATS;
         pm.ck_off = ck_floats;
         if (want_grad) ck_floats += pm.ck_stride * L.NS;
@@ -116,6 +134,10 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
     L.off_stats = o;    o += 128;
     L.off_prog_b = o;   o += align_up((size_t)L.items * 4, 256);
     L.off_hint_b = o;   o += align_up((size_t)L.items * 4, 256);
+    if (L.ring_units) {         // zeroed with the counters: a ring entry is valid when its tag (>= 1) is the expected one
+        L.off_ring = o;      o += (size_t)L.ring_ctas * L.ring_units * RING_ENTRIES * 16;
+        L.off_ring_prog = o; o += align_up((size_t)L.ring_ctas * L.ring_units * 4, 256);
+    }
     L.sync_bytes = o;
     L.off_VP = o;       o += align_up((size_t)L.items * 8, 256);
     L.off_Xs = o;       o += align_up((size_t)offsets[N] * (size_t)d * 4, 256);
@@ -161,6 +183,7 @@ struct Plan {
     int64_t m = 0;
     int32_t d = 0, N = 0;
     bool want_grad = false;
+    bool ring_ok = false;         // forward-only call without a band (the layout may use rings)
     int vs_words = 1;
     std::vector<int64_t> offsets;
     std::vector<float> weights;   // caller order; empty = unweighted
@@ -174,11 +197,12 @@ struct Plan {
 std::vector<Plan*> g_plans;
 uint64_t g_stamp = 0;
 
-int get_plan(int dev, int64_t m, int32_t d, const int64_t* offsets, int32_t N, const float* weights, bool want_grad,
-             cudaStream_t stream, Plan** out, int vs_words = 1) {
+int get_plan(const DeviceInfo& di, int64_t m, int32_t d, const int64_t* offsets, int32_t N, const float* weights, bool want_grad,
+             cudaStream_t stream, Plan** out, int vs_words = 1, bool ring_ok = false) {
+    const int dev = di.dev;
     for (Plan* pl : g_plans) {
         if (pl->dev == dev && pl->m == m && pl->d == d && pl->N == N && pl->want_grad == want_grad &&
-            pl->vs_words == vs_words &&
+            pl->vs_words == vs_words && pl->ring_ok == ring_ok &&
             std::memcmp(pl->offsets.data(), offsets, sizeof(int64_t) * (size_t)(N + 1)) == 0 &&
             (weights ? (!pl->weights.empty() && std::memcmp(pl->weights.data(), weights, sizeof(float) * (size_t)N) == 0)
                      : pl->weights.empty())) {
@@ -189,9 +213,10 @@ int get_plan(int dev, int64_t m, int32_t d, const int64_t* offsets, int32_t N, c
         }
     }
     Plan* pl = new Plan();
-    int rc = build_layout(m, d, offsets, N, want_grad, pl->L, vs_words);
+    int rc = build_layout(m, d, offsets, N, want_grad, pl->L, vs_words, ring_ok ? di.sms : 0);
     if (rc != SDTW_OK) { delete pl; return rc; }
     pl->vs_words = vs_words;
+    pl->ring_ok = ring_ok;
     pl->dev = dev; pl->m = m; pl->d = d; pl->N = N; pl->want_grad = want_grad;
     pl->offsets.assign(offsets, offsets + N + 1);
     cudaError_t e = cudaMalloc(&pl->d_pm, sizeof(PairMeta) * (size_t)N);
@@ -239,10 +264,8 @@ int persistent_grid(K kernel, int smem_bytes, int sms, long long items, int* gri
     return SDTW_OK;
 }
 
-template <int D> constexpr int fwd_warps() { return D <= 2 ? 32 : 16; }   // warps per CTA = strips per unit
-
 template <int D, bool CKPT>
-int launch_forward_t(Params P, int sms, cudaStream_t stream) {
+int launch_forward_t(Params P, int sms, cudaStream_t stream, int ring_ctas) {
     constexpr int FW = fwd_warps<D>();
     const int smem = FW * fwd_smem_floats<D>() * 4;
     auto kernel = forward_kernel<D, CKPT, FW>;
@@ -255,7 +278,11 @@ int launch_forward_t(Params P, int sms, cudaStream_t stream) {
     // spreads each pair's dependency chain over as many SMs as possible.
     const bool all_resident = (long long)P.NS * P.N <= (long long)sms * occ * FW;
     P.unit_strips = (g_unit_strips > 0) ? std::min(g_unit_strips, FW) : (all_resident ? 1 : FW);
-    {
+    if (P.ring) {               // ring layout (forward only): uniform CTA-full units, whatever the tuning hooks say
+        P.unit_strips = FW;
+        P.tail_unit = FW;
+        P.tail_from = P.NS / FW * FW;
+    } else {
         const int US = P.unit_strips;
         // The queue ends with small units: the last one-to-two CTA-fulls of strips of every pair go out 4 at a time, so
         // the sweeps still running when the queue empties are spread over all SMs (cfg 4 forward 68.3 -> 66.6 ms).
@@ -267,7 +294,8 @@ int launch_forward_t(Params P, int sms, cudaStream_t stream) {
     }
     const long long units = ((long long)(P.tail_from / P.unit_strips) +
                              (P.NS - P.tail_from + P.tail_unit - 1) / P.tail_unit) * P.N;
-    const int grid = (int)std::max(1LL, std::min(units, (long long)sms * occ));
+    const long long ctas = P.ring ? std::min((long long)sms * occ, (long long)ring_ctas) : (long long)sms * occ;
+    const int grid = (int)std::max(1LL, std::min(units, ctas));
     kernel<<<grid, FW * 32, smem, stream>>>(P);
     ++g_launches;
     CUDA_TRY(cudaGetLastError());
@@ -275,8 +303,8 @@ int launch_forward_t(Params P, int sms, cudaStream_t stream) {
 }
 
 template <int D>
-int launch_forward(const Params& P, bool ckpt, int sms, cudaStream_t stream) {
-    return ckpt ? launch_forward_t<D, true>(P, sms, stream) : launch_forward_t<D, false>(P, sms, stream);
+int launch_forward(const Params& P, bool ckpt, int sms, cudaStream_t stream, int ring_ctas) {
+    return ckpt ? launch_forward_t<D, true>(P, sms, stream, 0) : launch_forward_t<D, false>(P, sms, stream, ring_ctas);
 }
 
 // Two reverse kernels, same arithmetic.  reverse_kernel (sdtw_reverse.cuh: a CTA of 4 warps per strip, the recompute off
@@ -315,12 +343,12 @@ int launch_backward(const Params& P, int sms, cudaStream_t stream) {
     return SDTW_OK;
 }
 
-int dispatch_forward(int d, const Params& P, bool ckpt, int sms, cudaStream_t s) {
+int dispatch_forward(int d, const Params& P, bool ckpt, int sms, cudaStream_t s, int ring_ctas) {
     switch (d) {
-        case 1: return launch_forward<1>(P, ckpt, sms, s);
-        case 2: return launch_forward<2>(P, ckpt, sms, s);
-        case 3: return launch_forward<3>(P, ckpt, sms, s);
-        case 4: return launch_forward<4>(P, ckpt, sms, s);
+        case 1: return launch_forward<1>(P, ckpt, sms, s, ring_ctas);
+        case 2: return launch_forward<2>(P, ckpt, sms, s, ring_ctas);
+        case 3: return launch_forward<3>(P, ckpt, sms, s, ring_ctas);
+        case 4: return launch_forward<4>(P, ckpt, sms, s, ring_ctas);
     }
     return SDTW_ERR_UNSUPPORTED;
 }
@@ -380,6 +408,8 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     P.counters = reinterpret_cast<unsigned*>(ws + L.off_counters);
     P.prog_b = reinterpret_cast<unsigned*>(ws + L.off_prog_b);
     P.hint_b = reinterpret_cast<unsigned*>(ws + L.off_hint_b);
+    P.ring = L.ring_units ? reinterpret_cast<unsigned long long*>(ws + L.off_ring) : nullptr;
+    P.ring_prog = L.ring_units ? reinterpret_cast<unsigned*>(ws + L.off_ring_prog) : nullptr;
     P.VP = reinterpret_cast<double*>(ws + L.off_VP);
     P.VS = reinterpret_cast<float*>(ws + L.off_VS);
     P.ES = pl.want_grad ? reinterpret_cast<float*>(ws + L.off_ES) : nullptr;
@@ -417,7 +447,7 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
         CUDA_TRY(cudaGetLastError());
     }
     CUDA_TRY((cudaError_t)pr.mark(1, stream));
-    rc = dispatch_forward(pl.d, P, pl.want_grad, di.sms, stream);
+    rc = dispatch_forward(pl.d, P, pl.want_grad, di.sms, stream, L.ring_ctas);
     if (rc) return rc;
     } else CUDA_TRY((cudaError_t)pr.mark(1, stream));
     CUDA_TRY((cudaError_t)pr.mark(2, stream));
@@ -534,7 +564,7 @@ int sdtw_value_grad_ex(const float* Z, int64_t m, int32_t d, const float* X_conc
     rc = get_device(di);
     if (rc) return rc;
     Plan* pl = nullptr;
-    rc = get_plan(di.dev, m, d, offsets, N, weights, out_grad != nullptr, stream, &pl);
+    rc = get_plan(di, m, d, offsets, N, weights, out_grad != nullptr, stream, &pl, 1, out_grad == nullptr && band_eff < 0 && g_forward_rings);
     if (rc) return rc;
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
@@ -563,7 +593,7 @@ int sdtw_barycenter_ex(float* Z_inout, int64_t m, int32_t d, const float* X_conc
     if (rc) return rc;
     if (iters == 0) return SDTW_OK;
     Plan* pl = nullptr;
-    rc = get_plan(di.dev, m, d, offsets, N, weights, true, stream, &pl);
+    rc = get_plan(di, m, d, offsets, N, weights, true, stream, &pl);
     if (rc) return rc;
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
@@ -595,7 +625,7 @@ int sdtw_barycenter_backtracking(float* Z_inout, int64_t m, int32_t d, const flo
     rc = get_device(di);
     if (rc) return rc;
     Plan* pl = nullptr;
-    rc = get_plan(di.dev, m, d, offsets, N, weights, true, stream, &pl);
+    rc = get_plan(di, m, d, offsets, N, weights, true, stream, &pl);
     if (rc) return rc;
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
@@ -675,7 +705,7 @@ static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const floa
     rc = get_device(di);
     if (rc) return rc;
     Plan* pl = nullptr;
-    rc = get_plan(di.dev, m, d, offsets, N, nullptr, false, stream, &pl, 2);
+    rc = get_plan(di, m, d, offsets, N, nullptr, false, stream, &pl, 2);
     if (rc) return rc;
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
@@ -778,10 +808,19 @@ int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_co
 }
 
 // ---- workspace, status, instrumentation -------------------------------------------------------------------------
-size_t sdtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad) {
+size_t sdtw_workspace_bytes_ex(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad, int64_t band) {
     Layout L;
-    if (build_layout(m, d, offsets, N, want_grad != 0, L) != SDTW_OK) return 0;
+    int sms = 148;                                  // the layout of forward-only calls depends on the SM count: B200 unless
+    DeviceInfo di;                                  // a device is current
+    if (get_device(di) == SDTW_OK) sms = di.sms;
+    int band_eff = -1;
+    if (band >= 0 && offsets && N >= 1 && m >= 1 && check_ex(m, offsets, N, nullptr, band, &band_eff) != SDTW_OK) return 0;
+    if (build_layout(m, d, offsets, N, want_grad != 0, L, 1, (!want_grad && band_eff < 0) ? sms : 0) != SDTW_OK) return 0;
     return L.total;
+}
+
+size_t sdtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad) {
+    return sdtw_workspace_bytes_ex(m, d, offsets, N, want_grad, -1);
 }
 
 int sdtw_set_workspace(void* dev_ptr, size_t bytes) {
@@ -866,6 +905,12 @@ int sdtw_set_schedule(int unit_strips) {
 int sdtw_set_reverse_mode(int dense) {
     std::lock_guard<std::mutex> lock(g_mutex);
     g_dense_reverse = dense ? 1 : 0;
+    return SDTW_OK;
+}
+
+int sdtw_set_forward_rings(int on) {
+    std::lock_guard<std::mutex> lock(g_mutex);
+    g_forward_rings = on ? 1 : 0;
     return SDTW_OK;
 }
 

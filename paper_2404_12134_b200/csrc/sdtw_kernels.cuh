@@ -63,6 +63,10 @@ static_assert(W % 4 == 0, "checkpoints store h as float4");
 static_assert(CH % TR == 0 && CH <= 32, "a chunk holds a whole number of checkpoint blocks; one lane per step");
 static_assert(VS_PAD >= SKEW && XPAD >= SKEW && (XWIN * 1) % 32 == 0, "padding covers the lane skew");
 
+constexpr int RING_CHUNKS = 16;                    // chunks a producer may run ahead of its consumer inside a unit
+constexpr int RING_ENTRIES = RING_CHUNKS * CH;     // ring entries (one per pair of rows), a power of two
+static_assert((RING_ENTRIES & (RING_ENTRIES - 1)) == 0, "ring size is a power of two");
+
 struct PairMeta {   // one per pair, in schedule order (longest first)
     long long x_off;      // first row of this cycle in X_concat
     long long vs_off;     // float offset of strip 0's boundary column in VS / ES; strip stride = vs_stride
@@ -94,6 +98,10 @@ struct Params {
     int tail_from;        // strips >= tail_from (a multiple of unit_strips, <= NS) are handed out in units of tail_unit
     int tail_unit;        //   strips (>= 1): the last units in the queue are small, which shortens the drain
     int band;             // Sakoe-Chiba band (Table 1): cell (i, j) admissible iff |i - j| <= band; < 0: none
+    // forward-only sweeps (no checkpoints): strip-boundary values travel through small rings inside a unit (null: every
+    // boundary has a full column, as in the gradient path); see forward_kernel
+    unsigned long long* ring;   // [CTA][warp position][RING_ENTRIES][2]: (value bits | tag << 32) per row
+    unsigned* ring_prog;        // [CTA][warp position] entries of the left neighbour's ring this warp has consumed
     const float* wts;     // [N] per-pair weights of eq. 7 in schedule order, or null (all 1)
     float gscale;         // 2 / sqrt(kappa)
 };
@@ -119,6 +127,12 @@ __device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {
 }
 __device__ __forceinline__ void st_relaxed_u32(unsigned* p, unsigned v) {
     asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void ld_relaxed_v2u64(const unsigned long long* p, unsigned long long& a, unsigned long long& b) {
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void st_relaxed_v2u64(unsigned long long* p, unsigned long long a, unsigned long long b) {
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(p), "l"(a), "l"(b) : "memory");
 }
 __device__ __forceinline__ bool is_sentinel(float x) { return __float_as_uint(x) == SENTINEL; }
 
@@ -324,6 +338,7 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
     __syncthreads();
 
     int base = 0;                                          // strips of the units before unit k, mod FW
+    unsigned in_q = 0, out_q = 0;                          // ring entries consumed from the left / produced, all strips so far
     for (int k = 0;; ++k) {
         int u = 0;
         if (lane == 0) {                                   // the CTA's k-th unit: popped by whichever warp needs it first
@@ -366,9 +381,25 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
         const int item = ps * p.NS + J;
         const int T = J * 32 + lane;                       // global thread (column group) index
         const int j0 = T * W;
-        float* VSme = p.VS + pm.vs_off + (long long)J * pm.vs_stride + VS_PAD;      // indexed by row
-        const float* VSprev = VSme - pm.vs_stride;
+        // Strip-boundary values.  Gradient path (and forward-only calls without rings): one full column per strip, VS.
+        // Forward-only with rings (p.ring != null; CKPT == false, no band, uniform units): inside a unit the boundary
+        // values of strip sidx go to the warp one position further through a ring of RING_CHUNKS chunks in global
+        // memory (entry = value bits | tag << 32, tag = lap + 1; the buffer is zeroed per evaluation); the producer waits
+        // when it is a whole ring ahead of what the consumer has taken (ring_prog).  Only the LAST strip of a unit keeps
+        // a full column (its consumer is handed out much later): column g of the pair after unit g.  A warp's ring and
+        // its counters run on across the units it serves: producer (position q) and consumer (q + 1) see the same
+        // sequence of strips, so their cumulative entry counts agree.
+        const bool rings = !CKPT && p.ring != nullptr;
+        const bool in_ring = rings && sidx > 0, out_ring = rings && sidx + 1 < S;
+        const bool out_none = rings && !out_ring && J == p.NS - 1;            // nobody reads the last strip's boundary
+        const long long col = rings ? (out_ring ? 0 : g) : J;                 // my output column (when I have one)
+        float* VSme = p.VS + pm.vs_off + col * pm.vs_stride + VS_PAD;         // indexed by row
+        const float* VSprev = rings ? p.VS + pm.vs_off + (long long)(g - 1) * pm.vs_stride + VS_PAD : VSme - pm.vs_stride;
         float* CKme = p.CK + pm.ck_off + (long long)J * pm.ck_stride;
+        // ring of the warp at position q of this CTA, and the count of entries that warp has taken from its left neighbour
+        // (addresses are rebuilt where they are used: the kernel has no registers to spare)
+        auto ring_of = [&](const int q) { return p.ring + ((size_t)blockIdx.x * FW + q) * (RING_ENTRIES * 2); };
+        auto prog_of = [&](const int q) { return p.ring_prog + (size_t)blockIdx.x * FW + q; };
 
         float z[W][D], h[W];
 #pragma unroll
@@ -473,20 +504,32 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
         stage_x_async<D>(xs0 + (cf & 1) * XWIN * D, p.Xs, pm.x_off, n, cf, lane);
         const int vlane = (lane < CH) ? lane : 0;          // lanes >= CH duplicate lane 0's poll (CH < 32 only)
         float2 vreg = make_float2(0.f, 0.f);
-        if (J > 0) vreg = ld_relaxed_f2(VSprev + cf * CROWS + 2 * vlane);
-        auto unpublished = [&](const float2 v, const int r) {   // rows >= n are never used
-            return (r < n && is_sentinel(v.x)) || (r + 1 < n && is_sentinel(v.y));
+        bool vbad = false;                                 // vreg is not the published value yet
+        // boundary values of rows r, r + 1 (r = c CROWS + 2 vlane) from the left strip: column or ring; rows >= n are never used
+        auto load_in = [&](const int c) {
+            const int r = c * CROWS + 2 * vlane;
+            if (in_ring) {
+                const unsigned e = in_q + (unsigned)(c * CH + vlane);
+                unsigned long long a, b2;
+                ld_relaxed_v2u64(ring_of((mypos + FW - 1) % FW) + (size_t)(e & (RING_ENTRIES - 1)) * 2, a, b2);
+                const unsigned tag = e / RING_ENTRIES + 1u;
+                vreg = make_float2(__uint_as_float((unsigned)a), __uint_as_float((unsigned)b2));
+                vbad = (r < n && (unsigned)(a >> 32) != tag) || (r + 1 < n && (unsigned)(b2 >> 32) != tag);
+            } else {
+                vreg = ld_relaxed_f2(VSprev + r);
+                vbad = (r < n && is_sentinel(vreg.x)) || (r + 1 < n && is_sentinel(vreg.y));
+            }
         };
+        if (J > 0) load_in(cf);
+        unsigned cons_seen = 0;                            // my consumer's progress as last read (rings)
 
         for (int c = cf; c <= cl; ++c) {
             const int rbase = c * CROWS + 2 * vlane;       // lane 0 works on rows rbase, rbase + 1 at step `vlane`
             if (J > 0) {                                   // valid = the left strip has published these rows
-                bool bad = unpublished(vreg, rbase);
-                if (__any_sync(FULL, bad)) {
+                if (__any_sync(FULL, vbad)) {
                     for (;;) {
-                        if (bad) vreg = ld_relaxed_f2(VSprev + rbase);
-                        bad = unpublished(vreg, rbase);
-                        if (!__any_sync(FULL, bad)) break;
+                        if (vbad) load_in(c);
+                        if (!__any_sync(FULL, vbad)) break;
                         __nanosleep(100);
                     }
                 }
@@ -496,9 +539,11 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
             cp_async_wait_all();
             if (lane < CH) vin_s[lane] = vreg;
             __syncwarp();
+            if (in_ring && lane == 0) st_relaxed_u32(prog_of(mypos), in_q + (unsigned)((c + 1) * CH));   // chunk c taken
+            if (out_ring && lane == 0) cons_seen = ld_relaxed_u32(prog_of((mypos + 1) % FW));           // looked at below
             if (c + 1 <= cl) {                             // prefetch of chunk c + 1 (the other x buffer)
                 stage_x_async<D>(xs0 + ((c + 1) & 1) * XWIN * D, p.Xs, pm.x_off, n, c + 1, lane);
-                if (J > 0) vreg = ld_relaxed_f2(VSprev + rbase + CROWS);
+                if (J > 0) load_in(c + 1);
             }
             xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;    // rows of step t: xs_lane[2t], [2t+1]
             const bool inside = interior_chunk(c, n) && band_clear(c, J, band);
@@ -525,8 +570,31 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
             }
             __syncwarp();
             // lane 31 worked on rows c CROWS - SKEW + 2t (+1) at step t
-            if (lane < CH) st_relaxed_f2(VSme + c * CROWS - SKEW + 2 * lane, vout_s[lane]);
+            if (out_ring) {
+                // entry of rows (r, r + 1): out_base + r / 2.  The highest entry of this chunk reuses the slot of the entry
+                // RING_ENTRIES below it (an entry of this strip or of the strip before): my consumer must have taken it
+                {
+                    const unsigned need = out_q + (unsigned)((c - RING_CHUNKS + 1) * CH);   // cumulative; wraps like the counters
+                    unsigned seen = __shfl_sync(FULL, cons_seen, 0);
+                    while ((int)(seen - need) < 0) {
+                        __nanosleep(64);
+                        if (lane == 0) cons_seen = ld_relaxed_u32(prog_of((mypos + 1) % FW));
+                        seen = __shfl_sync(FULL, cons_seen, 0);
+                    }
+                }
+                const int q = c * CH - (SKEW / 2) + lane;               // r / 2 for r = c CROWS - SKEW + 2 lane
+                if (lane < CH && q >= 0) {
+                    const unsigned e = out_q + (unsigned)q;
+                    const unsigned long long tag = (unsigned long long)(e / RING_ENTRIES + 1u) << 32;
+                    const float2 vo = vout_s[lane];
+                    st_relaxed_v2u64(ring_of(mypos) + (size_t)(e & (RING_ENTRIES - 1)) * 2, tag | __float_as_uint(vo.x), tag | __float_as_uint(vo.y));
+                }
+            } else if (!out_none) {
+                if (lane < CH) st_relaxed_f2(VSme + c * CROWS - SKEW + 2 * lane, vout_s[lane]);
+            }
         }
+        if (in_ring) in_q += (unsigned)(C * CH);
+        if (out_ring) out_q += (unsigned)(C * CH);
         if (cl < C - 1) {
             // the right strip's last chunks (its band ends SW rows lower) still poll rows this strip never reaches: they
             // feed only cells outside the band or overridden inputs, so publish zeros for them

@@ -379,6 +379,32 @@ def test_cfg5_64_pairs_16_anomalous_full_size(B):
     assert np.median(v[data["anomalous"]]) > np.median(v[~data["anomalous"]])
 
 
+@pytest.mark.parametrize("d,N,m", [(1, 64, 10100), (2, 60, 10300), (4, 40, 8100)])
+def test_forward_only_rings_match_the_oracle_and_single_pair_calls(B, oracle, d, N, m):
+    """Forward-only calls with more strips than resident warps pass strip-boundary values through per-warp rings inside
+    a unit of strips and keep a boundary column only per unit (sdtw_kernels.cuh).  Short, ragged
+    cycles against a long Z: many strips, a few chunks each, several units per pair and a ragged last unit.  Values
+    against the oracle; and bit for bit against single-pair calls, which are small enough to take the one-column-per-strip
+    path, and against a second run (ring state is rebuilt per evaluation)."""
+    import torch
+    from dataclasses import replace
+    cfg = replace(synth.CONFIGS[5], name=f"rings_d{d}", N=N, n_lo=700, n_hi=1900, m=m, d=d, gamma=0.05)
+    data = synth.make(cfg)
+    # rings in use: the workspace is smaller than the one-column-per-strip layout a banded call of this shape needs
+    assert B.sdtw_workspace_bytes(m, d, data["offsets"], False) < B.sdtw_workspace_bytes_ex(m, d, data["offsets"], False, m - 100)
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    vals, G = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
+    vals2, _ = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
+    torch.cuda.synchronize()
+    assert G is None and torch.equal(vals, vals2)
+    ov, _ = oracle.value_grad(data["Z0"], data["X"], data["offsets"], cfg.gamma, want_grad=False, mode="checkpointed")
+    check_values(vals.cpu().numpy(), ov, data["lengths"], cfg, f"forward-only rings d={d}")
+    for k in (0, 1, N // 2, N - 1):
+        a, b = int(data["offsets"][k]), int(data["offsets"][k + 1])
+        vk, _ = B.sdtw_value_grad(Z, X[a:b], np.array([0, b - a]), cfg.gamma, want_grad=False)
+        assert vk.item() == vals[k].item(), (k, vk.item(), vals[k].item())
+
+
 @pytest.mark.timeout(1500)
 def test_full_size_batch_equals_single_pair_calls(B):
     """Schedule validation (the CUDA path against itself, not parity): at full size the batch call -- work queue,
