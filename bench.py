@@ -498,6 +498,7 @@ def run_score(args):
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_string(cfg) + "; op = sdtw_dtw_score (eq. 8)", "cells_per_step": cells,
+                   "workspace_gb": B.sdtw_dtw_workspace_bytes(cfg.m, cfg.d, data["offsets"]) / 1e9,
                    "l2": "no flush: inputs + strip-boundary columns exceed the 126 MB L2" if cells > 1e10 else "no flush (small)"},
         "roofline": {"bound": "alu", "kernel": "dtw_kernel", "achieved": algo * cells / (ms * 1e-3) / 1e9, "peak": peak / 1e9,
                      "unit": "Gthread-instr/s", "frac": algo * cells / (ms * 1e-3) / peak, "traffic": None,

@@ -179,6 +179,8 @@ int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_co
  */
 size_t sdtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad);
 size_t sdtw_workspace_bytes_ex(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad, int64_t band);
+/* What one sdtw_dtw_score / sdtw_subdtw call of this shape needs (d <= SDTW_DTW_MAX_D); 0 on invalid arguments. */
+size_t sdtw_dtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_t N);
 int sdtw_set_workspace(void* dev_ptr, size_t bytes);
 
 /* Static description of a status code; the cudaError_t behind the last SDTW_ERR_CUDA on this thread. */

@@ -34,6 +34,7 @@ SYMBOLS = {
     "sdtw_barycenter_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_workspace_bytes": (ctypes.c_size_t, [_i64, _i32, _i64p, _i32, ctypes.c_int]),
     "sdtw_workspace_bytes_ex": (ctypes.c_size_t, [_i64, _i32, _i64p, _i32, ctypes.c_int, _i64]),
+    "sdtw_dtw_workspace_bytes": (ctypes.c_size_t, [_i64, _i32, _i64p, _i32]),
     "sdtw_set_workspace": (ctypes.c_int, [_vp, ctypes.c_size_t]),
     "sdtw_status_string": (ctypes.c_char_p, [ctypes.c_int]),
     "sdtw_last_cuda_error": (ctypes.c_int, []),
@@ -44,6 +45,7 @@ SYMBOLS = {
     "sdtw_set_reverse_mode": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_reverse_kernel": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_forward_rings": (ctypes.c_int, [ctypes.c_int]),
+    "sdtw_set_forward_kernel": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_schedule": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_schedule_tail": (ctypes.c_int, [ctypes.c_int, ctypes.c_int]),
     "sdtw_reverse_stats": (ctypes.c_int, [ctypes.POINTER(ctypes.c_uint64)] * 2),
@@ -341,6 +343,11 @@ def sdtw_workspace_bytes_ex(m, d, offsets, want_grad=True, band=-1) -> int:
     return int(_lib.sdtw_workspace_bytes_ex(int(m), int(d), offp, N, 1 if want_grad else 0, int(band)))
 
 
+def sdtw_dtw_workspace_bytes(m, d, offsets) -> int:
+    offp, N = _offsets(offsets)[1:]
+    return int(_lib.sdtw_dtw_workspace_bytes(int(m), int(d), offp, N))
+
+
 def sdtw_set_workspace(tensor_or_none):
     """Register a device byte buffer (torch uint8 CUDA tensor, kept alive by the caller) or None to unregister."""
     if tensor_or_none is None:
@@ -387,6 +394,11 @@ def sdtw_set_reverse_mode(dense: bool):
 def sdtw_set_reverse_kernel(which: int = -1):
     """-1 automatic, 0 one warp per strip (throughput regime), 1 one CTA per strip (latency regime).  Same arithmetic."""
     _check(_lib.sdtw_set_reverse_kernel(int(which)))
+
+
+def sdtw_set_forward_kernel(which: int = -1):
+    """-1 automatic, 0 throughput instantiation, 1 latency instantiation of the forward kernel.  Bitwise the same results."""
+    _check(_lib.sdtw_set_forward_kernel(int(which)))
 
 
 def sdtw_set_forward_rings(on: bool = True):

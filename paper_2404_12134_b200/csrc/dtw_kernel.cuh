@@ -12,14 +12,18 @@
 // Same wavefront as the Soft-DTW forward kernel (sdtw_kernels.cuh): a work item is one strip of 32 x W columns of one
 // pair swept by one warp, lane l on rows 2(s-l), 2(s-l)+1 at step s; (r, len) of a lane's last column goes to the next
 // lane by shuffle and to the next strip through a sentinel-preset global column polled one chunk ahead.  No special
-// functions: the bound is the FP32/ALU issue rate.  Items are handed out strip-major from one atomic counter (every
-// item's producer was handed out earlier, so a waiting warp never blocks the warp it waits for).
+// functions: the bound is the FP32/ALU issue rate.  Schedule: the forward kernel's (units of adjacent strips popped
+// group-major by a CTA whose warps serve a rolling stream of strips).  When the problem has more strips than resident
+// warps a unit is a CTA-full and the boundary values travel inside a unit through per-warp rings (as in the forward-only
+// Soft-DTW sweep; an entry carries (r, len) of two rows as four tagged 64-bit words); only the last strip of a unit
+// keeps a full column.  Otherwise every strip is its own unit and keeps a column.
 #pragma once
 #include "sdtw_kernels.cuh"
 
 namespace sdtw {
 
-constexpr int DTW_WARPS = 8;
+// warps per CTA = strips per unit: a CTA-full at d <= 2 (the kernel fits 64 registers), 8 warps at more channels
+template <int D> __host__ __device__ constexpr int dtw_warps() { return D <= 2 ? 32 : 8; }
 #ifndef SDTW_DTW_W
 #define SDTW_DTW_W 4
 #endif
@@ -32,8 +36,11 @@ struct DtwParams {
     const float* Z;       // [m][D] natural units
     const float* X;       // [sum n][D]
     const PairMeta* pm;   // schedule order; vs_off / vs_stride in 32-bit words, 2 words (r, len) per row
-    unsigned* counter;    // work queue
+    unsigned* counter;    // work queue (units)
     unsigned* VS;         // strip-boundary columns: word 2 row = r bits, word 2 row + 1 = len
+    unsigned long long* ring;   // [CTA][warp position][RING_ENTRIES][4]: (r, len) of a row pair, each word | tag << 32; or null
+    unsigned* ring_prog;        // [CTA][warp position] entries of the left neighbour's ring this warp has consumed
+    int unit_strips;      // strips per unit: the CTA's warps (rings inside a unit, a column after it), or 1 (a column per strip)
     float* out_dtw;       // [N] caller order (may be null): DTW, or the Sub-DTW value
     int* out_len;         // [N] (may be null): |pi|, or a* (Sub-DTW)
     float* out_score;     // [N] (may be null): DTW / |pi| (not written by the Sub-DTW variant)
@@ -80,27 +87,45 @@ __device__ __forceinline__ void dtw_cell(const XRow<D>& x, const float (&z)[D], 
 // SUB = false: eq. 1 / eq. 8 (complete paths).  SUB = true: eq. 2, the rows (the series of
 // X_concat) have free ends: r_i0 = 0 for every i, value = min_i r_im, b* = the smallest such i, a* = the path's first row.
 template <int D, bool SUB>
-__global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) {
+__global__ void __launch_bounds__(dtw_warps<D>() * 32) dtw_kernel(const DtwParams p) {
     constexpr int W = dtw_w<D>();                                    // shadows sdtw::W inside this kernel
+    constexpr int FW = dtw_warps<D>();
     extern __shared__ __align__(16) float smem[];
+    __shared__ RollCtl ctl;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float* xs0 = smem + warp * dtw_smem_floats<D>();                 // [2][XWIN][D]
     uint4* vin_s = reinterpret_cast<uint4*>(xs0 + 2 * XWIN * D);     // [CH] (r, len) of the left strip for lane 0's two rows
     uint4* vout_s = vin_s + 32;                                      // [CH] (r, len) of lane 31's last column
     const int m = p.m;
     const float INF = __uint_as_float(F_INF);
+    const int US = p.unit_strips;
+    const int NG = (p.NS + US - 1) / US, NU = NG * p.N;              // units per pair, units
+    const int mypos = (warp & 3) * (FW / 4) + (warp >> 2);           // consecutive positions share a scheduler
+    if (threadIdx.x < 32) { ctl.seen[threadIdx.x] = 0; if (threadIdx.x == 0) { ctl.popped = 0; ctl.lock = 0; } }
+    __syncthreads();
 
-    for (;;) {
-        unsigned q = 0;
-        if (lane == 0) q = atomicAdd(p.counter, 1u);
-        q = __shfl_sync(FULL, q, 0);
-        if (q >= p.num_items) break;
-        const int J = q / p.N, ps = q - J * p.N;             // strip-major: every pair's strip J before any strip J + 1
+    int base = 0;
+    unsigned in_q = 0, out_q = 0;                          // ring entries consumed from the left / produced, all strips so far
+    for (int k = 0;; ++k) {
+        const int u = pop_unit<FW>(ctl, p.counter, k, NU, warp, lane);
+        if (u >= NU) break;
+        const int g = u / p.N, ps = u - g * p.N;             // group-major: every pair's unit g before any unit g + 1
+        const int S = min(US, p.NS - g * US);
+        const int sidx = (mypos - base + FW) % FW;
+        base = (base + S) % FW;
+        if (sidx >= S) continue;
+        const int J = g * US + sidx;
         const PairMeta pm = p.pm[ps];
         const int n = pm.n, C = pm.C;
         const int j0 = (J * 32 + lane) * W;
-        unsigned* VSme = p.VS + pm.vs_off + (long long)J * pm.vs_stride + 2 * VS_PAD;   // word 2 row
-        const unsigned* VSprev = VSme - pm.vs_stride;
+        const bool rings = p.ring != nullptr;
+        const bool in_ring = rings && sidx > 0, out_ring = rings && sidx + 1 < S;
+        const bool out_none = rings && !out_ring && J == p.NS - 1;
+        const long long col = rings ? (out_ring ? 0 : g) : J;
+        unsigned* VSme = p.VS + pm.vs_off + col * pm.vs_stride + 2 * VS_PAD;   // word 2 row
+        const unsigned* VSprev = rings ? p.VS + pm.vs_off + (long long)(g - 1) * pm.vs_stride + 2 * VS_PAD : VSme - pm.vs_stride;
+        auto ring_of = [&](const int q) { return p.ring + ((size_t)blockIdx.x * FW + q) * (RING_ENTRIES * 4); };
+        auto prog_of = [&](const int q) { return p.ring_prog + (size_t)blockIdx.x * FW + q; };
 
         float z[W][D], ru[W], lu[W];
 #pragma unroll
@@ -158,27 +183,44 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
             return SUB ? make_uint4(0u, __float_as_uint((float)(r + 1)), 0u, __float_as_uint((float)(r + 2))) : make_uint4(F_INF, 0u, F_INF, 0u);
         };
         uint4 vreg = border(2 * vlane);
-        if (J > 0) vreg = ld_relaxed_u4(VSprev + 2 * (2 * vlane));
-        auto unpublished = [&](const uint4 v, const int r) {   // rows >= n are never used
-            return (r < n && (v.x == SENTINEL || v.y == SENTINEL)) || (r + 1 < n && (v.z == SENTINEL || v.w == SENTINEL));
+        bool vbad = false;
+        // (r, len) of rows rb, rb + 1 (rb = c CROWS + 2 vlane) from the left strip: column or ring; rows >= n are never used
+        auto load_in = [&](const int c) {
+            const int rb = c * CROWS + 2 * vlane;
+            if (in_ring) {
+                const unsigned e = in_q + (unsigned)(c * CH + vlane);
+                const unsigned long long* q = ring_of((mypos + FW - 1) % FW) + (size_t)(e & (RING_ENTRIES - 1)) * 4;
+                unsigned long long a0, a1, a2, a3;
+                ld_relaxed_v2u64(q, a0, a1);
+                ld_relaxed_v2u64(q + 2, a2, a3);
+                const unsigned tag = e / RING_ENTRIES + 1u;
+                vreg = make_uint4((unsigned)a0, (unsigned)a1, (unsigned)a2, (unsigned)a3);
+                vbad = (rb < n && ((unsigned)(a0 >> 32) != tag || (unsigned)(a1 >> 32) != tag)) ||
+                       (rb + 1 < n && ((unsigned)(a2 >> 32) != tag || (unsigned)(a3 >> 32) != tag));
+            } else {
+                vreg = ld_relaxed_u4(VSprev + 2 * rb);
+                vbad = (rb < n && (vreg.x == SENTINEL || vreg.y == SENTINEL)) || (rb + 1 < n && (vreg.z == SENTINEL || vreg.w == SENTINEL));
+            }
         };
+        if (J > 0) load_in(0);
+        unsigned cons_seen = 0;
 
         for (int c = 0; c < C; ++c) {
             const int rbase = c * CROWS + 2 * vlane;
             if (J > 0) {
-                bool bad = unpublished(vreg, rbase);
-                while (__any_sync(FULL, bad)) {
+                while (__any_sync(FULL, vbad)) {
                     __nanosleep(100);
-                    if (bad) vreg = ld_relaxed_u4(VSprev + 2 * rbase);
-                    bad = unpublished(vreg, rbase);
+                    if (vbad) load_in(c);
                 }
             }
             cp_async_wait_all();
             if (lane < CH) vin_s[lane] = vreg;
             __syncwarp();
+            if (in_ring && lane == 0) st_relaxed_u32(prog_of(mypos), in_q + (unsigned)((c + 1) * CH));   // chunk c taken
+            if (out_ring && lane == 0) cons_seen = ld_relaxed_u32(prog_of((mypos + 1) % FW));           // looked at below
             if (c + 1 < C) {
                 stage_x_async<D>(xs0 + ((c + 1) & 1) * XWIN * D, p.X, pm.x_off, n, c + 1, lane);
-                vreg = (J > 0) ? ld_relaxed_u4(VSprev + 2 * (rbase + CROWS)) : border(rbase + CROWS);
+                if (J > 0) load_in(c + 1); else vreg = border(rbase + CROWS);
             }
             xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;
             if (interior_chunk(c, n)) {
@@ -189,8 +231,32 @@ __global__ void __launch_bounds__(DTW_WARPS * 32) dtw_kernel(const DtwParams p) 
                 for (int t = 0; t < CH; ++t) step(c, t, SlowTag{});
             }
             __syncwarp();
-            if (lane < CH) st_relaxed_u4(VSme + 2 * (c * CROWS - SKEW + 2 * lane), vout_s[lane]);
+            // lane 31 worked on rows c CROWS - SKEW + 2t (+1) at step t
+            if (out_ring) {
+                // the highest entry of this chunk reuses the slot of the entry RING_ENTRIES below it (of this strip or of the
+                // strip before): my consumer must have taken it
+                const unsigned need = out_q + (unsigned)((c - RING_CHUNKS + 1) * CH);
+                unsigned seen = __shfl_sync(FULL, cons_seen, 0);
+                while ((int)(seen - need) < 0) {
+                    __nanosleep(64);
+                    if (lane == 0) cons_seen = ld_relaxed_u32(prog_of((mypos + 1) % FW));
+                    seen = __shfl_sync(FULL, cons_seen, 0);
+                }
+                const int q = c * CH - (SKEW / 2) + lane;               // r / 2 for r = c CROWS - SKEW + 2 lane
+                if (lane < CH && q >= 0) {
+                    const unsigned e = out_q + (unsigned)q;
+                    const unsigned long long tag = (unsigned long long)(e / RING_ENTRIES + 1u) << 32;
+                    const uint4 vo = vout_s[lane];
+                    unsigned long long* dst = ring_of(mypos) + (size_t)(e & (RING_ENTRIES - 1)) * 4;
+                    st_relaxed_v2u64(dst, tag | vo.x, tag | vo.y);
+                    st_relaxed_v2u64(dst + 2, tag | vo.z, tag | vo.w);
+                }
+            } else if (!out_none) {
+                if (lane < CH) st_relaxed_u4(VSme + 2 * (c * CROWS - SKEW + 2 * lane), vout_s[lane]);
+            }
         }
+        if (in_ring) in_q += (unsigned)(C * CH);
+        if (out_ring) out_q += (unsigned)(C * CH);
         // rows >= n were never touched, so ru / lu hold row n of every column: r_{n,m} sits in column m - 1
 #pragma unroll
         for (int w = 0; w < W; ++w) {

@@ -27,6 +27,7 @@ UserWs g_user_ws[64];         // caller-registered workspace, one per device (sd
 // settings never change another thread's launch
 thread_local bool g_profile = false;
 thread_local int g_dense_reverse = 0;
+thread_local int g_forward_kernel = -1;     // -1 = automatic, 0 = throughput instantiation, 1 = latency instantiation (LAT)
 thread_local int g_forward_rings = 1;       // 0: forward-only calls keep a boundary column per strip (sdtw_set_forward_rings)
 thread_local int g_reverse_kernel = -1;    // -1 = automatic, 0 = backward_kernel, 1 = reverse_kernel (sdtw_set_reverse_kernel)
 thread_local int g_unit_strips = 0;        // 0 = automatic (sdtw_set_schedule)
@@ -107,7 +108,8 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
         return (offsets[a + 1] - offsets[a]) > (offsets[b + 1] - offsets[b]);
     });
-    if (ring_sms > 0 && !want_grad && vs_words == 1 && d <= SDTW_MAX_D &&
+    // (the DTW kernels, vs_words == 2, have a CTA-full of 32 warps only at d <= 2: more channels keep a column per strip)
+    if (ring_sms > 0 && !want_grad && (vs_words == 1 ? d <= SDTW_MAX_D : d <= 2) &&
         (long long)L.NS * N > (long long)ring_sms * fwd_warps_rt(d)) {
         L.ring_units = fwd_warps_rt(d);
         L.ring_ctas = ring_sms;
@@ -135,7 +137,7 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
     L.off_prog_b = o;   o += align_up((size_t)L.items * 4, 256);
     L.off_hint_b = o;   o += align_up((size_t)L.items * 4, 256);
     if (L.ring_units) {         // zeroed with the counters: a ring entry is valid when its tag (>= 1) is the expected one
-        L.off_ring = o;      o += (size_t)L.ring_ctas * L.ring_units * RING_ENTRIES * 16;
+        L.off_ring = o;      o += (size_t)L.ring_ctas * L.ring_units * RING_ENTRIES * 16 * vs_words;
         L.off_ring_prog = o; o += align_up((size_t)L.ring_ctas * L.ring_units * 4, 256);
     }
     L.sync_bytes = o;
@@ -178,8 +180,21 @@ int get_device(DeviceInfo& di) {
     return SDTW_OK;
 }
 
+// Instantiated CUDA graph of a whole call on a small problem (launch-bound: a barycenter iteration on configs[0] is
+// four kernels of a few microseconds each).  Keyed by everything the captured launches bake in.
+struct GraphKey {
+    const void *Z, *X, *values, *objective, *grad, *ws;
+    int32_t iters, band;
+    float gamma, step;
+    bool operator==(const GraphKey& o) const { return std::memcmp(this, &o, sizeof(GraphKey)) == 0; }
+};
+struct GraphEntry { GraphKey key; cudaGraphExec_t exec = nullptr; uint64_t launches = 0, stamp = 0; };
+
 struct Plan {
     int dev = -1;
+    std::vector<GraphEntry> graphs;
+    std::vector<GraphKey> seen;   // keys met once: a graph is built when a key comes back (a caller that never repeats pays nothing)
+    long long cells = 0;          // sum_k n_k * m
     int64_t m = 0;
     int32_t d = 0, N = 0;
     bool want_grad = false;
@@ -219,6 +234,7 @@ int get_plan(const DeviceInfo& di, int64_t m, int32_t d, const int64_t* offsets,
     pl->ring_ok = ring_ok;
     pl->dev = dev; pl->m = m; pl->d = d; pl->N = N; pl->want_grad = want_grad;
     pl->offsets.assign(offsets, offsets + N + 1);
+    pl->cells = (long long)offsets[N] * m;
     cudaError_t e = cudaMalloc(&pl->d_pm, sizeof(PairMeta) * (size_t)N);
     if (e == cudaSuccess) e = cudaMemcpyAsync(pl->d_pm, pl->L.pm.data(), sizeof(PairMeta) * (size_t)N, cudaMemcpyHostToDevice, stream);
     if (e == cudaSuccess && weights) {                 // eq. 7 weights, permuted to schedule order
@@ -242,6 +258,7 @@ int get_plan(const DeviceInfo& di, int64_t m, int32_t d, const int64_t* offsets,
         auto it = std::min_element(g_plans.begin(), g_plans.end(), [](Plan* a, Plan* b) { return a->stamp < b->stamp; });
         cudaFree((*it)->d_pm);
         if ((*it)->d_w) cudaFree((*it)->d_w);
+        for (auto& ge : (*it)->graphs) cudaGraphExecDestroy(ge.exec);
         cudaEventDestroy((*it)->uploaded);
         delete *it;
         g_plans.erase(it);
@@ -264,11 +281,11 @@ int persistent_grid(K kernel, int smem_bytes, int sms, long long items, int* gri
     return SDTW_OK;
 }
 
-template <int D, bool CKPT>
+template <int D, bool CKPT, bool LAT>
 int launch_forward_t(Params P, int sms, cudaStream_t stream, int ring_ctas) {
     constexpr int FW = fwd_warps<D>();
     const int smem = FW * fwd_smem_floats<D>() * 4;
-    auto kernel = forward_kernel<D, CKPT, FW>;
+    auto kernel = forward_kernel<D, CKPT, FW, LAT>;
     CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int occ = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, FW * 32, smem));
@@ -304,7 +321,11 @@ int launch_forward_t(Params P, int sms, cudaStream_t stream, int ring_ctas) {
 
 template <int D>
 int launch_forward(const Params& P, bool ckpt, int sms, cudaStream_t stream, int ring_ctas) {
-    return ckpt ? launch_forward_t<D, true>(P, sms, stream, 0) : launch_forward_t<D, false>(P, sms, stream, ring_ctas);
+    // latency regime (every strip resident at once: a pair's chain of strips bounds the launch): the LAT instantiation
+    const bool lat = !P.ring && ((g_forward_kernel >= 0) ? (g_forward_kernel == 1)
+                                                         : ((long long)P.NS * P.N <= (long long)sms * fwd_warps<D>()));
+    if (lat) return ckpt ? launch_forward_t<D, true, true>(P, sms, stream, 0) : launch_forward_t<D, false, true>(P, sms, stream, 0);
+    return ckpt ? launch_forward_t<D, true, false>(P, sms, stream, 0) : launch_forward_t<D, false, false>(P, sms, stream, ring_ctas);
 }
 
 // Two reverse kernels, same arithmetic.  reverse_kernel (sdtw_reverse.cuh: a CTA of 4 warps per strip, the recompute off
@@ -363,31 +384,35 @@ int dispatch_backward(int d, const Params& P, int sms, cudaStream_t s) {
 }
 
 template <int D, bool SUB>
-int launch_dtw(const DtwParams& P, int sms, cudaStream_t stream) {
-    const int smem = DTW_WARPS * dtw_smem_floats<D>() * 4;
+int launch_dtw(const DtwParams& P, int sms, cudaStream_t stream, int ring_ctas) {
+    constexpr int FW = dtw_warps<D>();
+    const int smem = FW * dtw_smem_floats<D>() * 4;
     CUDA_TRY(cudaFuncSetAttribute(dtw_kernel<D, SUB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int occ = 0;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dtw_kernel<D, SUB>, DTW_WARPS * 32, smem));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dtw_kernel<D, SUB>, FW * 32, smem));
     if (occ < 1) return SDTW_ERR_UNSUPPORTED;
-    const long long want = ((long long)P.num_items + DTW_WARPS - 1) / DTW_WARPS;
-    const int grid = (int)std::max(1LL, std::min(want, (long long)sms * occ));
-    dtw_kernel<D, SUB><<<grid, DTW_WARPS * 32, smem, stream>>>(P);
+    const long long units = (long long)((P.NS + P.unit_strips - 1) / P.unit_strips) * P.N;
+    // one strip per unit: a CTA serves FW units at a time
+    const long long want = (P.unit_strips == 1) ? (units + FW - 1) / FW : units;
+    const long long ctas = P.ring ? std::min((long long)sms * occ, (long long)ring_ctas) : (long long)sms * occ;
+    const int grid = (int)std::max(1LL, std::min(want, ctas));
+    dtw_kernel<D, SUB><<<grid, FW * 32, smem, stream>>>(P);
     ++g_launches;
     CUDA_TRY(cudaGetLastError());
     return SDTW_OK;
 }
 template <bool SUB>
-int dispatch_dtw(int d, const DtwParams& P, int sms, cudaStream_t s) {
+int dispatch_dtw(int d, const DtwParams& P, int sms, cudaStream_t s, int ring_ctas) {
     switch (d) {
-        case 1: return launch_dtw<1, SUB>(P, sms, s);
-        case 2: return launch_dtw<2, SUB>(P, sms, s);
-        case 3: return launch_dtw<3, SUB>(P, sms, s);
-        case 4: return launch_dtw<4, SUB>(P, sms, s);
-        case 5: return launch_dtw<5, SUB>(P, sms, s);
-        case 6: return launch_dtw<6, SUB>(P, sms, s);
-        case 7: return launch_dtw<7, SUB>(P, sms, s);
-        case 8: return launch_dtw<8, SUB>(P, sms, s);
-        case 9: return launch_dtw<9, SUB>(P, sms, s);
+        case 1: return launch_dtw<1, SUB>(P, sms, s, ring_ctas);
+        case 2: return launch_dtw<2, SUB>(P, sms, s, ring_ctas);
+        case 3: return launch_dtw<3, SUB>(P, sms, s, ring_ctas);
+        case 4: return launch_dtw<4, SUB>(P, sms, s, ring_ctas);
+        case 5: return launch_dtw<5, SUB>(P, sms, s, ring_ctas);
+        case 6: return launch_dtw<6, SUB>(P, sms, s, ring_ctas);
+        case 7: return launch_dtw<7, SUB>(P, sms, s, ring_ctas);
+        case 8: return launch_dtw<8, SUB>(P, sms, s, ring_ctas);
+        case 9: return launch_dtw<9, SUB>(P, sms, s, ring_ctas);
     }
     return SDTW_ERR_UNSUPPORTED;
 }
@@ -435,14 +460,16 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     CUDA_TRY((cudaError_t)pr.mark(0, stream));
     int rc = SDTW_OK;
     if (phase & 1) {
-    CUDA_TRY(cudaMemsetAsync(ws + L.off_counters, 0, L.sync_bytes, stream));
-    // every word of the strip-boundary columns starts as the sentinel the consumers poll for (sdtw_kernels.cuh)
-    CUDA_TRY(cudaMemsetAsync(ws + L.off_VS, 0xFF, L.vs_bytes, stream));
-    if (pl.want_grad) CUDA_TRY(cudaMemsetAsync(ws + L.off_ES, 0xFF, L.vs_bytes, stream));   // same protocol in reverse
     {
+        // one launch: counters / progress words / rings := 0, strip-boundary columns VS (and ES: same protocol in reverse)
+        // := the sentinel pattern the consumers poll for (sdtw_kernels.cuh), scaled copies of the inputs
+        const FillJob f0{reinterpret_cast<uint4*>(ws + L.off_counters), L.sync_bytes / 16, 0u};
+        const FillJob f1{reinterpret_cast<uint4*>(ws + L.off_VS), L.vs_bytes / 16, SENTINEL};
+        const FillJob f2{reinterpret_cast<uint4*>(ws + (pl.want_grad ? L.off_ES : L.off_VS)), pl.want_grad ? L.vs_bytes / 16 : 0, SENTINEL};
         const long long nx = (long long)pl.offsets[pl.N] * pl.d, nz = (long long)pl.m * pl.d;
-        const int blocks = (int)std::min<long long>((nx + nz + 255) / 256, (long long)di.sms * 8);
-        scale_inputs_kernel<<<blocks, 256, 0, stream>>>(X, nx, Z, nz, sqrtk, Xs, Zs);
+        const unsigned long long work = (unsigned long long)(nx + nz) + f0.count16 + f1.count16 + f2.count16;
+        const int blocks = (int)std::min<unsigned long long>((work + 255) / 256, (unsigned long long)di.sms * 16);
+        prologue_kernel<<<std::max(blocks, 1), 256, 0, stream>>>(f0, f1, f2, X, nx, Z, nz, sqrtk, Xs, Zs);
         ++g_launches;
         CUDA_TRY(cudaGetLastError());
     }
@@ -456,18 +483,16 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
         if (rc) return rc;
     }
     CUDA_TRY((cudaError_t)pr.mark(3, stream));
-    if ((phase & 1) && (out_values || out_objective || out_objective64)) {
-        finalize_values_kernel<<<1, 256, 0, stream>>>(P.VP, pl.d_pm, P.wts, pl.N, L.NS, inv_kappa, out_values, out_objective,
-                                                      out_objective64);
-        ++g_launches;
-        CUDA_TRY(cudaGetLastError());
-    }
-    if (pl.want_grad && (phase & 2)) {
-        const long long md = (long long)pl.m * pl.d;
-        const int blocks = (int)((md + 255) / 256);
-        reduce_pairs_kernel<<<blocks, 256, 0, stream>>>(P.Gk, P.wts, pl.N, md, out_grad, Z_update, step);
-        ++g_launches;
-        CUDA_TRY(cudaGetLastError());
+    {
+        const int want_values = ((phase & 1) && (out_values || out_objective || out_objective64)) ? 1 : 0;
+        const long long md = (pl.want_grad && (phase & 2)) ? (long long)pl.m * pl.d : 0;
+        const int blocks = (int)((md + 255) / 256) + want_values;
+        if (blocks > 0) {
+            epilogue_kernel<<<blocks, 256, 0, stream>>>(P.VP, pl.d_pm, P.wts, pl.N, L.NS, inv_kappa, want_values, out_values,
+                                                        out_objective, out_objective64, P.Gk, md, out_grad, Z_update, step);
+            ++g_launches;
+            CUDA_TRY(cudaGetLastError());
+        }
     }
     CUDA_TRY((cudaError_t)pr.mark(4, stream));
     pr.keep();
@@ -545,6 +570,62 @@ struct Workspace {
     ~Workspace() { if (cache && cache->last_use) cudaEventRecord(cache->last_use, stream); }
 };
 
+// Small problems are launch-bound: the whole call (all iterations) is captured once on a private stream into a CUDA
+// graph, cached on the plan, and replayed on the caller's stream.  Not used while profiling or when a tuning switch of
+// sdtw_debug.h is set (the captured launches would bake it in).  `enqueue(stream)` issues the call's launches.
+constexpr long long GRAPH_MAX_CELLS = 250000000LL;   // about 1 ms of kernel time per evaluation
+cudaStream_t g_capture_stream[64];
+
+bool graph_eligible(const Plan& pl) {
+    return pl.cells <= GRAPH_MAX_CELLS && !g_profile && !g_dense_reverse && g_unit_strips == 0 && g_tail_strips < 0 &&
+           g_reverse_kernel < 0 && g_forward_kernel < 0;
+}
+
+template <typename F>
+int run_graphed(Plan& pl, const GraphKey& key, cudaStream_t stream, F enqueue) {
+    for (auto& ge : pl.graphs) {
+        if (ge.key == key) {
+            ge.stamp = ++g_stamp;
+            CUDA_TRY(cudaGraphLaunch(ge.exec, stream));
+            g_launches += ge.launches;
+            return SDTW_OK;
+        }
+    }
+    if (std::find(pl.seen.begin(), pl.seen.end(), key) == pl.seen.end()) {   // first time: plain launches
+        if (pl.seen.size() >= 8) pl.seen.erase(pl.seen.begin());
+        pl.seen.push_back(key);
+        return enqueue(stream);
+    }
+    cudaStream_t& cap = g_capture_stream[pl.dev];
+    if (!cap) CUDA_TRY(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    const uint64_t launches0 = g_launches;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    int rc = SDTW_OK;
+    if (cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return enqueue(stream); }
+    rc = enqueue(cap);
+    const cudaError_t e_end = cudaStreamEndCapture(cap, &graph);
+    const uint64_t n_launch = g_launches - launches0;
+    g_launches = launches0;                       // nothing ran during the capture
+    if (rc != SDTW_OK || e_end != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        return rc != SDTW_OK ? rc : enqueue(stream);   // argument errors surface as they would without a graph
+    }
+    cudaGraphDestroy(graph);
+    if (pl.graphs.size() >= 4) {                  // evict the least recently used graph of this plan
+        auto it = std::min_element(pl.graphs.begin(), pl.graphs.end(), [](const GraphEntry& a, const GraphEntry& b) { return a.stamp < b.stamp; });
+        cudaGraphExecDestroy(it->exec);
+        pl.graphs.erase(it);
+    }
+    GraphEntry ge;
+    ge.key = key; ge.exec = exec; ge.launches = n_launch; ge.stamp = ++g_stamp;
+    pl.graphs.push_back(ge);
+    CUDA_TRY(cudaGraphLaunch(exec, stream));
+    g_launches += n_launch;
+    return SDTW_OK;
+}
+
 }  // namespace
 
 // =================================================================================================================
@@ -569,7 +650,15 @@ int sdtw_value_grad_ex(const float* Z, int64_t m, int32_t d, const float* X_conc
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
     if (rc) return rc;
-    return evaluate(*pl, ws.ptr, di, Z, X_concat, gamma, band_eff, out_values, out_objective, out_grad, nullptr, 0.f, stream);
+    auto enqueue = [&](cudaStream_t st) {
+        return evaluate(*pl, ws.ptr, di, Z, X_concat, gamma, band_eff, out_values, out_objective, out_grad, nullptr, 0.f, st);
+    };
+    if (!graph_eligible(*pl)) return enqueue(stream);
+    GraphKey key;
+    std::memset(&key, 0, sizeof(key));                 // keys are compared bytewise, padding included
+    key.Z = Z; key.X = X_concat; key.values = out_values; key.objective = out_objective; key.grad = out_grad; key.ws = ws.ptr;
+    key.iters = -1; key.band = band_eff; key.gamma = gamma; key.step = 0.f;
+    return run_graphed(*pl, key, stream, enqueue);
 }
 
 int sdtw_value_grad(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
@@ -598,13 +687,21 @@ int sdtw_barycenter_ex(float* Z_inout, int64_t m, int32_t d, const float* X_conc
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
     if (rc) return rc;
-    for (int it = 0; it < iters; ++it) {
-        float* vals = (it == iters - 1) ? out_values : nullptr;
-        float* obj = out_objective ? out_objective + it : nullptr;
-        rc = evaluate(*pl, ws.ptr, di, Z_inout, X_concat, gamma, band_eff, vals, obj, nullptr, Z_inout, step, stream);
-        if (rc) return rc;
-    }
-    return SDTW_OK;
+    auto enqueue = [&](cudaStream_t st) {
+        for (int it = 0; it < iters; ++it) {
+            float* vals = (it == iters - 1) ? out_values : nullptr;
+            float* obj = out_objective ? out_objective + it : nullptr;
+            const int r = evaluate(*pl, ws.ptr, di, Z_inout, X_concat, gamma, band_eff, vals, obj, nullptr, Z_inout, step, st);
+            if (r) return r;
+        }
+        return (int)SDTW_OK;
+    };
+    if (!graph_eligible(*pl)) return enqueue(stream);
+    GraphKey key;
+    std::memset(&key, 0, sizeof(key));
+    key.Z = Z_inout; key.X = X_concat; key.values = out_values; key.objective = out_objective; key.grad = nullptr; key.ws = ws.ptr;
+    key.iters = iters; key.band = band_eff; key.gamma = gamma; key.step = step;
+    return run_graphed(*pl, key, stream, enqueue);
 }
 
 int sdtw_barycenter_backtracking(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets,
@@ -705,7 +802,7 @@ static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const floa
     rc = get_device(di);
     if (rc) return rc;
     Plan* pl = nullptr;
-    rc = get_plan(di, m, d, offsets, N, nullptr, false, stream, &pl, 2);
+    rc = get_plan(di, m, d, offsets, N, nullptr, false, stream, &pl, 2, g_forward_rings != 0);
     if (rc) return rc;
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
@@ -715,6 +812,9 @@ static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const floa
     P.Z = Z; P.X = X_concat; P.pm = pl->d_pm;
     P.counter = reinterpret_cast<unsigned*>(ws.ptr + L.off_counters);
     P.VS = reinterpret_cast<unsigned*>(ws.ptr + L.off_VS);
+    P.ring = L.ring_units ? reinterpret_cast<unsigned long long*>(ws.ptr + L.off_ring) : nullptr;
+    P.ring_prog = L.ring_units ? reinterpret_cast<unsigned*>(ws.ptr + L.off_ring_prog) : nullptr;
+    P.unit_strips = L.ring_units ? L.ring_units : 1;
     P.out_dtw = out_val; P.out_len = out_i0; P.out_score = out_score; P.out_b = out_i1;
     P.m = (int)m; P.N = N; P.NS = L.NS; P.num_items = (unsigned)L.items;
     ProfScope pr;
@@ -723,7 +823,7 @@ static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const floa
     CUDA_TRY(cudaMemsetAsync(ws.ptr + L.off_counters, 0, L.sync_bytes, stream));
     CUDA_TRY(cudaMemsetAsync(ws.ptr + L.off_VS, 0xFF, L.vs_bytes, stream));   // sentinel preset (dtw_kernel.cuh)
     CUDA_TRY((cudaError_t)pr.mark(1, stream));
-    rc = sub ? dispatch_dtw<true>(d, P, di.sms, stream) : dispatch_dtw<false>(d, P, di.sms, stream);
+    rc = sub ? dispatch_dtw<true>(d, P, di.sms, stream, L.ring_ctas) : dispatch_dtw<false>(d, P, di.sms, stream, L.ring_ctas);
     if (rc) return rc;
     for (int i = 2; i <= 4; ++i) CUDA_TRY((cudaError_t)pr.mark(i, stream));   // "forward" slot = the DTW kernel
     pr.keep();
@@ -823,6 +923,15 @@ size_t sdtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_
     return sdtw_workspace_bytes_ex(m, d, offsets, N, want_grad, -1);
 }
 
+size_t sdtw_dtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_t N) {
+    Layout L;
+    int sms = 148;
+    DeviceInfo di;
+    if (get_device(di) == SDTW_OK) sms = di.sms;
+    if (build_layout(m, d, offsets, N, false, L, 2, sms) != SDTW_OK) return 0;
+    return L.total;
+}
+
 int sdtw_set_workspace(void* dev_ptr, size_t bytes) {
     std::lock_guard<std::mutex> lock(g_mutex);
     if (dev_ptr && (reinterpret_cast<uintptr_t>(dev_ptr) & 255u)) return SDTW_ERR_INVALID_ARG;
@@ -905,6 +1014,13 @@ int sdtw_set_schedule(int unit_strips) {
 int sdtw_set_reverse_mode(int dense) {
     std::lock_guard<std::mutex> lock(g_mutex);
     g_dense_reverse = dense ? 1 : 0;
+    return SDTW_OK;
+}
+
+int sdtw_set_forward_kernel(int which) {
+    if (which < -1 || which > 1) return SDTW_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    g_forward_kernel = which;
     return SDTW_OK;
 }
 

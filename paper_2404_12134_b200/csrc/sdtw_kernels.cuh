@@ -26,6 +26,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 
 namespace sdtw {
 
@@ -270,6 +271,8 @@ struct SlowTag { static constexpr bool slow = true; static constexpr bool val = 
 // crosses sit at a different height in every strip, so a slow path there adds its delay to EVERY strip's hand-over and
 // lengthens the whole dependency chain of a pair (it did: 48 instead of 30 us per strip on a cfg-4 pair)
 struct FastValTag { static constexpr bool slow = false; static constexpr bool val = true; };
+// latency-regime kernel: ONE unrolled step for every chunk, rows outside the matrix computed and discarded by selects
+struct LatTag { static constexpr bool slow = false; static constexpr bool val = true; };
 
 // chunk c (steps c CH .. c CH + CH-1, rows c CROWS - SKEW .. c CROWS + CROWS-1 over the 32 lanes) touches only valid rows
 __device__ __forceinline__ bool interior_chunk(int c, int n) { return c * CROWS >= SKEW && c * CROWS + CROWS <= n; }
@@ -296,12 +299,23 @@ __device__ __forceinline__ void band_chunks(int J, int band, int C, int& cf, int
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// prologue: the scaled copies of the inputs the two wavefront kernels read
-__global__ void scale_inputs_kernel(const float* __restrict__ X, long long nx, const float* __restrict__ Z, long long nz,
-                                    float s, float* __restrict__ Xs, float* __restrict__ Zs) {
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < nx + nz; e += stride) {
-        if (e < nx) Xs[e] = X[e] * s; else Zs[e - nx] = Z[e - nx] * s;
+// prologue, one launch: clear the work counters / progress words / rings, preset the strip-boundary
+// columns VS and ES to the sentinel pattern the consumers poll for, and write the scaled copies of the inputs the two
+// wavefront kernels read.  Fill regions are multiples of 16 bytes (the workspace layout aligns them to 256).
+struct FillJob { uint4* ptr; unsigned long long count16; unsigned word; };
+__global__ void prologue_kernel(const FillJob f0, const FillJob f1, const FillJob f2,
+                                const float* __restrict__ X, long long nx, const float* __restrict__ Z, long long nz,
+                                float s, float* __restrict__ Xs, float* __restrict__ Zs) {
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    const unsigned long long t = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    for (unsigned long long e = t; e < (unsigned long long)(nx + nz); e += stride) {
+        if (e < (unsigned long long)nx) Xs[e] = X[e] * s; else Zs[e - nx] = Z[e - nx] * s;
+    }
+    const FillJob jobs[3] = {f0, f1, f2};
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const uint4 v = make_uint4(jobs[q].word, jobs[q].word, jobs[q].word, jobs[q].word);
+        for (unsigned long long e = t; e < jobs[q].count16; e += stride) __stcs(jobs[q].ptr + e, v);
     }
 }
 
@@ -320,7 +334,48 @@ __global__ void scale_inputs_kernel(const float* __restrict__ X, long long nx, c
 constexpr int UNIT_RING = 16;
 struct RollCtl { int popped; int lock; int uid[UNIT_RING]; int seen[32]; };
 
-template <int D, bool CKPT, int FW>
+// the CTA's k-th unit (>= NU: the queue is empty): popped from the global counter by whichever warp needs it first
+template <int FW>
+__device__ __forceinline__ int pop_unit(RollCtl& ctl, unsigned* counter, const int k, const int NU, const int warp, const int lane) {
+    int u = 0;
+    if (lane == 0) {
+        volatile RollCtl* vc = &ctl;
+        while (vc->popped <= k) {
+            if (atomicCAS(&ctl.lock, 0, 1) == 0) {
+                const int pc = vc->popped;
+                if (pc <= k) {
+                    for (;;) {                         // ring slot free: every warp has read unit pc - UNIT_RING
+                        int mn = vc->seen[0];
+                        for (int w2 = 1; w2 < FW; ++w2) mn = min(mn, vc->seen[w2]);
+                        if (mn > pc - UNIT_RING) break;
+                        __nanosleep(100);
+                    }
+                    vc->uid[pc % UNIT_RING] = (int)min(atomicAdd(counter, 1u), (unsigned)NU);
+                    __threadfence_block();
+                    vc->popped = pc + 1;
+                }
+                __threadfence_block();
+                atomicExch(&ctl.lock, 0);
+            } else {
+                __nanosleep(50);
+            }
+        }
+        __threadfence_block();
+        u = vc->uid[k % UNIT_RING];
+        vc->seen[warp] = k + 1;
+    }
+    return __shfl_sync(FULL, u, 0);
+}
+
+//
+// LAT (latency regime: every strip of the problem is resident at once, so a pair's chain of strips bounds the launch).
+// A strip can start chunk c when its left neighbour has published chunk c + 1, so the hand-over from strip to strip costs
+// the neighbour's first TWO chunks -- and chunk 0, where the lanes enter one by one, ran the general step at half speed:
+// 18 + 9 us per strip, inherited by every strip to the right.  The LAT instantiation runs one unrolled step on every
+// chunk: rows outside [0, n) are computed on zero-filled data and discarded by selects, the staircase bookkeeping is
+// always on.  Same cells, same operations, same order of the value additions: bitwise the results of the other kernel.
+// It holds no other unrolled variant (the general step remains for bands and m < W), so it is the smaller binary.
+template <int D, bool CKPT, int FW, bool LAT>
 __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kernel(const Params p) {
     extern __shared__ __align__(16) float smem[];
     __shared__ RollCtl ctl;
@@ -340,34 +395,7 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
     int base = 0;                                          // strips of the units before unit k, mod FW
     unsigned in_q = 0, out_q = 0;                          // ring entries consumed from the left / produced, all strips so far
     for (int k = 0;; ++k) {
-        int u = 0;
-        if (lane == 0) {                                   // the CTA's k-th unit: popped by whichever warp needs it first
-            volatile RollCtl* vc = &ctl;
-            while (vc->popped <= k) {
-                if (atomicCAS(&ctl.lock, 0, 1) == 0) {
-                    const int pc = vc->popped;
-                    if (pc <= k) {
-                        for (;;) {                         // ring slot free: every warp has read unit pc - UNIT_RING
-                            int mn = vc->seen[0];
-                            for (int w2 = 1; w2 < FW; ++w2) mn = min(mn, vc->seen[w2]);
-                            if (mn > pc - UNIT_RING) break;
-                            __nanosleep(100);
-                        }
-                        vc->uid[pc % UNIT_RING] = (int)min(atomicAdd(p.counters + 0, 1u), (unsigned)NU);
-                        __threadfence_block();
-                        vc->popped = pc + 1;
-                    }
-                    __threadfence_block();
-                    atomicExch(&ctl.lock, 0);
-                } else {
-                    __nanosleep(50);
-                }
-            }
-            __threadfence_block();
-            u = vc->uid[k % UNIT_RING];
-            vc->seen[warp] = k + 1;
-        }
-        u = __shfl_sync(FULL, u, 0);
+        const int u = pop_unit<FW>(ctl, p.counters + 0, k, NU, warp, lane);
         if (u >= NU) break;
         const int g = u / p.N, ps = u - g * p.N;
         const int Jg = (g < NG1) ? g * US : p.tail_from + (g - NG1) * p.tail_unit;   // first strip of this unit
@@ -460,7 +488,37 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
             if (lane == 0) { const float2 qv = vin_s[t]; va = qv.x; vb = qv.y; }
             XRow<D> xa, xb;
             load_x2<D>(xs_lane, 2 * t, xa, xb);
-            if constexpr (!slow) {
+            if constexpr (std::is_same<decltype(tag), LatTag>::value) {
+                const int i0 = RP * (c * CH + t - lane);
+                const bool actA = (unsigned)i0 < (unsigned)n, actB = (unsigned)(i0 + 1) < (unsigned)n;
+                float hA[W], hB[W], dummy0, dummy1;
+#pragma unroll
+                for (int w = 0; w < W; ++w) {
+                    float tl, acc;
+                    hA[w] = h[w];
+                    sqdist2<D>(xa, z[w], tl, acc);
+                    cell<false, (D > 1)>(tl, acc, hA[w], va, dummy0, dummy1, D <= 2 && ((SDTW_POLY_MASK_A >> w) & 1));
+                    hB[w] = hA[w];
+                    sqdist2<D>(xb, z[w], tl, acc);
+                    cell<false, (D > 1)>(tl, acc, hB[w], vb, dummy0, dummy1, D <= 2 && ((SDTW_POLY_MASK_B >> w) & 1));
+                }
+                // the value staircase: the additions of the general row, in its order (rows outside [0, n) match no window)
+                if ((unsigned)(i0 - r_v0 - 1) < (unsigned)(r_v1 - r_v0)) vacc += va;
+                if (i0 == r_h) {
+#pragma unroll
+                    for (int w = 0; w < W; ++w) if (j0 + w >= jlo && j0 + w <= jhi) hsum += hA[w];
+                }
+                if (T == 0 && i0 == 0) hsum += sqdist<D>(xa, z[0]);   // r_11 = D_11
+                if ((unsigned)(i0 - r_v0) < (unsigned)(r_v1 - r_v0)) vacc += vb;
+                if (i0 + 1 == r_h) {
+#pragma unroll
+                    for (int w = 0; w < W; ++w) if (j0 + w >= jlo && j0 + w <= jhi) hsum += hB[w];
+                }
+#pragma unroll
+                for (int w = 0; w < W; ++w) h[w] = actB ? hB[w] : (actA ? hA[w] : h[w]);
+                vp0 = actA ? va : vp0;
+                vp1 = actB ? vb : vp1;
+            } else if constexpr (!slow) {
                 constexpr bool val = decltype(tag)::val;
                 const int i0 = RP * (c * CH + t - lane);   // used by the staircase bookkeeping only
                 float dummy0, dummy1;
@@ -520,6 +578,47 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
                 vbad = (r < n && is_sentinel(vreg.x)) || (r + 1 < n && is_sentinel(vreg.y));
             }
         };
+        // LAT, no band, m >= W: the boundary values are exchanged per BLOCK of TR steps instead of per chunk.  Lane 31 reaches
+        // rows 2 s' - 62 at its step s', so the right strip's block k needs this strip's block k + 4: it runs 5 blocks (40
+        // steps) behind instead of two chunks (64 steps), and the chain of a pair shortens accordingly.
+        bool fine = false;
+        if constexpr (LAT) fine = (band < 0 && Tfull > 0);
+        if (fine) {
+            float2 breg = make_float2(0.f, 0.f);           // lanes < TR: boundary values of the next block's steps
+            bool bbad = false;
+            auto load_blk = [&](const int blk) {           // blk = c (CH / TR) + b; lane u < TR: rows of step blk TR + u
+                const int r = RP * (blk * TR + (lane & (TR - 1)));
+                breg = ld_relaxed_f2(VSprev + r);
+                bbad = lane < TR && ((r < n && is_sentinel(breg.x)) || (r + 1 < n && is_sentinel(breg.y)));
+            };
+            if (J > 0) load_blk(0);
+            for (int c = 0; c <= cl; ++c) {
+                cp_async_wait_all();
+                __syncwarp();
+                if (c + 1 <= cl) stage_x_async<D>(xs0 + ((c + 1) & 1) * XWIN * D, p.Xs, pm.x_off, n, c + 1, lane);
+                xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;
+#pragma unroll 1
+                for (int b = 0; b < CH / TR; ++b) {
+                    const int blk = c * (CH / TR) + b;
+                    if (J > 0) {
+                        while (__any_sync(FULL, bbad)) {
+                            if (bbad) load_blk(blk);
+                        }
+                    } else {
+                        breg = make_float2((blk == 0 && lane == 0) ? BIG : 0.f, 0.f);
+                    }
+                    if (lane < TR) vin_s[b * TR + lane] = breg;
+                    __syncwarp();
+                    if (J > 0 && blk + 1 < (cl + 1) * (CH / TR)) load_blk(blk + 1);
+#pragma unroll
+                    for (int u = 0; u < TR; ++u) step(c, b * TR + u, LatTag{});
+                    if (CKPT) checkpoint(blk + 1);
+                    __syncwarp();
+                    // lane 31 worked on rows c CROWS - SKEW + 2t (+1) at step t
+                    if (lane < TR) st_relaxed_f2(VSme + c * CROWS - SKEW + 2 * (b * TR + lane), vout_s[b * TR + lane]);
+                }
+            }
+        } else {
         if (J > 0) load_in(cf);
         unsigned cons_seen = 0;                            // my consumer's progress as last read (rings)
 
@@ -547,6 +646,22 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
             }
             xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;    // rows of step t: xs_lane[2t], [2t+1]
             const bool inside = interior_chunk(c, n) && band_clear(c, J, band);
+            if constexpr (LAT) {
+                if (band < 0 && Tfull > 0) {
+#pragma unroll 1
+                    for (int b = 0; b < CH / TR; ++b) {
+#pragma unroll
+                        for (int u = 0; u < TR; ++u) step(c, b * TR + u, LatTag{});
+                        if (CKPT) checkpoint(c * (CH / TR) + b + 1);
+                    }
+                } else {
+#pragma unroll 1
+                    for (int t = 0; t < CH; ++t) {
+                        step(c, t, SlowTag{});
+                        if (CKPT && ((t + 1) & (TR - 1)) == 0) checkpoint((c * CH + t + 1) / TR);
+                    }
+                }
+            } else
             if (inside && (c < c_v0 || c > c_v1)) {
 #pragma unroll 1
                 for (int b = 0; b < CH / TR; ++b) {
@@ -593,6 +708,7 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
                 if (lane < CH) st_relaxed_f2(VSme + c * CROWS - SKEW + 2 * lane, vout_s[lane]);
             }
         }
+        }   // !fine
         if (in_ring) in_q += (unsigned)(C * CH);
         if (out_ring) out_q += (unsigned)(C * CH);
         if (cl < C - 1) {
@@ -885,34 +1001,34 @@ __global__ void __launch_bounds__(WARPS * 32) backward_kernel(const Params p) {
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// small kernels: per-pair values from the item partials, objective, reduction over pairs, descent step
-__global__ void finalize_values_kernel(const double* __restrict__ VP, const PairMeta* __restrict__ pm,
-                                       const float* __restrict__ wts, int N, int NS,
-                                       double inv_kappa, float* __restrict__ out_values, float* __restrict__ out_objective,
-                                       double* __restrict__ out_objective64) {
+// epilogue, one launch.  Last block (if want_values): per-pair values from the item partials in caller order, objective
+// (eq. 7: sum_k w_k value_k) by a fixed-shape tree.  Other blocks (if md > 0): G[e] = sum over pairs in schedule order with
+// an fp64 accumulator (deterministic, no atomics), optionally fused with the descent step Z <- Z - step G.
+__global__ void epilogue_kernel(const double* __restrict__ VP, const PairMeta* __restrict__ pm, const float* __restrict__ wts,
+                                int N, int NS, double inv_kappa, int want_values, float* __restrict__ out_values,
+                                float* __restrict__ out_objective, double* __restrict__ out_objective64,
+                                const float* __restrict__ Gk, long long md, float* __restrict__ out_grad, float* __restrict__ Z,
+                                float step) {
     __shared__ double red[256];
-    double local = 0.0;
-    for (int ps = threadIdx.x; ps < N; ps += blockDim.x) {
-        double s = 0.0;
-        for (int J = 0; J < NS; ++J) s += VP[(long long)ps * NS + J];
-        s *= inv_kappa;
-        if (out_values) out_values[pm[ps].k] = (float)s;
-        local += wts ? (double)wts[ps] * s : s;              // eq. 7: objective = sum_k w_k value_k
-    }
-    // objective: fixed-shape tree over the block (deterministic)
-    red[threadIdx.x] = local;
-    __syncthreads();
-    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
-        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+    if (want_values && blockIdx.x == gridDim.x - 1) {
+        double local = 0.0;
+        for (int ps = threadIdx.x; ps < N; ps += blockDim.x) {
+            double s = 0.0;
+            for (int J = 0; J < NS; ++J) s += VP[(long long)ps * NS + J];
+            s *= inv_kappa;
+            if (out_values) out_values[pm[ps].k] = (float)s;
+            local += wts ? (double)wts[ps] * s : s;
+        }
+        red[threadIdx.x] = local;
         __syncthreads();
+        for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+            if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0 && out_objective) *out_objective = (float)red[0];
+        if (threadIdx.x == 0 && out_objective64) *out_objective64 = red[0];
+        return;
     }
-    if (threadIdx.x == 0 && out_objective) *out_objective = (float)red[0];
-    if (threadIdx.x == 0 && out_objective64) *out_objective64 = red[0];
-}
-
-// G[e] = sum over pairs (schedule order, fp64 accumulator: deterministic, no atomics); optional descent step
-__global__ void reduce_pairs_kernel(const float* __restrict__ Gk, const float* __restrict__ wts, int N, long long md,
-                                    float* __restrict__ out_grad, float* __restrict__ Z, float step) {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= md) return;
     double acc = 0.0;

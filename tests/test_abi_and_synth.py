@@ -82,6 +82,13 @@ def test_workspace_bytes_planner(binding):
     assert binding.sdtw_workspace_bytes(10, 5, off, True) == 0                        # d above compiled maximum
     # size is monotone in the problem
     assert binding.sdtw_workspace_bytes(30000, 1, off[:3], True) < full
+    # forward-only sweeps keep O(chunks) boundary state per resident strip and one column per unit of strips (SURVEY.md
+    # 8(a) a3): the scoring sweep of configs[4] (1000 cycles of 20-40k against m = 30000) needs about 1 GB, not a column
+    # per strip (28 GB, what a banded forward-only call of the same shape still takes); the DTW kernels likewise
+    off5 = synth.make(5)["offsets"]
+    assert binding.sdtw_workspace_bytes(30000, 1, off5, False) < 1.1e9
+    assert binding.sdtw_workspace_bytes_ex(30000, 1, off5, False, 25000) > 25e9
+    assert binding.sdtw_dtw_workspace_bytes(30000, 1, off5) < 2.2e9
 
 
 def test_synth_is_deterministic_and_shaped():
