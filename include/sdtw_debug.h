@@ -62,12 +62,6 @@ int sdtw_set_reverse_kernel(int which);
  * sdtw_workspace_bytes_ex and a band that excludes a cell); 1 restores the default.  The values are bitwise the same.
  */
 int sdtw_set_forward_rings(int on);
-/*
- * The forward kernel has a throughput instantiation (0) and a latency instantiation (1: one unrolled step on every
- * chunk, rows outside the matrix discarded by selects; sdtw_kernels.cuh, LAT).  -1 (default): the latency one when
- * every strip of the problem is resident at once.  Bitwise the same results.  Other values => SDTW_ERR_INVALID_ARG.
- */
-int sdtw_set_forward_kernel(int which);
 
 /*
  * Forward schedule (tuning, does not change any result bit): the forward kernel hands out UNITS of `unit_strips`

@@ -45,7 +45,6 @@ SYMBOLS = {
     "sdtw_set_reverse_mode": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_reverse_kernel": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_forward_rings": (ctypes.c_int, [ctypes.c_int]),
-    "sdtw_set_forward_kernel": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_schedule": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_set_schedule_tail": (ctypes.c_int, [ctypes.c_int, ctypes.c_int]),
     "sdtw_reverse_stats": (ctypes.c_int, [ctypes.POINTER(ctypes.c_uint64)] * 2),
@@ -394,11 +393,6 @@ def sdtw_set_reverse_mode(dense: bool):
 def sdtw_set_reverse_kernel(which: int = -1):
     """-1 automatic, 0 one warp per strip (throughput regime), 1 one CTA per strip (latency regime).  Same arithmetic."""
     _check(_lib.sdtw_set_reverse_kernel(int(which)))
-
-
-def sdtw_set_forward_kernel(which: int = -1):
-    """-1 automatic, 0 throughput instantiation, 1 latency instantiation of the forward kernel.  Bitwise the same results."""
-    _check(_lib.sdtw_set_forward_kernel(int(which)))
 
 
 def sdtw_set_forward_rings(on: bool = True):

@@ -12,18 +12,22 @@
 // Same wavefront as the Soft-DTW forward kernel (sdtw_kernels.cuh): a work item is one strip of 32 x W columns of one
 // pair swept by one warp, lane l on rows 2(s-l), 2(s-l)+1 at step s; (r, len) of a lane's last column goes to the next
 // lane by shuffle and to the next strip through a sentinel-preset global column polled one chunk ahead.  No special
-// functions: the bound is the FP32/ALU issue rate.  Schedule: the forward kernel's (units of adjacent strips popped
-// group-major by a CTA whose warps serve a rolling stream of strips).  When the problem has more strips than resident
-// warps a unit is a CTA-full and the boundary values travel inside a unit through per-warp rings (as in the forward-only
-// Soft-DTW sweep; an entry carries (r, len) of two rows as four tagged 64-bit words); only the last strip of a unit
-// keeps a full column.  Otherwise every strip is its own unit and keeps a column.
+// functions: the bound is the FP32/ALU issue rate.  Two layouts.  COLUMNS (FW = 8): items are handed out strip-major from
+// one atomic counter to independent warps (every item's producer was handed out earlier, so a waiting warp never blocks
+// the warp it waits for) and every strip keeps a boundary column.  RINGS (FW = 32, chosen when the problem has more
+// strips than resident warps, d <= 2): the forward kernel's schedule -- units of 32 adjacent strips popped group-major by
+// a CTA whose warps serve a rolling stream of strips -- with the boundary values travelling inside a unit through
+// per-warp rings (as in the forward-only Soft-DTW sweep; an entry carries (r, len) of two rows as four tagged 64-bit
+// words); only the last strip of a unit keeps a full column.  cfg 5: 56.7 -> 1.9 GB of workspace, 326 -> 352 ms.
 #pragma once
 #include "sdtw_kernels.cuh"
 
 namespace sdtw {
 
-// warps per CTA = strips per unit: a CTA-full at d <= 2 (the kernel fits 64 registers), 8 warps at more channels
-template <int D> __host__ __device__ constexpr int dtw_warps() { return D <= 2 ? 32 : 8; }
+// warps per CTA: 8 independent warps in the column layout; a CTA-full of 32 (= strips per unit) in the ring layout, which
+// exists at d <= 2 only (the kernel fits 64 registers there)
+constexpr int DTW_WARPS = 8;
+constexpr int DTW_RING_WARPS = 32;
 #ifndef SDTW_DTW_W
 #define SDTW_DTW_W 4
 #endif
@@ -40,7 +44,6 @@ struct DtwParams {
     unsigned* VS;         // strip-boundary columns: word 2 row = r bits, word 2 row + 1 = len
     unsigned long long* ring;   // [CTA][warp position][RING_ENTRIES][4]: (r, len) of a row pair, each word | tag << 32; or null
     unsigned* ring_prog;        // [CTA][warp position] entries of the left neighbour's ring this warp has consumed
-    int unit_strips;      // strips per unit: the CTA's warps (rings inside a unit, a column after it), or 1 (a column per strip)
     float* out_dtw;       // [N] caller order (may be null): DTW, or the Sub-DTW value
     int* out_len;         // [N] (may be null): |pi|, or a* (Sub-DTW)
     float* out_score;     // [N] (may be null): DTW / |pi| (not written by the Sub-DTW variant)
@@ -86,10 +89,10 @@ __device__ __forceinline__ void dtw_cell(const XRow<D>& x, const float (&z)[D], 
 
 // SUB = false: eq. 1 / eq. 8 (complete paths).  SUB = true: eq. 2, the rows (the series of
 // X_concat) have free ends: r_i0 = 0 for every i, value = min_i r_im, b* = the smallest such i, a* = the path's first row.
-template <int D, bool SUB>
-__global__ void __launch_bounds__(dtw_warps<D>() * 32) dtw_kernel(const DtwParams p) {
+template <int D, bool SUB, int FW>
+__global__ void __launch_bounds__(FW * 32) dtw_kernel(const DtwParams p) {
     constexpr int W = dtw_w<D>();                                    // shadows sdtw::W inside this kernel
-    constexpr int FW = dtw_warps<D>();
+    constexpr bool RINGS = (FW == DTW_RING_WARPS);
     extern __shared__ __align__(16) float smem[];
     __shared__ RollCtl ctl;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -98,8 +101,8 @@ __global__ void __launch_bounds__(dtw_warps<D>() * 32) dtw_kernel(const DtwParam
     uint4* vout_s = vin_s + 32;                                      // [CH] (r, len) of lane 31's last column
     const int m = p.m;
     const float INF = __uint_as_float(F_INF);
-    const int US = p.unit_strips;
-    const int NG = (p.NS + US - 1) / US, NU = NG * p.N;              // units per pair, units
+    constexpr int US = FW;                                            // RINGS: strips per unit
+    const int NG = (p.NS + US - 1) / US, NU = NG * p.N;              // RINGS: units per pair, units
     const int mypos = (warp & 3) * (FW / 4) + (warp >> 2);           // consecutive positions share a scheduler
     if (threadIdx.x < 32) { ctl.seen[threadIdx.x] = 0; if (threadIdx.x == 0) { ctl.popped = 0; ctl.lock = 0; } }
     __syncthreads();
@@ -107,18 +110,27 @@ __global__ void __launch_bounds__(dtw_warps<D>() * 32) dtw_kernel(const DtwParam
     int base = 0;
     unsigned in_q = 0, out_q = 0;                          // ring entries consumed from the left / produced, all strips so far
     for (int k = 0;; ++k) {
-        const int u = pop_unit<FW>(ctl, p.counter, k, NU, warp, lane);
-        if (u >= NU) break;
-        const int g = u / p.N, ps = u - g * p.N;             // group-major: every pair's unit g before any unit g + 1
-        const int S = min(US, p.NS - g * US);
-        const int sidx = (mypos - base + FW) % FW;
-        base = (base + S) % FW;
-        if (sidx >= S) continue;
-        const int J = g * US + sidx;
+        int J, ps, g = 0, S = 1, sidx = 0;
+        if constexpr (RINGS) {
+            const int u = pop_unit<FW>(ctl, p.counter, k, NU, warp, lane);
+            if (u >= NU) break;
+            g = u / p.N; ps = u - g * p.N;                   // group-major: every pair's unit g before any unit g + 1
+            S = min(US, p.NS - g * US);
+            sidx = (mypos - base + FW) % FW;
+            base = (base + S) % FW;
+            if (sidx >= S) continue;
+            J = g * US + sidx;
+        } else {
+            unsigned q = 0;
+            if (lane == 0) q = atomicAdd(p.counter, 1u);
+            q = __shfl_sync(FULL, q, 0);
+            if (q >= p.num_items) break;
+            J = q / p.N; ps = q - J * p.N;                   // strip-major: every pair's strip J before any strip J + 1
+        }
         const PairMeta pm = p.pm[ps];
         const int n = pm.n, C = pm.C;
         const int j0 = (J * 32 + lane) * W;
-        const bool rings = p.ring != nullptr;
+        constexpr bool rings = RINGS;
         const bool in_ring = rings && sidx > 0, out_ring = rings && sidx + 1 < S;
         const bool out_none = rings && !out_ring && J == p.NS - 1;
         const long long col = rings ? (out_ring ? 0 : g) : J;

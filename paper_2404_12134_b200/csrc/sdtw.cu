@@ -27,7 +27,6 @@ UserWs g_user_ws[64];         // caller-registered workspace, one per device (sd
 // settings never change another thread's launch
 thread_local bool g_profile = false;
 thread_local int g_dense_reverse = 0;
-thread_local int g_forward_kernel = -1;     // -1 = automatic, 0 = throughput instantiation, 1 = latency instantiation (LAT)
 thread_local int g_forward_rings = 1;       // 0: forward-only calls keep a boundary column per strip (sdtw_set_forward_rings)
 thread_local int g_reverse_kernel = -1;    // -1 = automatic, 0 = backward_kernel, 1 = reverse_kernel (sdtw_set_reverse_kernel)
 thread_local int g_unit_strips = 0;        // 0 = automatic (sdtw_set_schedule)
@@ -281,11 +280,11 @@ int persistent_grid(K kernel, int smem_bytes, int sms, long long items, int* gri
     return SDTW_OK;
 }
 
-template <int D, bool CKPT, bool LAT>
+template <int D, bool CKPT>
 int launch_forward_t(Params P, int sms, cudaStream_t stream, int ring_ctas) {
     constexpr int FW = fwd_warps<D>();
     const int smem = FW * fwd_smem_floats<D>() * 4;
-    auto kernel = forward_kernel<D, CKPT, FW, LAT>;
+    auto kernel = forward_kernel<D, CKPT, FW>;
     CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int occ = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, FW * 32, smem));
@@ -321,11 +320,7 @@ int launch_forward_t(Params P, int sms, cudaStream_t stream, int ring_ctas) {
 
 template <int D>
 int launch_forward(const Params& P, bool ckpt, int sms, cudaStream_t stream, int ring_ctas) {
-    // latency regime (every strip resident at once: a pair's chain of strips bounds the launch): the LAT instantiation
-    const bool lat = !P.ring && ((g_forward_kernel >= 0) ? (g_forward_kernel == 1)
-                                                         : ((long long)P.NS * P.N <= (long long)sms * fwd_warps<D>()));
-    if (lat) return ckpt ? launch_forward_t<D, true, true>(P, sms, stream, 0) : launch_forward_t<D, false, true>(P, sms, stream, 0);
-    return ckpt ? launch_forward_t<D, true, false>(P, sms, stream, 0) : launch_forward_t<D, false, false>(P, sms, stream, ring_ctas);
+    return ckpt ? launch_forward_t<D, true>(P, sms, stream, 0) : launch_forward_t<D, false>(P, sms, stream, ring_ctas);
 }
 
 // Two reverse kernels, same arithmetic.  reverse_kernel (sdtw_reverse.cuh: a CTA of 4 warps per strip, the recompute off
@@ -383,23 +378,31 @@ int dispatch_backward(int d, const Params& P, int sms, cudaStream_t s) {
     return SDTW_ERR_UNSUPPORTED;
 }
 
-template <int D, bool SUB>
-int launch_dtw(const DtwParams& P, int sms, cudaStream_t stream, int ring_ctas) {
-    constexpr int FW = dtw_warps<D>();
+template <int D, bool SUB, int FW>
+int launch_dtw_t(const DtwParams& P, int sms, cudaStream_t stream, int ring_ctas) {
     const int smem = FW * dtw_smem_floats<D>() * 4;
-    CUDA_TRY(cudaFuncSetAttribute(dtw_kernel<D, SUB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    auto kernel = dtw_kernel<D, SUB, FW>;
+    CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int occ = 0;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, dtw_kernel<D, SUB>, FW * 32, smem));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, FW * 32, smem));
     if (occ < 1) return SDTW_ERR_UNSUPPORTED;
-    const long long units = (long long)((P.NS + P.unit_strips - 1) / P.unit_strips) * P.N;
-    // one strip per unit: a CTA serves FW units at a time
-    const long long want = (P.unit_strips == 1) ? (units + FW - 1) / FW : units;
-    const long long ctas = P.ring ? std::min((long long)sms * occ, (long long)ring_ctas) : (long long)sms * occ;
+    long long want, ctas = (long long)sms * occ;
+    if (FW == DTW_RING_WARPS) {                     // ring layout: one unit of FW strips at a time per CTA
+        want = (long long)((P.NS + FW - 1) / FW) * P.N;
+        ctas = std::min(ctas, (long long)ring_ctas);
+    } else {
+        want = ((long long)P.num_items + FW - 1) / FW;
+    }
     const int grid = (int)std::max(1LL, std::min(want, ctas));
-    dtw_kernel<D, SUB><<<grid, FW * 32, smem, stream>>>(P);
+    kernel<<<grid, FW * 32, smem, stream>>>(P);
     ++g_launches;
     CUDA_TRY(cudaGetLastError());
     return SDTW_OK;
+}
+template <int D, bool SUB>
+int launch_dtw(const DtwParams& P, int sms, cudaStream_t stream, int ring_ctas) {
+    if constexpr (D <= 2) { if (P.ring) return launch_dtw_t<D, SUB, DTW_RING_WARPS>(P, sms, stream, ring_ctas); }
+    return launch_dtw_t<D, SUB, DTW_WARPS>(P, sms, stream, 0);
 }
 template <bool SUB>
 int dispatch_dtw(int d, const DtwParams& P, int sms, cudaStream_t s, int ring_ctas) {
@@ -578,7 +581,7 @@ cudaStream_t g_capture_stream[64];
 
 bool graph_eligible(const Plan& pl) {
     return pl.cells <= GRAPH_MAX_CELLS && !g_profile && !g_dense_reverse && g_unit_strips == 0 && g_tail_strips < 0 &&
-           g_reverse_kernel < 0 && g_forward_kernel < 0;
+           g_reverse_kernel < 0;
 }
 
 template <typename F>
@@ -814,7 +817,6 @@ static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const floa
     P.VS = reinterpret_cast<unsigned*>(ws.ptr + L.off_VS);
     P.ring = L.ring_units ? reinterpret_cast<unsigned long long*>(ws.ptr + L.off_ring) : nullptr;
     P.ring_prog = L.ring_units ? reinterpret_cast<unsigned*>(ws.ptr + L.off_ring_prog) : nullptr;
-    P.unit_strips = L.ring_units ? L.ring_units : 1;
     P.out_dtw = out_val; P.out_len = out_i0; P.out_score = out_score; P.out_b = out_i1;
     P.m = (int)m; P.N = N; P.NS = L.NS; P.num_items = (unsigned)L.items;
     ProfScope pr;
@@ -1014,13 +1016,6 @@ int sdtw_set_schedule(int unit_strips) {
 int sdtw_set_reverse_mode(int dense) {
     std::lock_guard<std::mutex> lock(g_mutex);
     g_dense_reverse = dense ? 1 : 0;
-    return SDTW_OK;
-}
-
-int sdtw_set_forward_kernel(int which) {
-    if (which < -1 || which > 1) return SDTW_ERR_INVALID_ARG;
-    std::lock_guard<std::mutex> lock(g_mutex);
-    g_forward_kernel = which;
     return SDTW_OK;
 }
 

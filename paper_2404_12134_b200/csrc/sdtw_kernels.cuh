@@ -26,7 +26,6 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
-#include <type_traits>
 
 namespace sdtw {
 
@@ -271,8 +270,6 @@ struct SlowTag { static constexpr bool slow = true; static constexpr bool val = 
 // crosses sit at a different height in every strip, so a slow path there adds its delay to EVERY strip's hand-over and
 // lengthens the whole dependency chain of a pair (it did: 48 instead of 30 us per strip on a cfg-4 pair)
 struct FastValTag { static constexpr bool slow = false; static constexpr bool val = true; };
-// latency-regime kernel: ONE unrolled step for every chunk, rows outside the matrix computed and discarded by selects
-struct LatTag { static constexpr bool slow = false; static constexpr bool val = true; };
 
 // chunk c (steps c CH .. c CH + CH-1, rows c CROWS - SKEW .. c CROWS + CROWS-1 over the 32 lanes) touches only valid rows
 __device__ __forceinline__ bool interior_chunk(int c, int n) { return c * CROWS >= SKEW && c * CROWS + CROWS <= n; }
@@ -367,15 +364,7 @@ __device__ __forceinline__ int pop_unit(RollCtl& ctl, unsigned* counter, const i
     return __shfl_sync(FULL, u, 0);
 }
 
-//
-// LAT (latency regime: every strip of the problem is resident at once, so a pair's chain of strips bounds the launch).
-// A strip can start chunk c when its left neighbour has published chunk c + 1, so the hand-over from strip to strip costs
-// the neighbour's first TWO chunks -- and chunk 0, where the lanes enter one by one, ran the general step at half speed:
-// 18 + 9 us per strip, inherited by every strip to the right.  The LAT instantiation runs one unrolled step on every
-// chunk: rows outside [0, n) are computed on zero-filled data and discarded by selects, the staircase bookkeeping is
-// always on.  Same cells, same operations, same order of the value additions: bitwise the results of the other kernel.
-// It holds no other unrolled variant (the general step remains for bands and m < W), so it is the smaller binary.
-template <int D, bool CKPT, int FW, bool LAT>
+template <int D, bool CKPT, int FW>
 __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kernel(const Params p) {
     extern __shared__ __align__(16) float smem[];
     __shared__ RollCtl ctl;
@@ -488,37 +477,7 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
             if (lane == 0) { const float2 qv = vin_s[t]; va = qv.x; vb = qv.y; }
             XRow<D> xa, xb;
             load_x2<D>(xs_lane, 2 * t, xa, xb);
-            if constexpr (std::is_same<decltype(tag), LatTag>::value) {
-                const int i0 = RP * (c * CH + t - lane);
-                const bool actA = (unsigned)i0 < (unsigned)n, actB = (unsigned)(i0 + 1) < (unsigned)n;
-                float hA[W], hB[W], dummy0, dummy1;
-#pragma unroll
-                for (int w = 0; w < W; ++w) {
-                    float tl, acc;
-                    hA[w] = h[w];
-                    sqdist2<D>(xa, z[w], tl, acc);
-                    cell<false, (D > 1)>(tl, acc, hA[w], va, dummy0, dummy1, D <= 2 && ((SDTW_POLY_MASK_A >> w) & 1));
-                    hB[w] = hA[w];
-                    sqdist2<D>(xb, z[w], tl, acc);
-                    cell<false, (D > 1)>(tl, acc, hB[w], vb, dummy0, dummy1, D <= 2 && ((SDTW_POLY_MASK_B >> w) & 1));
-                }
-                // the value staircase: the additions of the general row, in its order (rows outside [0, n) match no window)
-                if ((unsigned)(i0 - r_v0 - 1) < (unsigned)(r_v1 - r_v0)) vacc += va;
-                if (i0 == r_h) {
-#pragma unroll
-                    for (int w = 0; w < W; ++w) if (j0 + w >= jlo && j0 + w <= jhi) hsum += hA[w];
-                }
-                if (T == 0 && i0 == 0) hsum += sqdist<D>(xa, z[0]);   // r_11 = D_11
-                if ((unsigned)(i0 - r_v0) < (unsigned)(r_v1 - r_v0)) vacc += vb;
-                if (i0 + 1 == r_h) {
-#pragma unroll
-                    for (int w = 0; w < W; ++w) if (j0 + w >= jlo && j0 + w <= jhi) hsum += hB[w];
-                }
-#pragma unroll
-                for (int w = 0; w < W; ++w) h[w] = actB ? hB[w] : (actA ? hA[w] : h[w]);
-                vp0 = actA ? va : vp0;
-                vp1 = actB ? vb : vp1;
-            } else if constexpr (!slow) {
+            if constexpr (!slow) {
                 constexpr bool val = decltype(tag)::val;
                 const int i0 = RP * (c * CH + t - lane);   // used by the staircase bookkeeping only
                 float dummy0, dummy1;
@@ -578,47 +537,6 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
                 vbad = (r < n && is_sentinel(vreg.x)) || (r + 1 < n && is_sentinel(vreg.y));
             }
         };
-        // LAT, no band, m >= W: the boundary values are exchanged per BLOCK of TR steps instead of per chunk.  Lane 31 reaches
-        // rows 2 s' - 62 at its step s', so the right strip's block k needs this strip's block k + 4: it runs 5 blocks (40
-        // steps) behind instead of two chunks (64 steps), and the chain of a pair shortens accordingly.
-        bool fine = false;
-        if constexpr (LAT) fine = (band < 0 && Tfull > 0);
-        if (fine) {
-            float2 breg = make_float2(0.f, 0.f);           // lanes < TR: boundary values of the next block's steps
-            bool bbad = false;
-            auto load_blk = [&](const int blk) {           // blk = c (CH / TR) + b; lane u < TR: rows of step blk TR + u
-                const int r = RP * (blk * TR + (lane & (TR - 1)));
-                breg = ld_relaxed_f2(VSprev + r);
-                bbad = lane < TR && ((r < n && is_sentinel(breg.x)) || (r + 1 < n && is_sentinel(breg.y)));
-            };
-            if (J > 0) load_blk(0);
-            for (int c = 0; c <= cl; ++c) {
-                cp_async_wait_all();
-                __syncwarp();
-                if (c + 1 <= cl) stage_x_async<D>(xs0 + ((c + 1) & 1) * XWIN * D, p.Xs, pm.x_off, n, c + 1, lane);
-                xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;
-#pragma unroll 1
-                for (int b = 0; b < CH / TR; ++b) {
-                    const int blk = c * (CH / TR) + b;
-                    if (J > 0) {
-                        while (__any_sync(FULL, bbad)) {
-                            if (bbad) load_blk(blk);
-                        }
-                    } else {
-                        breg = make_float2((blk == 0 && lane == 0) ? BIG : 0.f, 0.f);
-                    }
-                    if (lane < TR) vin_s[b * TR + lane] = breg;
-                    __syncwarp();
-                    if (J > 0 && blk + 1 < (cl + 1) * (CH / TR)) load_blk(blk + 1);
-#pragma unroll
-                    for (int u = 0; u < TR; ++u) step(c, b * TR + u, LatTag{});
-                    if (CKPT) checkpoint(blk + 1);
-                    __syncwarp();
-                    // lane 31 worked on rows c CROWS - SKEW + 2t (+1) at step t
-                    if (lane < TR) st_relaxed_f2(VSme + c * CROWS - SKEW + 2 * (b * TR + lane), vout_s[b * TR + lane]);
-                }
-            }
-        } else {
         if (J > 0) load_in(cf);
         unsigned cons_seen = 0;                            // my consumer's progress as last read (rings)
 
@@ -646,22 +564,6 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
             }
             xs_lane = xs0 + (c & 1) * XWIN * D + (XPAD - 2 * lane) * D;    // rows of step t: xs_lane[2t], [2t+1]
             const bool inside = interior_chunk(c, n) && band_clear(c, J, band);
-            if constexpr (LAT) {
-                if (band < 0 && Tfull > 0) {
-#pragma unroll 1
-                    for (int b = 0; b < CH / TR; ++b) {
-#pragma unroll
-                        for (int u = 0; u < TR; ++u) step(c, b * TR + u, LatTag{});
-                        if (CKPT) checkpoint(c * (CH / TR) + b + 1);
-                    }
-                } else {
-#pragma unroll 1
-                    for (int t = 0; t < CH; ++t) {
-                        step(c, t, SlowTag{});
-                        if (CKPT && ((t + 1) & (TR - 1)) == 0) checkpoint((c * CH + t + 1) / TR);
-                    }
-                }
-            } else
             if (inside && (c < c_v0 || c > c_v1)) {
 #pragma unroll 1
                 for (int b = 0; b < CH / TR; ++b) {
@@ -708,7 +610,6 @@ __global__ void __launch_bounds__(FW * 32, (D >= 3 ? 1 : 32 / FW)) forward_kerne
                 if (lane < CH) st_relaxed_f2(VSme + c * CROWS - SKEW + 2 * lane, vout_s[lane]);
             }
         }
-        }   // !fine
         if (in_ring) in_q += (unsigned)(C * CH);
         if (out_ring) out_q += (unsigned)(C * CH);
         if (cl < C - 1) {
