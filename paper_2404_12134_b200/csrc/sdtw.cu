@@ -72,7 +72,7 @@ struct Layout {
     int ring_units = 0;         // forward-only ring mode: strips per unit (0: one full boundary column per strip)
     int ring_ctas = 0;          // CTAs the ring buffers are sized for
     size_t off_ring = 0, off_ring_prog = 0;
-    size_t off_counters = 0, off_prog_b = 0, off_hint_b = 0, off_VP = 0, off_Xs = 0, off_Zs = 0, off_VS = 0, off_ES = 0, off_CK = 0,
+    size_t off_counters = 0, off_prog_b = 0, off_hint_b = 0, off_ready_b = 0, off_VP = 0, off_Xs = 0, off_Zs = 0, off_VS = 0, off_ES = 0, off_CK = 0,
            off_Gk = 0, off_G = 0, off_Zt = 0, off_Vt = 0, off_scal = 0;   // last four: line-search scratch
     size_t sync_bytes = 0;      // counters + stats + prog_b: cleared before every evaluation
     size_t vs_bytes = 0;        // VS: preset to the sentinel pattern before every evaluation
@@ -135,6 +135,7 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
     L.off_stats = o;    o += 128;
     L.off_prog_b = o;   o += align_up((size_t)L.items * 4, 256);
     L.off_hint_b = o;   o += align_up((size_t)L.items * 4, 256);
+    L.off_ready_b = o;  o += want_grad ? align_up((size_t)L.items * 4, 256) : 0;
     if (L.ring_units) {         // zeroed with the counters: a ring entry is valid when its tag (>= 1) is the expected one
         L.off_ring = o;      o += (size_t)L.ring_ctas * L.ring_units * RING_ENTRIES * 16 * vs_words;
         L.off_ring_prog = o; o += align_up((size_t)L.ring_ctas * L.ring_units * 4, 256);
@@ -436,6 +437,7 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     P.counters = reinterpret_cast<unsigned*>(ws + L.off_counters);
     P.prog_b = reinterpret_cast<unsigned*>(ws + L.off_prog_b);
     P.hint_b = reinterpret_cast<unsigned*>(ws + L.off_hint_b);
+    P.ready_b = reinterpret_cast<unsigned*>(ws + L.off_ready_b);
     P.ring = L.ring_units ? reinterpret_cast<unsigned long long*>(ws + L.off_ring) : nullptr;
     P.ring_prog = L.ring_units ? reinterpret_cast<unsigned*>(ws + L.off_ring_prog) : nullptr;
     P.VP = reinterpret_cast<double*>(ws + L.off_VP);

@@ -82,9 +82,10 @@ struct Params {
     const float* Zs;      // sqrt(kappa) * Z
     const float* Xs;      // sqrt(kappa) * X_concat
     const PairMeta* pm;
-    unsigned* counters;   // [0] forward work queue, [1] reverse work queue
+    unsigned* counters;   // [0] forward work queue, [1] reverse work queue (head), [2] tail of ready_b
     unsigned* prog_b;     // [N * NS] progress word of each reverse item: FIN | z when it is done
     unsigned* hint_b;     // [N * NS] 1 + the first chunk the reverse item visited (0: none yet)
+    unsigned* ready_b;    // [N * NS] reverse_kernel's work queue behind the first N entries: 1 + item, in order of readiness
     float* VS;            // strip-boundary v columns, indexed by row
     float* ES;            // strip-boundary E messages, indexed by row
     float* CK;            // checkpoints

@@ -101,18 +101,27 @@ __global__ void __launch_bounds__(RW * 32) reverse_kernel(const Params p) {
     unsigned n_ann = 0;        // announcements seen (warps 1..) or made (warp 0)
 
     for (;;) {
+        // Work queue in order of READINESS: the first N entries are the right-most strips of the pairs; every other strip is
+        // appended by its right neighbour when that one announces its first visited chunk (or its end), which is when
+        // the strip's hint exists.  So a CTA never sits on a strip that cannot start yet: with three CTAs per SM there
+        // are only 4.4 strips in flight per pair on cfg 4, and a pair's chain needs about 3.5 of them working.
         if (threadIdx.x == 0) {
             const unsigned q = atomicAdd(p.counters + 1, 1u);
-            ctl.item = q < p.num_items ? (int)q : -1;
+            int it = -1;
+            if (q < (unsigned)p.N) it = (int)q * p.NS + p.NS - 1;
+            else if (q < p.num_items) {
+                unsigned v;
+                while ((v = ld_relaxed_u32(p.ready_b + (q - p.N))) == 0u) __nanosleep(64);
+                it = (int)v - 1;
+            }
+            ctl.item = it;
         }
         __syncthreads();
-        const int q = ctl.item;
-        if (q < 0) break;
-        const int Jr = q / p.N, ps = q - Jr * p.N;
-        const int J = p.NS - 1 - Jr;                          // right-most strip first
+        const int item = ctl.item;
+        if (item < 0) break;
+        const int ps = item / p.NS, J = item - ps * p.NS;
         const PairMeta pm = p.pm[ps];
         const int n = pm.n, C = pm.C;
-        const int item = ps * p.NS + J;
         const int j0 = (J * 32 + lane) * W;
         const bool has_right = (J < p.NS - 1);
         const int band = p.band;
@@ -335,11 +344,15 @@ __global__ void __launch_bounds__(RW * 32) reverse_kernel(const Params p) {
         auto announce = [&](const int c) {
             if (lane == 0) {
                 ctl.ann[n_ann & 3] = c;
-                // first visited chunk of this strip: the left strip's input is +0 in every chunk with a larger index
-                if (c >= 0 && !hinted && J > 0) st_relaxed_u32(p.hint_b + item, (unsigned)c + 1u);
                 mbar_arrive(&ctl.ann_bar);
+                if (!hinted && J > 0) {
+                    // first visited chunk of this strip: the left strip's input is +0 in every chunk with a larger index;
+                    // the left strip can start now (or, if this strip ends without a visit, has nothing to do): queue it
+                    if (c >= 0) st_relaxed_u32(p.hint_b + item, (unsigned)c + 1u);
+                    st_relaxed_u32(p.ready_b + atomicAdd(p.counters + 2, 1u), (unsigned)item);   // item - 1, stored + 1
+                }
             }
-            if (c >= 0) hinted = true;
+            hinted = true;
             c_ann = c;
             ++n_ann;
         };
