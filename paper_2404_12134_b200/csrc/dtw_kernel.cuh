@@ -28,6 +28,14 @@ namespace sdtw {
 // exists at d <= 2 only (the kernel fits 64 registers there)
 constexpr int DTW_WARPS = 8;
 constexpr int DTW_RING_WARPS = 32;
+#ifndef SDTW_DTW_RING_CHUNKS
+#define SDTW_DTW_RING_CHUNKS 8
+#endif
+// ring of the DTW kernels: 32 bytes per entry, so half as many chunks as the Soft-DTW ring keep the rings of all resident
+// warps (148 x 32 x 8 KB = 39 MB) inside the L2 (with 16 chunks the ring traffic, 96 GB on cfg 5, went through HBM)
+constexpr int DTW_RING_CHUNKS = SDTW_DTW_RING_CHUNKS;
+constexpr int DTW_RING_ENTRIES = DTW_RING_CHUNKS * CH;
+static_assert((DTW_RING_ENTRIES & (DTW_RING_ENTRIES - 1)) == 0, "ring size is a power of two");
 #ifndef SDTW_DTW_W
 #define SDTW_DTW_W 4
 #endif
@@ -136,7 +144,7 @@ __global__ void __launch_bounds__(FW * 32) dtw_kernel(const DtwParams p) {
         const long long col = rings ? (out_ring ? 0 : g) : J;
         unsigned* VSme = p.VS + pm.vs_off + col * pm.vs_stride + 2 * VS_PAD;   // word 2 row
         const unsigned* VSprev = rings ? p.VS + pm.vs_off + (long long)(g - 1) * pm.vs_stride + 2 * VS_PAD : VSme - pm.vs_stride;
-        auto ring_of = [&](const int q) { return p.ring + ((size_t)blockIdx.x * FW + q) * (RING_ENTRIES * 4); };
+        auto ring_of = [&](const int q) { return p.ring + ((size_t)blockIdx.x * FW + q) * (DTW_RING_ENTRIES * 4); };
         auto prog_of = [&](const int q) { return p.ring_prog + (size_t)blockIdx.x * FW + q; };
 
         float z[W][D], ru[W], lu[W];
@@ -201,11 +209,11 @@ __global__ void __launch_bounds__(FW * 32) dtw_kernel(const DtwParams p) {
             const int rb = c * CROWS + 2 * vlane;
             if (in_ring) {
                 const unsigned e = in_q + (unsigned)(c * CH + vlane);
-                const unsigned long long* q = ring_of((mypos + FW - 1) % FW) + (size_t)(e & (RING_ENTRIES - 1)) * 4;
+                const unsigned long long* q = ring_of((mypos + FW - 1) % FW) + (size_t)(e & (DTW_RING_ENTRIES - 1)) * 4;
                 unsigned long long a0, a1, a2, a3;
                 ld_relaxed_v2u64(q, a0, a1);
                 ld_relaxed_v2u64(q + 2, a2, a3);
-                const unsigned tag = e / RING_ENTRIES + 1u;
+                const unsigned tag = e / DTW_RING_ENTRIES + 1u;
                 vreg = make_uint4((unsigned)a0, (unsigned)a1, (unsigned)a2, (unsigned)a3);
                 vbad = (rb < n && ((unsigned)(a0 >> 32) != tag || (unsigned)(a1 >> 32) != tag)) ||
                        (rb + 1 < n && ((unsigned)(a2 >> 32) != tag || (unsigned)(a3 >> 32) != tag));
@@ -247,7 +255,7 @@ __global__ void __launch_bounds__(FW * 32) dtw_kernel(const DtwParams p) {
             if (out_ring) {
                 // the highest entry of this chunk reuses the slot of the entry RING_ENTRIES below it (of this strip or of the
                 // strip before): my consumer must have taken it
-                const unsigned need = out_q + (unsigned)((c - RING_CHUNKS + 1) * CH);
+                const unsigned need = out_q + (unsigned)((c - DTW_RING_CHUNKS + 1) * CH);
                 unsigned seen = __shfl_sync(FULL, cons_seen, 0);
                 while ((int)(seen - need) < 0) {
                     __nanosleep(64);
@@ -257,9 +265,9 @@ __global__ void __launch_bounds__(FW * 32) dtw_kernel(const DtwParams p) {
                 const int q = c * CH - (SKEW / 2) + lane;               // r / 2 for r = c CROWS - SKEW + 2 lane
                 if (lane < CH && q >= 0) {
                     const unsigned e = out_q + (unsigned)q;
-                    const unsigned long long tag = (unsigned long long)(e / RING_ENTRIES + 1u) << 32;
+                    const unsigned long long tag = (unsigned long long)(e / DTW_RING_ENTRIES + 1u) << 32;
                     const uint4 vo = vout_s[lane];
-                    unsigned long long* dst = ring_of(mypos) + (size_t)(e & (RING_ENTRIES - 1)) * 4;
+                    unsigned long long* dst = ring_of(mypos) + (size_t)(e & (DTW_RING_ENTRIES - 1)) * 4;
                     st_relaxed_v2u64(dst, tag | vo.x, tag | vo.y);
                     st_relaxed_v2u64(dst + 2, tag | vo.z, tag | vo.w);
                 }

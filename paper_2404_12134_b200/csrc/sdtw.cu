@@ -137,7 +137,7 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
     L.off_hint_b = o;   o += align_up((size_t)L.items * 4, 256);
     L.off_ready_b = o;  o += want_grad ? align_up((size_t)L.items * 4, 256) : 0;
     if (L.ring_units) {         // zeroed with the counters: a ring entry is valid when its tag (>= 1) is the expected one
-        L.off_ring = o;      o += (size_t)L.ring_ctas * L.ring_units * RING_ENTRIES * 16 * vs_words;
+        L.off_ring = o;      o += (size_t)L.ring_ctas * L.ring_units * (vs_words == 2 ? DTW_RING_ENTRIES * 32 : RING_ENTRIES * 16);
         L.off_ring_prog = o; o += align_up((size_t)L.ring_ctas * L.ring_units * 4, 256);
     }
     L.sync_bytes = o;
