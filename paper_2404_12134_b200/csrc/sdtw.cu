@@ -466,11 +466,11 @@ int evaluate(const Plan& pl, char* ws, const DeviceInfo& di, const float* Z, con
     int rc = SDTW_OK;
     if (phase & 1) {
     {
-        // one launch: counters / progress words / rings := 0, strip-boundary columns VS (and ES: same protocol in reverse)
-        // := the sentinel pattern the consumers poll for (sdtw_kernels.cuh), scaled copies of the inputs
+        // one launch: counters / progress words / rings := 0, strip-boundary columns VS := the sentinel pattern the
+        // consumers poll for (sdtw_kernels.cuh), scaled copies of the inputs
         const FillJob f0{reinterpret_cast<uint4*>(ws + L.off_counters), L.sync_bytes / 16, 0u};
         const FillJob f1{reinterpret_cast<uint4*>(ws + L.off_VS), L.vs_bytes / 16, SENTINEL};
-        const FillJob f2{reinterpret_cast<uint4*>(ws + (pl.want_grad ? L.off_ES : L.off_VS)), pl.want_grad ? L.vs_bytes / 16 : 0, SENTINEL};
+        const FillJob f2{reinterpret_cast<uint4*>(ws + L.off_VS), 0, SENTINEL};   // (ES is preset by the forward kernel, strip by strip)
         const long long nx = (long long)pl.offsets[pl.N] * pl.d, nz = (long long)pl.m * pl.d;
         const unsigned long long work = (unsigned long long)(nx + nz) + f0.count16 + f1.count16 + f2.count16;
         const int blocks = (int)std::min<unsigned long long>((work + 255) / 256, (unsigned long long)di.sms * 16);
