@@ -21,8 +21,10 @@
 //   reverse  ES[row]: E messages from the right strip to the left one, same protocol (sentinel preset, relaxed data-word
 //            polling one chunk ahead); only the END of an item is published with a release (its progress word).
 // Every TR steps the forward kernel checkpoints the warp state (h[W] + the two values in flight) to HBM; the reverse
-// kernel restores a checkpoint, recomputes TR steps keeping the transition weights in shared memory, then runs the E
-// recurrence over those TR steps backwards, accumulating the gradient contraction of eq. 6 in registers.
+// kernels restore a checkpoint, recompute TR steps keeping the transition weights in shared memory, then run the E
+// recurrence over those TR steps backwards, accumulating the gradient contraction of eq. 6 in registers.  This file
+// holds the throughput-regime reverse kernel (backward_kernel: one warp per strip); sdtw_reverse.cuh holds the
+// latency-regime one (reverse_kernel: a CTA of four warps per strip).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
