@@ -583,6 +583,41 @@ def test_band_dense_reverse_and_schedule_are_bitwise_neutral(B):
         assert torch.isfinite(g0).all()
 
 
+def test_small_problem_graph_replay_is_bitwise_the_plain_launches(B):
+    """Calls on small problems are captured into a CUDA graph the second time the same call (same buffers, same scalars)
+    comes back, and replayed from then on.  First call = plain launches, second = capture + launch, third
+    and fourth = replay: same bits every time, the launch counter advances by the same amount, other arguments (another
+    step, another iteration count) get their own graph and their own results."""
+    import torch
+    for idx in (1, 2):
+        data = synth.make(idx)
+        cfg = data["cfg"]
+        Z0, X = _dev(data["Z0"]), _dev(data["X"])
+        Z = Z0.clone()
+        vals = torch.empty(cfg.N, dtype=torch.float32, device=Z.device)
+        obj = torch.empty(cfg.iters, dtype=torch.float32, device=Z.device)
+        G = torch.empty_like(Z0)
+        ref, counts = None, []
+        for rep in range(4):
+            Z.copy_(Z0)
+            n0 = B.sdtw_launch_count()
+            B.sdtw_barycenter(Z, X, data["offsets"], cfg.gamma, cfg.iters, cfg.step, out_values=vals, out_objective=obj)
+            B.sdtw_value_grad(Z0, X, data["offsets"], cfg.gamma, out_values=vals, out_grad=G)
+            torch.cuda.synchronize()
+            counts.append(B.sdtw_launch_count() - n0)
+            cur = (Z.clone(), obj.clone(), vals.clone(), G.clone())
+            if ref is None:
+                ref = cur
+            assert all(torch.equal(a, b) for a, b in zip(ref, cur)), (idx, rep)
+        assert len(set(counts)) == 1 and counts[0] == 4 * (cfg.iters + 1), counts
+        Z.copy_(Z0)
+        B.sdtw_barycenter(Z, X, data["offsets"], cfg.gamma, 2, 0.5 * cfg.step, out_values=vals, out_objective=obj)
+        Z.copy_(Z0)
+        B.sdtw_barycenter(Z, X, data["offsets"], cfg.gamma, 2, 0.5 * cfg.step, out_values=vals, out_objective=obj)
+        torch.cuda.synchronize()
+        assert not torch.equal(Z, ref[0]) and torch.isfinite(Z).all()
+
+
 @pytest.mark.parametrize("kernel", [0, 1])
 def test_both_reverse_kernels_against_the_oracle(B, oracle, kernel):
     """The reverse pass has a latency-regime and a throughput-regime kernel (include/sdtw_debug.h,
