@@ -165,13 +165,18 @@ int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_co
                          float gamma, int32_t iters, float step, float* out_values, float* out_objective, void* stream);
 
 /*
- * Workspace.  sdtw_workspace_bytes() is what one call needs (tile-boundary strips, checkpoints of the forward state,
- * per-pair gradient partials).  If a workspace has been registered with sdtw_set_workspace() it is used (it must be
- * large enough, else SDTW_ERR_WORKSPACE); otherwise the library keeps one grow-only device buffer per GPU
+ * Workspace.  sdtw_workspace_bytes() is what one call needs to evaluate all its pairs at once (tile-boundary strips,
+ * checkpoints of the forward state: 0.375 bytes per DP cell, per-pair gradient partials).  If a workspace has been
+ * registered with sdtw_set_workspace() it is used; otherwise the library keeps one grow-only device buffer per GPU
  * (cudaMalloc on first use / when a larger problem arrives -- that call blocks the host while allocating).  Calls
  * that share the buffer from different streams are ordered on it with an event, so they are safe but not concurrent.
  * sdtw_set_workspace(NULL, 0) unregisters the caller's buffer and frees the library-owned one of the current device.
  * The pointer must be 256-byte aligned.  sdtw_workspace_bytes returns 0 on invalid arguments.
+ * WAVES.  When that size exceeds the budget -- sdtw_set_workspace_limit(bytes) if set (0 = unset), else the registered
+ * workspace, else what the device has free -- sdtw_value_grad[_ex] and sdtw_barycenter[_ex] evaluate the pair set as
+ * consecutive waves of pairs in the same workspace (pairs are independent): per-pair values are bitwise
+ * the same, the gradients of the waves are added in wave order (float32 round-off against the unsplit call).  Only when
+ * a single pair does not fit the budget: SDTW_ERR_WORKSPACE.  (sdtw_barycenter_backtracking and the DTW calls do not split.)
  * Forward-only calls (want_grad == 0) without a band keep O(chunks) boundary state per resident strip plus one
  * boundary column per unit of strips; a forward-only call WITH a band that excludes cells keeps a
  * full boundary column per strip: size its workspace with sdtw_workspace_bytes_ex(..., band).  The forward-only size
@@ -182,6 +187,7 @@ size_t sdtw_workspace_bytes_ex(int64_t m, int32_t d, const int64_t* offsets, int
 /* What one sdtw_dtw_score / sdtw_subdtw call of this shape needs (d <= SDTW_DTW_MAX_D); 0 on invalid arguments. */
 size_t sdtw_dtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, int32_t N);
 int sdtw_set_workspace(void* dev_ptr, size_t bytes);
+int sdtw_set_workspace_limit(size_t bytes);
 
 /* Static description of a status code; the cudaError_t behind the last SDTW_ERR_CUDA on this thread. */
 const char* sdtw_status_string(int status);

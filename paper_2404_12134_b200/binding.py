@@ -36,6 +36,7 @@ SYMBOLS = {
     "sdtw_workspace_bytes_ex": (ctypes.c_size_t, [_i64, _i32, _i64p, _i32, ctypes.c_int, _i64]),
     "sdtw_dtw_workspace_bytes": (ctypes.c_size_t, [_i64, _i32, _i64p, _i32]),
     "sdtw_set_workspace": (ctypes.c_int, [_vp, ctypes.c_size_t]),
+    "sdtw_set_workspace_limit": (ctypes.c_int, [ctypes.c_size_t]),
     "sdtw_status_string": (ctypes.c_char_p, [ctypes.c_int]),
     "sdtw_last_cuda_error": (ctypes.c_int, []),
     "sdtw_launch_count": (ctypes.c_uint64, []),
@@ -354,6 +355,11 @@ def sdtw_set_workspace(tensor_or_none):
     else:
         t = tensor_or_none
         _check(_lib.sdtw_set_workspace(ctypes.c_void_p(t.data_ptr()), t.numel() * t.element_size()))
+
+
+def sdtw_set_workspace_limit(nbytes: int = 0):
+    """Workspace budget of the calls that follow (0 = unset): beyond it the pair set is evaluated in waves (sdtw.h)."""
+    _check(_lib.sdtw_set_workspace_limit(int(nbytes)))
 
 
 def sdtw_launch_count() -> int:

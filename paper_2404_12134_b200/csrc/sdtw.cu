@@ -23,6 +23,7 @@ std::mutex g_mutex;
 uint64_t g_launches = 0;
 struct UserWs { void* ptr = nullptr; size_t bytes = 0; };
 UserWs g_user_ws[64];         // caller-registered workspace, one per device (sdtw_set_workspace)
+size_t g_ws_limit = 0;        // sdtw_set_workspace_limit: 0 = what the device has free
 // instrumentation / tuning switches of include/sdtw_debug.h: per calling thread, so that one thread's measurement
 // settings never change another thread's launch
 thread_local bool g_profile = false;
@@ -254,7 +255,7 @@ int get_plan(const DeviceInfo& di, int64_t m, int32_t d, const int64_t* offsets,
         return SDTW_ERR_CUDA;
     }
     pl->stamp = ++g_stamp;
-    if (g_plans.size() >= 8) {   // evict the least recently used plan
+    if (g_plans.size() >= 32) {   // evict the least recently used plan
         auto it = std::min_element(g_plans.begin(), g_plans.end(), [](Plan* a, Plan* b) { return a->stamp < b->stamp; });
         cudaFree((*it)->d_pm);
         if ((*it)->d_w) cudaFree((*it)->d_w);
@@ -631,6 +632,101 @@ int run_graphed(Plan& pl, const GraphKey& key, cudaStream_t stream, F enqueue) {
     return SDTW_OK;
 }
 
+// ---- waves: a call whose workspace would not fit is evaluated as consecutive sub-batches of pairs ------------------
+// Pairs are independent, so the pair set can be cut into WAVES [b_w, b_{w+1}) of consecutive pairs, each
+// evaluated by itself in the same workspace; values land in their slots, the gradients of the waves are added in wave
+// order (the sum over pairs is then grouped by wave: a difference of float32 round-off against the unsplit call).
+// The budget: sdtw_set_workspace_limit, else the registered workspace, else what the device has free.
+__global__ void add_inplace_kernel(float* __restrict__ acc, const float* __restrict__ x, long long count) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < count) acc[e] += x[e];
+}
+__global__ void sum_objective_kernel(const double* __restrict__ parts, int W, float* __restrict__ out) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < W; ++w) s += parts[w];
+        *out = (float)s;
+    }
+}
+
+size_t workspace_budget(int dev, size_t need) {
+    if (g_ws_limit) return g_ws_limit;
+    if (g_user_ws[dev].ptr) return g_user_ws[dev].bytes;
+    if (g_ws_cache[dev].bytes >= need) return need;
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); return need; }
+    const size_t avail = free_b + g_ws_cache[dev].bytes;        // the grow-only buffer is freed before it is regrown
+    return need <= avail - avail / 16 ? need : avail - avail / 8;
+}
+
+// bounds of the waves (bounds[0] = 0 < ... < bounds[W] = N) such that every wave's layout fits `budget`; *max_bytes =
+// the largest of them.  SDTW_ERR_WORKSPACE if a single pair does not fit.
+int plan_waves(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, int ring_sms, size_t budget,
+               std::vector<int>& bounds, size_t* max_bytes) {
+    std::vector<int64_t> sub;
+    std::vector<int> candidates;                    // wave counts tried: 1 .. 8, then growing by a quarter, at last N
+    for (int W = 1; W < N; W = (W < 8 ? W + 1 : W + W / 4)) candidates.push_back(W);
+    candidates.push_back(N);
+    for (const int W : candidates) {
+        bounds.clear();
+        for (int w = 0; w <= W; ++w) bounds.push_back((int)((long long)w * N / W));
+        size_t mx = 0;
+        bool ok = true;
+        for (int w = 0; w < W && ok; ++w) {
+            const int k0 = bounds[w], k1 = bounds[w + 1];
+            sub.assign(offsets + k0, offsets + k1 + 1);
+            for (auto& o : sub) o -= offsets[k0];
+            Layout L;
+            const int rc = build_layout(m, d, sub.data(), k1 - k0, want_grad, L, 1, ring_sms);
+            if (rc != SDTW_OK) return rc;
+            mx = std::max(mx, L.total);
+            ok = L.total <= budget;
+        }
+        if (ok) { *max_bytes = mx; return SDTW_OK; }
+    }
+    return SDTW_ERR_WORKSPACE;
+}
+
+// one evaluation over waves.  G (m d floats) receives the summed gradient when want_grad; Gtmp is scratch of the same size;
+// obj64 (W doubles) scratch for the objective.  out_objective may be null.
+int evaluate_waves(const DeviceInfo& di, const std::vector<int>& bounds, char* ws, const float* Z, int64_t m, int32_t d,
+                   const float* X, const int64_t* offsets, const float* weights, float gamma, int band_eff, bool ring_ok,
+                   float* out_values, float* out_objective, float* G, float* Gtmp, double* obj64, cudaStream_t stream) {
+    const int W = (int)bounds.size() - 1;
+    const long long md = (long long)m * d;
+    std::vector<int64_t> sub;
+    for (int w = 0; w < W; ++w) {
+        const int k0 = bounds[w], k1 = bounds[w + 1];
+        sub.assign(offsets + k0, offsets + k1 + 1);
+        for (auto& o : sub) o -= offsets[k0];
+        Plan* pl = nullptr;
+        int rc = get_plan(di, m, d, sub.data(), k1 - k0, weights ? weights + k0 : nullptr, G != nullptr, stream, &pl, 1, ring_ok);
+        if (rc) return rc;
+        float* Gw = (w == 0) ? G : Gtmp;
+        rc = evaluate(*pl, ws, di, Z, X + offsets[k0] * d, gamma, band_eff, out_values ? out_values + k0 : nullptr, nullptr, Gw,
+                      nullptr, 0.f, stream, 3, obj64 + w);
+        if (rc) return rc;
+        if (w > 0 && G) {
+            add_inplace_kernel<<<(int)((md + 255) / 256), 256, 0, stream>>>(G, Gtmp, md);
+            ++g_launches;
+            CUDA_TRY(cudaGetLastError());
+        }
+    }
+    if (out_objective) {
+        sum_objective_kernel<<<1, 32, 0, stream>>>(obj64, W, out_objective);
+        ++g_launches;
+        CUDA_TRY(cudaGetLastError());
+    }
+    return SDTW_OK;
+}
+
+struct DevBuf {
+    void* p = nullptr;
+    cudaStream_t s = nullptr;
+    int alloc(size_t bytes, cudaStream_t st) { s = st; CUDA_TRY(cudaMallocAsync(&p, bytes, st)); return SDTW_OK; }
+    ~DevBuf() { if (p) cudaFreeAsync(p, s); }
+};
+
 }  // namespace
 
 // =================================================================================================================
@@ -649,8 +745,29 @@ int sdtw_value_grad_ex(const float* Z, int64_t m, int32_t d, const float* X_conc
     DeviceInfo di;
     rc = get_device(di);
     if (rc) return rc;
+    const bool ring_ok = out_grad == nullptr && band_eff < 0 && g_forward_rings;
+    {   // does the workspace of the whole pair set fit?  If not: waves of pairs
+        Layout L;
+        rc = build_layout(m, d, offsets, N, out_grad != nullptr, L, 1, ring_ok ? di.sms : 0);
+        if (rc) return rc;
+        const size_t budget = workspace_budget(di.dev, L.total);
+        if (L.total > budget) {
+            std::vector<int> bounds;
+            size_t max_bytes = 0;
+            rc = plan_waves(m, d, offsets, N, out_grad != nullptr, ring_ok ? di.sms : 0, budget, bounds, &max_bytes);
+            if (rc) return rc;
+            Workspace ws;
+            rc = ws.acquire(max_bytes, di.dev, stream);
+            if (rc) return rc;
+            DevBuf Gtmp, obj64;
+            if (out_grad && (rc = Gtmp.alloc((size_t)m * d * 4, stream))) return rc;
+            if ((rc = obj64.alloc(sizeof(double) * (bounds.size() - 1), stream))) return rc;
+            return evaluate_waves(di, bounds, ws.ptr, Z, m, d, X_concat, offsets, weights, gamma, band_eff, ring_ok, out_values,
+                                  out_objective, out_grad, (float*)Gtmp.p, (double*)obj64.p, stream);
+        }
+    }
     Plan* pl = nullptr;
-    rc = get_plan(di, m, d, offsets, N, weights, out_grad != nullptr, stream, &pl, 1, out_grad == nullptr && band_eff < 0 && g_forward_rings);
+    rc = get_plan(di, m, d, offsets, N, weights, out_grad != nullptr, stream, &pl, 1, ring_ok);
     if (rc) return rc;
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
@@ -686,6 +803,36 @@ int sdtw_barycenter_ex(float* Z_inout, int64_t m, int32_t d, const float* X_conc
     rc = get_device(di);
     if (rc) return rc;
     if (iters == 0) return SDTW_OK;
+    {   // waves of pairs when the workspace of the whole pair set does not fit (see evaluate_waves)
+        Layout L;
+        rc = build_layout(m, d, offsets, N, true, L);
+        if (rc) return rc;
+        const size_t budget = workspace_budget(di.dev, L.total);
+        if (L.total > budget) {
+            std::vector<int> bounds;
+            size_t max_bytes = 0;
+            rc = plan_waves(m, d, offsets, N, true, 0, budget, bounds, &max_bytes);
+            if (rc) return rc;
+            Workspace ws;
+            rc = ws.acquire(max_bytes, di.dev, stream);
+            if (rc) return rc;
+            DevBuf G, Gtmp, obj64;
+            const long long md = (long long)m * d;
+            if ((rc = G.alloc((size_t)md * 4, stream)) || (rc = Gtmp.alloc((size_t)md * 4, stream)) ||
+                (rc = obj64.alloc(sizeof(double) * (bounds.size() - 1), stream)))
+                return rc;
+            for (int it = 0; it < iters; ++it) {
+                rc = evaluate_waves(di, bounds, ws.ptr, Z_inout, m, d, X_concat, offsets, weights, gamma, band_eff, false,
+                                    it == iters - 1 ? out_values : nullptr, out_objective ? out_objective + it : nullptr,
+                                    (float*)G.p, (float*)Gtmp.p, (double*)obj64.p, stream);
+                if (rc) return rc;
+                gd_update_kernel<<<(int)((md + 255) / 256), 256, 0, stream>>>(Z_inout, (const float*)G.p, md, step);
+                ++g_launches;
+                CUDA_TRY(cudaGetLastError());
+            }
+            return SDTW_OK;
+        }
+    }
     Plan* pl = nullptr;
     rc = get_plan(di, m, d, offsets, N, weights, true, stream, &pl);
     if (rc) return rc;
@@ -858,14 +1005,6 @@ int sdtw_gd_update(float* Z_inout, const float* G, int64_t count, float step, vo
 }
 
 // ---- host-buffer variants ---------------------------------------------------------------------------------------
-namespace {
-struct DevBuf {
-    void* p = nullptr;
-    cudaStream_t s = nullptr;
-    int alloc(size_t bytes, cudaStream_t st) { s = st; CUDA_TRY(cudaMallocAsync(&p, bytes, st)); return SDTW_OK; }
-    ~DevBuf() { if (p) cudaFreeAsync(p, s); }
-};
-}  // namespace
 
 int sdtw_value_grad_host(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
                          float gamma, float* out_values, float* out_grad, void* stream_) {
@@ -934,6 +1073,12 @@ size_t sdtw_dtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, in
     if (get_device(di) == SDTW_OK) sms = di.sms;
     if (build_layout(m, d, offsets, N, false, L, 2, sms) != SDTW_OK) return 0;
     return L.total;
+}
+
+int sdtw_set_workspace_limit(size_t bytes) {
+    std::lock_guard<std::mutex> lock(g_mutex);
+    g_ws_limit = bytes;
+    return SDTW_OK;
 }
 
 int sdtw_set_workspace(void* dev_ptr, size_t bytes) {

@@ -236,6 +236,43 @@ def test_determinism_bitwise_and_workspace_registration(B):
     assert torch.equal(v1, v4) and torch.equal(g1, g4)
 
 
+def test_waves_of_pairs_when_the_workspace_budget_is_small(B):
+    """include/sdtw.h, WAVES: with a workspace budget below what the whole pair set needs, the pairs are evaluated in
+    consecutive waves in the same workspace.  Values: bitwise those of the unsplit call.  Gradient, objective and the
+    descent: the same up to the grouping of the sum over pairs (float32 round-off)."""
+    import torch
+    cfg = synth.scaled(synth.CONFIGS[4], 0.1, N=13)
+    data = synth.make(cfg)
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    w = B.eq7_weights(data["lengths"])
+    v0, g0, o0 = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, weights=w)
+    step = 0.02 / cfg.N
+    Zb0, vb0, ob0 = B.sdtw_barycenter(Z.clone(), X, data["offsets"], cfg.gamma, 3, step)
+    vf0, _ = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
+    need = B.sdtw_workspace_bytes(cfg.m, cfg.d, data["offsets"], True)
+    n0 = B.sdtw_launch_count()
+    try:
+        B.sdtw_set_workspace_limit(need // 3)
+        v1, g1, o1 = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, weights=w)
+        launches = B.sdtw_launch_count() - n0
+        Zb1, vb1, ob1 = B.sdtw_barycenter(Z.clone(), X, data["offsets"], cfg.gamma, 3, step)
+        B.sdtw_set_workspace_limit(B.sdtw_workspace_bytes(cfg.m, cfg.d, data["offsets"], False) // 2)
+        vf1, _ = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
+        B.sdtw_set_workspace_limit(1024)                     # not even one pair fits
+        with pytest.raises(B.SdtwError) as ei:
+            B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+        assert ei.value.status == B.SDTW_ERR_WORKSPACE
+    finally:
+        B.sdtw_set_workspace_limit(0)
+    assert launches >= 4 * 4                                   # at least four waves of four launches
+    assert torch.equal(v0, v1) and torch.equal(vf0, vf1) and torch.equal(vf0, v0)
+    assert rel_l2(g1.cpu().numpy(), g0.cpu().numpy()) <= 1e-6
+    assert abs(float(o1) - float(o0)) <= 1e-6 * abs(float(o0))
+    moved = float(torch.linalg.norm(Zb0 - Z))
+    assert float(torch.linalg.norm(Zb1 - Zb0)) <= 1e-5 * moved
+    assert torch.allclose(ob1, ob0, rtol=1e-6) and torch.allclose(vb1, vb0, rtol=1e-6, atol=0)
+
+
 def test_argument_errors_leave_outputs_untouched(B):
     import torch
     data = synth.make(1)
