@@ -277,6 +277,40 @@ def barycenter(Z0, X_concat, offsets, gamma, iters, step, mode="full", nthreads=
     return Z, values, obj[:iters]
 
 
+def lbfgs_direction(S, Y, g):
+    """r = H g by the two-loop recursion over the stored pairs (rows of S, Y: oldest first); float64."""
+    g = np.ascontiguousarray(g, np.float64).reshape(-1)
+    S = np.ascontiguousarray(S, np.float64).reshape(-1, g.size) if len(S) else np.zeros((0, g.size))
+    Y = np.ascontiguousarray(Y, np.float64).reshape(-1, g.size) if len(Y) else np.zeros((0, g.size))
+    r = np.zeros_like(g)
+    _chk(_load().oracle_lbfgs_direction(_d(S) if len(S) else None, _d(Y) if len(Y) else None, ctypes.c_int(len(S)),
+                                        ctypes.c_int64(g.size), _d(g), _d(r)))
+    return r
+
+
+def barycenter_lbfgs(Z0, X_concat, offsets, gamma, iters, hist, step0, shrink=0.5, c1=1e-4, max_trials=20, mode="full",
+                     nthreads=0, weights=None, band=-1):
+    """Mirror of sdtw_barycenter_lbfgs (Table 1's optimiser: two-loop L-BFGS + Armijo backtracking), float64.
+    Returns (Z (m,d), values (N,) at the final Z, objective (iters+1,), steps (iters,), trials (iters,))."""
+    Z0, X, off = _f32_inputs(Z0, X_concat, offsets)
+    m, d = Z0.shape
+    N = len(off) - 1
+    Z = np.zeros((m, d), np.float64)
+    values = np.zeros(N, np.float64)
+    obj = np.zeros(iters + 1, np.float64)
+    steps = np.zeros(max(iters, 1), np.float64)
+    trials = np.zeros(max(iters, 1), np.int32)
+    w, wp = _weights(weights, N)
+    _chk(_load().oracle_barycenter_lbfgs_f32(
+        Z0.ctypes.data_as(_c_float_p), ctypes.c_int64(m), ctypes.c_int(d), X.ctypes.data_as(_c_float_p),
+        off.ctypes.data_as(_c_i64_p), ctypes.c_int(N), ctypes.c_double(gamma), wp, ctypes.c_int64(band),
+        ctypes.c_int(iters), ctypes.c_int(hist), ctypes.c_double(step0), ctypes.c_double(shrink), ctypes.c_double(c1),
+        ctypes.c_int(max_trials), _d(Z), _d(values), _d(obj), _d(steps),
+        trials.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), ctypes.c_int(1 if mode == "checkpointed" else 0),
+        ctypes.c_int(nthreads)))
+    return Z, values, obj, steps[:iters], trials[:iters]
+
+
 def barycenter_backtracking(Z0, X_concat, offsets, gamma, iters, step0, shrink=0.5, c1=1e-4, max_trials=20, mode="full",
                             nthreads=0, weights=None, band=-1):
     """Mirror of sdtw_barycenter_backtracking: descent with an Armijo backtracking line search, float64.

@@ -617,3 +617,73 @@ def test_descent_driven_one_evaluation_at_a_time_is_the_c_loop_bitwise(oracle):
     v1, g1, o1 = oracle.value_grad_f64z(data["Z0"].astype(np.float64), data["X"], data["offsets"], 1.0)
     v2, g2, o2 = oracle.value_grad(data["Z0"], data["X"], data["offsets"], 1.0, want_objective=True)
     assert np.array_equal(v1, v2) and np.array_equal(g1, g2) and o1 == o2
+
+
+# ------------------------------------------------------------------------------------------- L-BFGS (Table 1; C23)
+def _dense_bfgs_inverse(S, Y):
+    """The inverse-Hessian approximation of BFGS after the pairs (s_i, y_i), oldest first, from H0 = (s.y / y.y of the
+    newest pair) I, by the textbook update H <- (I - rho s y^T) H (I - rho y s^T) + rho s s^T, as a dense matrix."""
+    n = S.shape[1]
+    H = (S[-1] @ Y[-1]) / (Y[-1] @ Y[-1]) * np.eye(n)
+    for s, y in zip(S, Y):
+        rho = 1.0 / (s @ y)
+        V = np.eye(n) - rho * np.outer(y, s)
+        H = V.T @ H @ V + rho * np.outer(s, s)
+    return H
+
+
+def test_lbfgs_two_loop_recursion_is_the_dense_bfgs_operator(oracle):
+    """oracle.lbfgs_direction (the two-loop recursion, Nocedal & Wright Alg. 7.4) against the dense BFGS matrix built by
+    the update formula in numpy; the secant equation H y = s for the newest pair; no pairs = the identity."""
+    rng = np.random.Generator(np.random.PCG64(555))
+    n = 23
+    A = rng.standard_normal((n, n))
+    A = A @ A.T + n * np.eye(n)                              # curvature of a strictly convex quadratic: y = A s, s.y > 0
+    for count in (1, 2, 5, 9):
+        S = rng.standard_normal((count, n))
+        Y = S @ A
+        g = rng.standard_normal(n)
+        r = oracle.lbfgs_direction(S, Y, g)
+        H = _dense_bfgs_inverse(S, Y)
+        assert np.abs(r - H @ g).max() <= 1e-12 * np.abs(H @ g).max()
+        assert np.abs(oracle.lbfgs_direction(S, Y, Y[-1]) - S[-1]).max() <= 1e-12 * np.abs(S[-1]).max()   # secant equation
+        # a transposed operand (y . q instead of s . q in the first loop) or swapped loop order breaks the symmetry of H
+        g2 = rng.standard_normal(n)
+        assert abs(g2 @ r - g @ oracle.lbfgs_direction(S, Y, g2)) <= 1e-10 * abs(g2 @ r)
+    g = rng.standard_normal(n)
+    assert np.array_equal(oracle.lbfgs_direction(np.zeros((0, n)), np.zeros((0, n)), g), g)
+
+
+def test_lbfgs_descent_pins(oracle):
+    """hist = 0 is the Armijo backtracking descent operation for operation; with history every accepted step satisfies
+    the Armijo condition along its own direction (replayed with independent evaluations), the objective decreases
+    monotonically, and after the first iteration the unit step is tried first."""
+    data = synth.make(1)
+    cfg = data["cfg"]
+    Z0, X, off = data["Z0"], data["X"], data["offsets"]
+    a = oracle.barycenter_backtracking(Z0, X, off, cfg.gamma, 6, 0.05)
+    b = oracle.barycenter_lbfgs(Z0, X, off, cfg.gamma, 6, 0, 0.05)
+    assert all(np.array_equal(x, y) for x, y in zip(a, b))
+    c1, step0 = 1e-4, 0.05
+    # replay: drive the recursion here with independent evaluations (oracle.value_grad_f64z) and numpy vectors
+    Z = Z0.astype(np.float64)
+    Zl, vl, obj, steps, trials = oracle.barycenter_lbfgs(Z0, X, off, cfg.gamma, 7, 4, step0, 0.5, c1)
+    assert np.all(np.diff(obj) < 0) and np.all(steps[1:] == 1.0) and steps[0] == step0
+    S, Y = [], []
+    v, G, f = oracle.value_grad_f64z(Z, X, off, cfg.gamma)
+    for it in range(7):
+        assert abs(f - obj[it]) <= 1e-12 * abs(f)
+        d = -oracle.lbfgs_direction(np.array(S[-4:]), np.array(Y[-4:]), G.reshape(-1)).reshape(G.shape) if S else -G
+        t = steps[it]
+        Zn = Z + t * d
+        vn, Gn, fn = oracle.value_grad_f64z(Zn, X, off, cfg.gamma)
+        assert fn <= f + c1 * t * float((G * d).sum())                       # Armijo along the L-BFGS direction
+        if trials[it] > 1:                                                   # the step before it was rejected
+            tp = t / 0.5
+            _, _, fp = oracle.value_grad_f64z(Z + tp * d, X, off, cfg.gamma, want_grad=False)
+            assert fp > f + c1 * tp * float((G * d).sum())
+        S.append((Zn - Z).reshape(-1)); Y.append((Gn - G).reshape(-1))
+        Z, G, f = Zn, Gn, fn
+    assert np.abs(Z - Zl).max() <= 1e-12 * np.abs(Zl).max() and abs(f - obj[7]) <= 1e-12 * abs(f)
+    # L-BFGS beats plain backtracking descent on the same budget of iterations
+    assert obj[7] < oracle.barycenter_backtracking(Z0, X, off, cfg.gamma, 7, step0, 0.5, c1)[2][7]
