@@ -118,6 +118,24 @@ int sdtw_barycenter_backtracking(float* Z_inout, int64_t m, int32_t d, const flo
                                  float* out_steps, int32_t* out_trials, void* stream);
 
 /*
+ * sdtw_barycenter_lbfgs -- the optimiser Table 1 names (l.320-332: "L-BFGS"; the paper takes it off the shelf, so the
+ * recursion is the textbook one, Nocedal & Wright Algorithm 7.4, with the Armijo backtracking of
+ * sdtw_barycenter_backtracking as its line search; reading C23) on the objective of eq. 7.
+ *   d = -H G by the two-loop recursion over the last `hist` accepted pairs (s = Z' - Z, y = G' - G), H0 = (s.y / y.y of
+ *   the newest pair) I; a direction with G.d >= 0 drops the pairs and falls back to -G.  Trial steps t = step0 when no
+ *   pair is stored, else 1, shrunk by `shrink` up to max_trials times; accept when f(Z + t d) <= f(Z) + c1 t (G.d).
+ *   A pair is stored iff s.y > 1e-10 |s| |y|.  hist = 0 is sdtw_barycenter_backtracking.  hist <= 64.
+ * Vectors are float32 on the device; dot products are float64 fixed-shape trees read back by the host, which runs the
+ * recursion's scalars and the accept test in double: the call BLOCKS (a stream synchronisation per dot product and per
+ * trial).  A trial costs a forward sweep; an accepted trial reuses its checkpoints for the reverse sweep.
+ * Arguments as sdtw_barycenter_backtracking (out_objective HOST [iters + 1] double, out_steps / out_trials HOST [iters]).
+ */
+int sdtw_barycenter_lbfgs(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                          float gamma, const float* weights, int64_t band, int32_t iters, int32_t hist, float step0,
+                          float shrink, float c1, int32_t max_trials, float* out_values, double* out_objective,
+                          float* out_steps, int32_t* out_trials, void* stream);
+
+/*
  * sdtw_dtw_score -- Step 3 of the paper (section 3.4, Def. 8 / eq. 8, l.233-242): the classic DTW of eq. 1 (l.123-127;
  * eq. 5 with gamma = 0, squared-Euclidean delta) between the prototype Z and each cycle x_k, the number of cells
  * |pi_k| of the optimal alignment path, and the similarity score d_score = DTW / |pi|.  When several paths attain the

@@ -27,6 +27,8 @@ SYMBOLS = {
     "sdtw_barycenter_ex": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _i64, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_barycenter_backtracking": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _i64, _i32, _f32, _f32,
                                                     _f32, _i32, _vp, _vp, _vp, _vp, _vp]),
+    "sdtw_barycenter_lbfgs": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _i64, _i32, _i32, _f32, _f32,
+                                             _f32, _i32, _vp, _vp, _vp, _vp, _vp]),
     "sdtw_dtw_score": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _vp, _vp, _vp, _vp]),
     "sdtw_subdtw": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _vp, _vp, _vp, _vp]),
     "sdtw_gd_update": (ctypes.c_int, [_vp, _vp, _i64, _f32, _vp]),
@@ -222,6 +224,29 @@ def sdtw_barycenter_backtracking(Z_inout, X_concat, offsets, gamma, iters, step0
                                                  float(step0), float(shrink), float(c1), int(max_trials), _ptr(out_values),
                                                  ctypes.c_void_p(obj.ctypes.data), ctypes.c_void_p(steps.ctypes.data),
                                                  ctypes.c_void_p(trials.ctypes.data), _stream(stream)))
+    return Z, out_values, obj, steps[:iters], trials[:iters]
+
+
+def sdtw_barycenter_lbfgs(Z_inout, X_concat, offsets, gamma, iters, hist, step0, shrink=0.5, c1=1e-4, max_trials=20,
+                          weights=None, band=-1, out_values=None, stream=None):
+    """L-BFGS (Table 1's optimiser) with an Armijo backtracking line search, in place on Z_inout (include/sdtw.h; blocks).
+    Returns (Z_inout, values (dev, N), objective (iters + 1,) f64, steps (iters,) f32, trials (iters,) i32)."""
+    import torch
+    Z = _dev_f32(Z_inout, "Z_inout")
+    X = _dev_f32(X_concat, "X_concat")
+    m, d = _dims(Z)
+    off, offp, N = _offsets(offsets)
+    w, wp = _weights(weights, N)
+    if out_values is None:
+        out_values = torch.zeros(N, dtype=torch.float32, device=Z.device)
+    obj = np.zeros(int(iters) + 1, np.float64)
+    steps = np.zeros(max(int(iters), 1), np.float32)
+    trials = np.zeros(max(int(iters), 1), np.int32)
+    with torch.cuda.device(Z.device):
+        _check(_lib.sdtw_barycenter_lbfgs(_ptr(Z), m, d, _ptr(X), offp, N, float(gamma), wp, int(band), int(iters), int(hist),
+                                          float(step0), float(shrink), float(c1), int(max_trials), _ptr(out_values),
+                                          ctypes.c_void_p(obj.ctypes.data), ctypes.c_void_p(steps.ctypes.data),
+                                          ctypes.c_void_p(trials.ctypes.data), _stream(stream)))
     return Z, out_values, obj, steps[:iters], trials[:iters]
 
 

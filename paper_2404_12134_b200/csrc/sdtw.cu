@@ -936,6 +936,145 @@ int sdtw_barycenter_backtracking(float* Z_inout, int64_t m, int32_t d, const flo
     return SDTW_OK;
 }
 
+int sdtw_barycenter_lbfgs(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                          float gamma, const float* weights, int64_t band, int32_t iters, int32_t hist, float step0,
+                          float shrink, float c1, int32_t max_trials, float* out_values, double* out_objective,
+                          float* out_steps, int32_t* out_trials, void* stream_) {
+    int rc = check_common(Z_inout, m, d, X_concat, offsets, N, gamma);
+    if (rc) return rc;
+    if (iters < 0 || hist < 0 || hist > 64 || !(std::isfinite(step0) && step0 > 0.f) || !(shrink > 0.f && shrink < 1.f) ||
+        !(std::isfinite(c1) && c1 >= 0.f) || max_trials < 1 || !out_objective || (iters > 0 && (!out_steps || !out_trials)))
+        return SDTW_ERR_INVALID_ARG;
+    int band_eff = -1;
+    rc = check_ex(m, offsets, N, weights, band, &band_eff);
+    if (rc) return rc;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    DeviceInfo di;
+    rc = get_device(di);
+    if (rc) return rc;
+    Plan* pl = nullptr;
+    rc = get_plan(di, m, d, offsets, N, weights, true, stream, &pl);
+    if (rc) return rc;
+    Workspace ws;
+    rc = ws.acquire(pl->L.total, di.dev, stream);
+    if (rc) return rc;
+    const Layout& L = pl->L;
+    const long long md = (long long)m * d;
+    const int blocks = (int)((md + 255) / 256);
+    float* G = reinterpret_cast<float*>(ws.ptr + L.off_G);           // gradient at the current iterate
+    float* Zt = reinterpret_cast<float*>(ws.ptr + L.off_Zt);         // trial point
+    float* Vt = reinterpret_cast<float*>(ws.ptr + L.off_Vt);
+    double* scal = reinterpret_cast<double*>(ws.ptr + L.off_scal);   // [0] objective, [1] dot product
+    // direction, the gradient at the accepted point, and the stored pairs (s_i, y_i): stream-ordered scratch
+    DevBuf vec;
+    const int H = std::max(hist, 1);
+    if ((rc = vec.alloc((size_t)(2 + 2 * H) * md * 4, stream))) return rc;
+    float* Dv = static_cast<float*>(vec.p);
+    float* Gn = Dv + md;
+    float* S = Gn + md;                                                // [H][md], slot i
+    float* Y = S + (size_t)H * md;
+    double h[2] = {0.0, 0.0};
+    auto read_scalars = [&]() -> int {
+        CUDA_TRY(cudaMemcpyAsync(h, scal, sizeof(h), cudaMemcpyDeviceToHost, stream));
+        CUDA_TRY(cudaStreamSynchronize(stream));
+        return SDTW_OK;
+    };
+    auto dot = [&](const float* a, const float* b, double* out) -> int {      // blocks the host: the recursion needs the value
+        dot_kernel<<<1, 1024, 0, stream>>>(a, b, md, scal + 1);
+        ++g_launches;
+        CUDA_TRY(cudaGetLastError());
+        int r = read_scalars();
+        *out = h[1];
+        return r;
+    };
+    auto axpby = [&](float* y, const float* x, double a, double b) -> int {
+        axpby_kernel<<<blocks, 256, 0, stream>>>(y, x, md, (float)a, (float)b);
+        ++g_launches;
+        CUDA_TRY(cudaGetLastError());
+        return SDTW_OK;
+    };
+    // f, values and G at Z0
+    rc = evaluate(*pl, ws.ptr, di, Z_inout, X_concat, gamma, band_eff, out_values, nullptr, G, nullptr, 0.f, stream, 3, scal);
+    if (rc || (rc = read_scalars())) return rc;
+    double f = h[0];
+    out_objective[0] = f;
+    std::vector<int> slots;                                            // ring slots of the stored pairs, oldest first
+    std::vector<double> rho, alpha;
+    bool stopped = false;
+    for (int it = 0; it < iters; ++it) {
+        out_steps[it] = 0.f; out_trials[it] = 0;
+        if (!stopped) {
+            // d = -H G: the two-loop recursion over the stored pairs (include/sdtw.h); scalars in float64 on the host
+            if ((rc = axpby(Dv, G, 1.0, 0.0))) return rc;             // q = G
+            alpha.assign(slots.size(), 0.0);
+            for (int i = (int)slots.size() - 1; i >= 0; --i) {
+                double sq;
+                if ((rc = dot(S + (size_t)slots[i] * md, Dv, &sq))) return rc;
+                alpha[i] = rho[i] * sq;
+                if ((rc = axpby(Dv, Y + (size_t)slots[i] * md, -alpha[i], 1.0))) return rc;
+            }
+            if (!slots.empty()) {
+                const float* sn = S + (size_t)slots.back() * md; const float* yn = Y + (size_t)slots.back() * md;
+                double sy, yy;
+                if ((rc = dot(sn, yn, &sy)) || (rc = dot(yn, yn, &yy))) return rc;
+                if ((rc = axpby(Dv, Dv, sy / yy, 0.0))) return rc;   // r = (s.y / y.y) q
+            }
+            for (size_t i = 0; i < slots.size(); ++i) {
+                double yr;
+                if ((rc = dot(Y + (size_t)slots[i] * md, Dv, &yr))) return rc;
+                if ((rc = axpby(Dv, S + (size_t)slots[i] * md, alpha[i] - rho[i] * yr, 1.0))) return rc;
+            }
+            if ((rc = axpby(Dv, Dv, -1.0, 0.0))) return rc;          // d = -r
+            double gd;
+            if ((rc = dot(G, Dv, &gd))) return rc;
+            if (!(gd < 0.0)) {                                        // not a descent direction: restart from -G
+                slots.clear(); rho.clear();
+                if ((rc = axpby(Dv, G, -1.0, 0.0)) || (rc = dot(G, Dv, &gd))) return rc;
+            }
+            double t = slots.empty() ? (double)step0 : 1.0;
+            bool accepted = false;
+            for (int tr = 0; tr < max_trials; ++tr) {
+                trial_point_kernel<<<blocks, 256, 0, stream>>>(Zt, Z_inout, Dv, md, (float)-t);   // Zt = Z - (-t) d = Z + t d
+                ++g_launches;
+                CUDA_TRY(cudaGetLastError());
+                rc = evaluate(*pl, ws.ptr, di, Zt, X_concat, gamma, band_eff, Vt, nullptr, nullptr, nullptr, 0.f, stream, 1, scal);
+                if (rc || (rc = read_scalars())) return rc;
+                out_trials[it] = tr + 1;
+                if (h[0] <= f + (double)c1 * t * gd) {                 // Armijo condition, on the host in double
+                    // gradient at the accepted point (reverse sweep on the checkpoints the trial wrote), then the pair
+                    rc = evaluate(*pl, ws.ptr, di, Zt, X_concat, gamma, band_eff, nullptr, nullptr, Gn, nullptr, 0.f, stream, 2);
+                    if (rc) return rc;
+                    f = h[0];
+                    if (hist > 0) {
+                        int slot;
+                        if ((int)slots.size() == hist) { slot = slots.front(); slots.erase(slots.begin()); rho.erase(rho.begin()); }
+                        else { slot = 0; while (std::find(slots.begin(), slots.end(), slot) != slots.end()) ++slot; }
+                        float* sn = S + (size_t)slot * md; float* yn = Y + (size_t)slot * md;
+                        diff_kernel<<<blocks, 256, 0, stream>>>(sn, Zt, Z_inout, md);
+                        diff_kernel<<<blocks, 256, 0, stream>>>(yn, Gn, G, md);
+                        g_launches += 2;
+                        CUDA_TRY(cudaGetLastError());
+                        double sy, ss, yy;
+                        if ((rc = dot(sn, yn, &sy)) || (rc = dot(sn, sn, &ss)) || (rc = dot(yn, yn, &yy))) return rc;
+                        if (sy > 1e-10 * std::sqrt(ss) * std::sqrt(yy)) { slots.push_back(slot); rho.push_back(1.0 / sy); }
+                    }
+                    CUDA_TRY(cudaMemcpyAsync(Z_inout, Zt, (size_t)md * 4, cudaMemcpyDeviceToDevice, stream));
+                    CUDA_TRY(cudaMemcpyAsync(G, Gn, (size_t)md * 4, cudaMemcpyDeviceToDevice, stream));
+                    if (out_values) CUDA_TRY(cudaMemcpyAsync(out_values, Vt, (size_t)N * 4, cudaMemcpyDeviceToDevice, stream));
+                    out_steps[it] = (float)t;
+                    accepted = true;
+                    break;
+                }
+                t *= (double)shrink;
+            }
+            if (!accepted) stopped = true;
+        }
+        out_objective[it + 1] = f;
+    }
+    return SDTW_OK;
+}
+
 int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
                     float gamma, int32_t iters, float step, float* out_values, float* out_objective, void* stream_) {
     return sdtw_barycenter_ex(Z_inout, m, d, X_concat, offsets, N, gamma, nullptr, -1, iters, step, out_values,

@@ -970,6 +970,31 @@ __global__ void sqnorm_kernel(const float* __restrict__ G, long long count, doub
     if (threadIdx.x == 0) *out = red[0];
 }
 
+// L-BFGS helpers (sdtw_barycenter_lbfgs): a . b by a fixed-shape tree in float64 (one block; deterministic), and the
+// vector updates of the two-loop recursion, in float32 with a float64 scalar rounded once
+__global__ void dot_kernel(const float* __restrict__ a, const float* __restrict__ b, long long count, double* __restrict__ out) {
+    __shared__ double red[1024];
+    double acc = 0.0;
+    for (long long e = threadIdx.x; e < count; e += blockDim.x) acc += (double)a[e] * (double)b[e];
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = red[0];
+}
+// y = a x + b y  (b = 0: y = a x, y need not be initialised)
+__global__ void axpby_kernel(float* __restrict__ y, const float* __restrict__ x, long long count, float a, float b) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < count) y[e] = (b == 0.f) ? a * x[e] : fmaf(a, x[e], b * y[e]);
+}
+// out = a - b
+__global__ void diff_kernel(float* __restrict__ out, const float* __restrict__ a, const float* __restrict__ b, long long count) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < count) out[e] = a[e] - b[e];
+}
+
 __global__ void gd_update_kernel(float* __restrict__ Z, const float* __restrict__ G, long long count, float step) {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e < count) Z[e] = Z[e] - step * G[e];

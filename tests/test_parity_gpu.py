@@ -936,6 +936,41 @@ def test_backtracking_equals_fixed_step_when_always_accepted(B):
         B.sdtw_barycenter_backtracking(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, 2, 0.1, shrink=1.5)
 
 
+@pytest.mark.parametrize("idx,scale,N,iters,hist,step0", [(1, 1.0, 8, 8, 4, 0.64), (2, 1.0, 16, 6, 5, 0.04), (4, 0.1, 8, 5, 3, 0.02),
+                                                          (3, 0.05, 4, 5, 10, 0.4)])
+def test_lbfgs_descent_matches_oracle(B, oracle, idx, scale, N, iters, hist, step0):
+    """sdtw_barycenter_lbfgs (Table 1's optimiser; include/sdtw.h, C23) against the float64 oracle of the same
+    algorithm: accepted steps, trial counts, objective history and the final barycenter.  The curvature pairs are
+    differences of float32 gradients, so the iterates drift apart faster than under plain descent: the bar on the
+    barycenter stays 2e-3 of the distance moved."""
+    cfg = synth.scaled(synth.CONFIGS[idx], scale, N=N) if (scale != 1.0 or N != synth.CONFIGS[idx].N) else synth.CONFIGS[idx]
+    data = synth.make(cfg)
+    Z, vals, obj, steps, trials = B.sdtw_barycenter_lbfgs(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma,
+                                                          iters, hist, step0)
+    Zo, vo, oo, so, to = oracle.barycenter_lbfgs(data["Z0"], data["X"], data["offsets"], cfg.gamma, iters, hist, step0,
+                                                 mode="checkpointed")
+    print(f"[{cfg.name}] L-BFGS steps {steps.tolist()} (oracle {so.tolist()}), trials {trials.tolist()} ({to.tolist()}), "
+          f"objective {obj.tolist()} (oracle {oo.tolist()})")
+    assert np.array_equal(trials, to) and np.allclose(steps, so, rtol=1e-6)
+    assert np.all(np.diff(obj) < 0)
+    scale_f = np.sum(cfg.gamma * (data["lengths"] + cfg.m))
+    assert np.all(np.abs(obj - oo) <= 1e-4 * np.maximum(np.abs(oo), scale_f))
+    check_barycenter(Z.cpu().numpy(), Zo, data["Z0"], cfg.name + " L-BFGS")
+    check_values(vals.cpu().numpy(), vo, data["lengths"], cfg, f"{cfg.name} values at the final Z (L-BFGS)")
+
+
+def test_lbfgs_without_history_is_the_backtracking_descent(B):
+    import torch
+    data = synth.make(2)
+    cfg = data["cfg"]
+    a = B.sdtw_barycenter_backtracking(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, 4, 0.04)
+    b = B.sdtw_barycenter_lbfgs(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, 4, 0, 0.04)
+    assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+    assert np.array_equal(a[3], b[3]) and np.array_equal(a[4], b[4])
+    with pytest.raises(B.SdtwError):
+        B.sdtw_barycenter_lbfgs(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, 2, -1, 0.04)
+
+
 @pytest.mark.parametrize("d", [5, 7, 9])
 def test_dtw_and_subdtw_up_to_nine_channels(B, oracle, d):
     """The paper's Step 1 aligns all 9 robot variables at once: sdtw_dtw_score / sdtw_subdtw accept
