@@ -35,13 +35,17 @@
  *   eq. 7  per-series weights lambda_i / m_i: the *_ex entry points take one
  *                               weight w_k per pair; objective = sum_k w_k value_k and
  *                               grad = sum_k w_k grad_k (values[k] stay unweighted).
+ *   Table 1  the optimiser ("L-BFGS", off the shelf): oracle_barycenter_backtracking_f32 (descent with
+ *                               an Armijo backtracking line search, reading C22) and oracle_barycenter_lbfgs_f32 (textbook
+ *                               two-loop recursion + the same line search, reading C23; oracle_lbfgs_direction).
  *
  * Index convention: x has n rows (time steps) of d channels, z has m rows of d channels,
  * both row-major [t][c].  R is stored with the paper's 0-row/0-column border (and one more
  * border row/column at n+1 / m+1 for the reverse pass), i.e. (n+2) x (m+2), 1-based cells.
  *
  * parity pins: see tests/test_oracle_pins.py (brute force over all alignment paths, closed
- * forms, Delannoy counts, gamma->0 bounds, invariants of E, finite differences, symmetries).
+ * forms, Delannoy counts, gamma->0 bounds, invariants of E, finite differences, symmetries; the two-loop recursion
+ * against the dense BFGS update formula and the secant equation; Armijo conditions replayed step by step).
  * Not pinned: agreement with TSLearn / the authors' code ("parity unpinned" for that item
  * only -- neither exists in this environment).
  */
