@@ -28,11 +28,12 @@ _c_i64_p = ctypes.POINTER(ctypes.c_int64)
 
 
 def build(force: bool = False) -> Path:
-    """Compile sdtw_oracle.c -> libsdtw_oracle.so (no-op when up to date)."""
-    if force or (not _LIB.exists()) or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+    """Compile sdtw_oracle.c + sdtw_oracle_lbfgs.c -> libsdtw_oracle.so (no-op when up to date)."""
+    srcs = [_SRC, _SRC.with_name("sdtw_oracle_lbfgs.c")]
+    if force or (not _LIB.exists()) or any(_LIB.stat().st_mtime < p.stat().st_mtime for p in srcs):
         tmp = _LIB.with_suffix(f".tmp{os.getpid()}.so")
         cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-fPIC", "-shared", "-fopenmp",
-               "-o", str(tmp), str(_SRC), "-lm"]
+               "-o", str(tmp)] + [str(p) for p in srcs] + ["-lm"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _LIB)
     return _LIB
