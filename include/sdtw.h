@@ -194,7 +194,8 @@ int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_co
  * workspace, else what the device has free -- sdtw_value_grad[_ex] and sdtw_barycenter[_ex] evaluate the pair set as
  * consecutive waves of pairs in the same workspace (pairs are independent): per-pair values are bitwise
  * the same, the gradients of the waves are added in wave order (float32 round-off against the unsplit call).  Only when
- * a single pair does not fit the budget: SDTW_ERR_WORKSPACE.  (sdtw_barycenter_backtracking and the DTW calls do not split.)
+ * a single pair does not fit the budget: SDTW_ERR_WORKSPACE.  (sdtw_barycenter_backtracking, sdtw_barycenter_lbfgs and the
+ * DTW calls do not split.)
  * Forward-only calls (want_grad == 0) without a band keep O(chunks) boundary state per resident strip plus one
  * boundary column per unit of strips; a forward-only call WITH a band that excludes cells keeps a
  * full boundary column per strip: size its workspace with sdtw_workspace_bytes_ex(..., band).  The forward-only size
