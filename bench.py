@@ -364,7 +364,6 @@ def run_ours(args):
         t_fwd, t_bwd = prof["ms_forward"] / n_eval * 1e-3, prof["ms_backward"] / n_eval * 1e-3
         # reverse pass: cells it visited (a visited (strip, chunk) unit = 32 steps x 32 lanes x 2 x 4 cells; the other
         # units carry E = +0 exactly and are skipped)
-        cells_per_chunk = 32 * 32 * 2 * 4
         tile = B.sdtw_tile_info()
         cells_per_chunk = tile["chunk_steps"] * 32 * tile["rows_per_step"] * tile["cols_per_thread"]
         visited_cells = (rev_chunks - rev_skipped) * cells_per_chunk
