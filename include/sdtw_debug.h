@@ -56,10 +56,13 @@ int sdtw_reverse_stats(uint64_t* chunks, uint64_t* skipped);
  */
 int sdtw_set_reverse_kernel(int which);
 /*
- * Forward-only calls without a band pass strip-boundary values through per-warp rings inside a unit of strips when
- * the problem has more strips than resident warps (sdtw_kernels.cuh).  sdtw_set_forward_rings(0) makes them keep one
- * boundary column per strip instead, as the gradient path does (the workspace then has to be sized with
- * sdtw_workspace_bytes_ex and a band that excludes a cell); 1 restores the default.  The values are bitwise the same.
+ * Forward-only calls without a band (and the DTW calls at d <= 2) can pass strip-boundary values through per-warp
+ * rings inside a unit of strips instead of keeping one boundary column per strip (sdtw_kernels.cuh).  1 (default): when
+ * the problem has more strips than resident warps AND the columns would take more than 6 GB (1000 cycles of 30k: 28 GB
+ * of columns, 1 GB with rings, 1 % slower; a few hundred cycles are faster with columns, whose schedule can end with
+ * small units).  2: whenever the problem has more strips than resident warps.  0: never (the workspace then has to be
+ * sized with sdtw_workspace_bytes_ex and a band that excludes a cell).  The values are bitwise the same.
+ * Other values => SDTW_ERR_INVALID_ARG.
  */
 int sdtw_set_forward_rings(int on);
 

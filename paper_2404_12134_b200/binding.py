@@ -426,9 +426,10 @@ def sdtw_set_reverse_kernel(which: int = -1):
     _check(_lib.sdtw_set_reverse_kernel(int(which)))
 
 
-def sdtw_set_forward_rings(on: bool = True):
-    """False: forward-only calls keep one boundary column per strip (the layout of the gradient path).  Same values."""
-    _check(_lib.sdtw_set_forward_rings(1 if on else 0))
+def sdtw_set_forward_rings(mode=1):
+    """0 / False: a boundary column per strip; 1 / True (default): rings when the columns would be large; 2: rings whenever
+    the problem has more strips than resident warps (include/sdtw_debug.h).  Same values."""
+    _check(_lib.sdtw_set_forward_rings(int(mode)))
 
 
 def sdtw_set_schedule(unit_strips: int = 0):

@@ -28,7 +28,7 @@ size_t g_ws_limit = 0;        // sdtw_set_workspace_limit: 0 = what the device h
 // settings never change another thread's launch
 thread_local bool g_profile = false;
 thread_local int g_dense_reverse = 0;
-thread_local int g_forward_rings = 1;       // 0: forward-only calls keep a boundary column per strip (sdtw_set_forward_rings)
+thread_local int g_forward_rings = 1;       // 0: never, 1: when the boundary columns would be large, 2: whenever possible (sdtw_set_forward_rings)
 thread_local int g_reverse_kernel = -1;    // -1 = automatic, 0 = backward_kernel, 1 = reverse_kernel (sdtw_set_reverse_kernel)
 thread_local int g_unit_strips = 0;        // 0 = automatic (sdtw_set_schedule)
 thread_local int g_tail_strips = -1, g_tail_unit = 0;   // -1 = automatic (sdtw_set_schedule_tail)
@@ -109,10 +109,24 @@ int build_layout(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool w
         return (offsets[a + 1] - offsets[a]) > (offsets[b + 1] - offsets[b]);
     });
     // (the DTW kernels, vs_words == 2, have a CTA-full of 32 warps only at d <= 2: more channels keep a column per strip)
-    if (ring_sms > 0 && !want_grad && (vs_words == 1 ? d <= SDTW_MAX_D : d <= 2) &&
-        (long long)L.NS * N > (long long)ring_sms * fwd_warps_rt(d)) {
-        L.ring_units = fwd_warps_rt(d);
-        L.ring_ctas = ring_sms;
+    // ring_sms < 0: rings whenever the problem has more strips than resident warps.  ring_sms > 0: only when, besides,
+    // a column per strip would take more than RING_MIN_COLUMN_BYTES: the ring layout hands out uniform units (a small
+    // unit costs a column), and without the small units at the end of the queue a launch of a few hundred pairs drains
+    // badly (100 pairs of 30k, forward only: 62.5 ms with columns, 70.3 ms with rings; 1000 pairs: 577 / 584 ms).
+    constexpr long long RING_MIN_COLUMN_BYTES = 6LL << 30;
+    const int rsms = ring_sms < 0 ? -ring_sms : ring_sms;
+    if (rsms > 0 && !want_grad && (vs_words == 1 ? d <= SDTW_MAX_D : d <= 2) &&
+        (long long)L.NS * N > (long long)rsms * fwd_warps_rt(d)) {
+        long long column_bytes = 0;
+        for (int k = 0; k < N; ++k) {
+            const long long n = offsets[k + 1] - offsets[k];
+            const long long C = ((n + RP - 1) / RP + 31 + CH - 1) / CH;
+            column_bytes += 4LL * vs_words * (VS_PAD + C * CROWS) * L.NS;
+        }
+        if (ring_sms < 0 || column_bytes > RING_MIN_COLUMN_BYTES) {
+            L.ring_units = fwd_warps_rt(d);
+            L.ring_ctas = rsms;
+        }
     }
     const int cols_per_pair = L.ring_units ? (L.NS + L.ring_units - 1) / L.ring_units - 1 : L.NS;   // boundary columns kept
     L.pm.resize(N);
@@ -199,7 +213,7 @@ struct Plan {
     int64_t m = 0;
     int32_t d = 0, N = 0;
     bool want_grad = false;
-    bool ring_ok = false;         // forward-only call without a band (the layout may use rings)
+    int ring_ok = 0;              // forward-only call without a band: 1 = the layout may use rings, 2 = rings whenever possible
     int vs_words = 1;
     std::vector<int64_t> offsets;
     std::vector<float> weights;   // caller order; empty = unweighted
@@ -214,7 +228,7 @@ std::vector<Plan*> g_plans;
 uint64_t g_stamp = 0;
 
 int get_plan(const DeviceInfo& di, int64_t m, int32_t d, const int64_t* offsets, int32_t N, const float* weights, bool want_grad,
-             cudaStream_t stream, Plan** out, int vs_words = 1, bool ring_ok = false) {
+             cudaStream_t stream, Plan** out, int vs_words = 1, int ring_ok = 0) {
     const int dev = di.dev;
     for (Plan* pl : g_plans) {
         if (pl->dev == dev && pl->m == m && pl->d == d && pl->N == N && pl->want_grad == want_grad &&
@@ -229,7 +243,7 @@ int get_plan(const DeviceInfo& di, int64_t m, int32_t d, const int64_t* offsets,
         }
     }
     Plan* pl = new Plan();
-    int rc = build_layout(m, d, offsets, N, want_grad, pl->L, vs_words, ring_ok ? di.sms : 0);
+    int rc = build_layout(m, d, offsets, N, want_grad, pl->L, vs_words, ring_ok == 2 ? -di.sms : (ring_ok ? di.sms : 0));
     if (rc != SDTW_OK) { delete pl; return rc; }
     pl->vs_words = vs_words;
     pl->ring_ok = ring_ok;
@@ -690,7 +704,7 @@ int plan_waves(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool wan
 // one evaluation over waves.  G (m d floats) receives the summed gradient when want_grad; Gtmp is scratch of the same size;
 // obj64 (W doubles) scratch for the objective.  out_objective may be null.
 int evaluate_waves(const DeviceInfo& di, const std::vector<int>& bounds, char* ws, const float* Z, int64_t m, int32_t d,
-                   const float* X, const int64_t* offsets, const float* weights, float gamma, int band_eff, bool ring_ok,
+                   const float* X, const int64_t* offsets, const float* weights, float gamma, int band_eff, int ring_ok,
                    float* out_values, float* out_objective, float* G, float* Gtmp, double* obj64, cudaStream_t stream) {
     const int W = (int)bounds.size() - 1;
     const long long md = (long long)m * d;
@@ -745,16 +759,17 @@ int sdtw_value_grad_ex(const float* Z, int64_t m, int32_t d, const float* X_conc
     DeviceInfo di;
     rc = get_device(di);
     if (rc) return rc;
-    const bool ring_ok = out_grad == nullptr && band_eff < 0 && g_forward_rings;
+    const int ring_ok = (out_grad == nullptr && band_eff < 0) ? g_forward_rings : 0;
+    const int ring_arg = ring_ok == 2 ? -di.sms : (ring_ok ? di.sms : 0);
     {   // does the workspace of the whole pair set fit?  If not: waves of pairs
         Layout L;
-        rc = build_layout(m, d, offsets, N, out_grad != nullptr, L, 1, ring_ok ? di.sms : 0);
+        rc = build_layout(m, d, offsets, N, out_grad != nullptr, L, 1, ring_arg);
         if (rc) return rc;
         const size_t budget = workspace_budget(di.dev, L.total);
         if (L.total > budget) {
             std::vector<int> bounds;
             size_t max_bytes = 0;
-            rc = plan_waves(m, d, offsets, N, out_grad != nullptr, ring_ok ? di.sms : 0, budget, bounds, &max_bytes);
+            rc = plan_waves(m, d, offsets, N, out_grad != nullptr, ring_arg, budget, bounds, &max_bytes);
             if (rc) return rc;
             Workspace ws;
             rc = ws.acquire(max_bytes, di.dev, stream);
@@ -1093,7 +1108,7 @@ static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const floa
     rc = get_device(di);
     if (rc) return rc;
     Plan* pl = nullptr;
-    rc = get_plan(di, m, d, offsets, N, nullptr, false, stream, &pl, 2, g_forward_rings != 0);
+    rc = get_plan(di, m, d, offsets, N, nullptr, false, stream, &pl, 2, g_forward_rings);
     if (rc) return rc;
     Workspace ws;
     rc = ws.acquire(pl->L.total, di.dev, stream);
@@ -1197,7 +1212,8 @@ size_t sdtw_workspace_bytes_ex(int64_t m, int32_t d, const int64_t* offsets, int
     if (get_device(di) == SDTW_OK) sms = di.sms;
     int band_eff = -1;
     if (band >= 0 && offsets && N >= 1 && m >= 1 && check_ex(m, offsets, N, nullptr, band, &band_eff) != SDTW_OK) return 0;
-    if (build_layout(m, d, offsets, N, want_grad != 0, L, 1, (!want_grad && band_eff < 0) ? sms : 0) != SDTW_OK) return 0;
+    const int ring_arg = (!want_grad && band_eff < 0) ? (g_forward_rings == 2 ? -sms : (g_forward_rings ? sms : 0)) : 0;
+    if (build_layout(m, d, offsets, N, want_grad != 0, L, 1, ring_arg) != SDTW_OK) return 0;
     return L.total;
 }
 
@@ -1210,7 +1226,7 @@ size_t sdtw_dtw_workspace_bytes(int64_t m, int32_t d, const int64_t* offsets, in
     int sms = 148;
     DeviceInfo di;
     if (get_device(di) == SDTW_OK) sms = di.sms;
-    if (build_layout(m, d, offsets, N, false, L, 2, sms) != SDTW_OK) return 0;
+    if (build_layout(m, d, offsets, N, false, L, 2, g_forward_rings == 2 ? -sms : (g_forward_rings ? sms : 0)) != SDTW_OK) return 0;
     return L.total;
 }
 
@@ -1307,7 +1323,8 @@ int sdtw_set_reverse_mode(int dense) {
 
 int sdtw_set_forward_rings(int on) {
     std::lock_guard<std::mutex> lock(g_mutex);
-    g_forward_rings = on ? 1 : 0;
+    if (on < 0 || on > 2) return SDTW_ERR_INVALID_ARG;
+    g_forward_rings = on;
     return SDTW_OK;
 }
 

@@ -428,13 +428,15 @@ def test_forward_only_rings_match_the_oracle_and_single_pair_calls(B, oracle, d,
     cfg = replace(synth.CONFIGS[5], name=f"rings_d{d}", N=N, n_lo=700, n_hi=1900, m=m, d=d, gamma=0.05)
     data = synth.make(cfg)
     Z, X = _dev(data["Z0"]), _dev(data["X"])
-    vals, G = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
-    vals2, _ = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
     try:
-        B.sdtw_set_forward_rings(False)                       # one boundary column per strip (sdtw_debug.h)
+        B.sdtw_set_forward_rings(2)                           # rings although the columns of this problem are small (sdtw_debug.h)
+        assert B.sdtw_workspace_bytes(m, d, data["offsets"], False) != B.sdtw_workspace_bytes_ex(m, d, data["offsets"], False, m - 100)
+        vals, G = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
+        vals2, _ = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
+        B.sdtw_set_forward_rings(0)                           # one boundary column per strip
         vals3, _ = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
     finally:
-        B.sdtw_set_forward_rings(True)
+        B.sdtw_set_forward_rings(1)
     torch.cuda.synchronize()
     assert G is None and torch.equal(vals, vals2) and torch.equal(vals, vals3)
     ov, _ = oracle.value_grad(data["Z0"], data["X"], data["offsets"], cfg.gamma, want_grad=False, mode="checkpointed")
@@ -454,14 +456,15 @@ def test_dtw_kernels_rings_bit_exact(B, oracle, d, N, m):
     cfg = replace(synth.CONFIGS[5], name=f"dtwrings_d{d}", N=N, n_lo=700, n_hi=1900, m=m, d=d)
     data = synth.make(cfg)
     Z, X = _dev(data["Z0"]), _dev(data["X"])
-    a = [t.cpu().numpy() for t in B.sdtw_dtw_score(Z, X, data["offsets"])]
-    sa = [t.cpu().numpy() for t in B.sdtw_subdtw(Z, X, data["offsets"])]
     try:
-        B.sdtw_set_forward_rings(False)
+        B.sdtw_set_forward_rings(2)
+        a = [t.cpu().numpy() for t in B.sdtw_dtw_score(Z, X, data["offsets"])]
+        sa = [t.cpu().numpy() for t in B.sdtw_subdtw(Z, X, data["offsets"])]
+        B.sdtw_set_forward_rings(0)
         b = [t.cpu().numpy() for t in B.sdtw_dtw_score(Z, X, data["offsets"])]
         sb = [t.cpu().numpy() for t in B.sdtw_subdtw(Z, X, data["offsets"])]
     finally:
-        B.sdtw_set_forward_rings(True)
+        B.sdtw_set_forward_rings(1)
     for x, y in zip(a + sa, b + sb):
         assert np.array_equal(x.view(np.uint32) if x.dtype == np.float32 else x, y.view(np.uint32) if y.dtype == np.float32 else y)
     ov, ol, osc = oracle.dtw_score(data["Z0"], data["X"], data["offsets"])
