@@ -46,6 +46,7 @@ extern "C" {
 #define SDTW_ERR_UNSUPPORTED (-2) /* d > SDTW_MAX_D, sizes beyond the stated limits, device is not sm_100        */
 #define SDTW_ERR_WORKSPACE (-3)   /* registered workspace smaller than sdtw_workspace_bytes()                    */
 #define SDTW_ERR_CUDA (-4)        /* a CUDA runtime call failed; see sdtw_last_cuda_error()                      */
+#define SDTW_ERR_STATIC_LIMIT (-5) /* sdtw_value_static: the problem needs more than the built-in scratch array holds */
 
 #define SDTW_MAX_D 4
 #define SDTW_DTW_MAX_D 9 /* sdtw_dtw_score / sdtw_subdtw: the paper's Step 1 aligns all 9 robot variables at once (l.300) */
@@ -171,6 +172,54 @@ int sdtw_subdtw(const float* Z, int64_t m, int32_t d, const float* X_concat, con
  * gradient is all-reduced across GPUs between sdtw_value_grad and the update.
  */
 int sdtw_gd_update(float* Z_inout, const float* G, int64_t count, float step, void* stream);
+
+/*
+ * sdtw_value_static -- the forward-only sweep of sdtw_value_grad (eq. 5, l.162-167: value_k = Soft-DTW^gamma(x_k, Z) for
+ * every pair, no gradient) for callers that must not allocate device memory.
+ *
+ * Who that is: a plug-in running inside a host application that reserved the whole GPU for its own memory pool up front
+ * (a cudaMalloc from a guest library then fails, or fragments the pool); a control or monitoring loop with a latency
+ * budget, where the implicit device-wide synchronisation of cudaMalloc / cudaFree stalls every other stream; code that
+ * runs where the platform forbids allocation after start-up (certified or long-running services that fix their memory
+ * footprint at load time).  Every other entry point of this header may allocate: the plan metadata of a new shape and,
+ * unless sdtw_set_workspace() registered a buffer, the workspace.  This one never does.
+ *
+ * How: all scratch of the sweep (scaled input copies, work-queue counters, strip-boundary columns, per-strip value
+ * partials, the per-pair schedule table) lives in ONE array of SDTW_STATIC_SCRATCH_BYTES (32 MiB) that is compiled into
+ * the library as a static device variable.  Every GPU on which the library's CUDA module is loaded carries those 32 MiB
+ * from load until the process exits, whether or not this call is ever made; that is the price of the guarantee.  The
+ * call issues kernel launches only (the same prologue / forward / epilogue kernels as sdtw_value_grad with out_grad ==
+ * NULL, column layout, so out_values are BITWISE what that call returns): no cudaMalloc, cudaFree, cudaMallocAsync,
+ * event or stream creation, no memcpy, no host synchronisation.  Profiling (sdtw_debug.h) is ignored by this call.
+ *
+ * Limits.  N <= SDTW_STATIC_MAX_PAIRS (64; the schedule table travels as a kernel argument), and the sweep's scratch
+ * must fit the array: roughly  4 * (n_k + 128) * ceil(m / 128)  bytes per pair  +  8 * d * (sum_k n_k + m)  bytes.
+ * 32 MiB holds one pair of the paper's size (n_k <= 33000 against m = 30000, any d <= SDTW_MAX_D), or 64 pairs of
+ * 3000 x 3000.  Beyond either limit: SDTW_ERR_STATIC_LIMIT, nothing enqueued, outputs untouched.  Other argument errors
+ * as in sdtw_value_grad.
+ *
+ * Sharing.  There is one array per GPU and every call on that GPU uses it, from whichever host thread or stream.  A
+ * call first re-initialises what has to start clean (queue counters to zero, boundary columns to the "not yet written"
+ * pattern), so leftovers of the previous call are harmless -- but two calls whose kernels are in flight at the same
+ * time (different streams, or different host threads on different streams) overwrite each other's scratch and return
+ * garbage or hang.  Keep calls on one GPU stream-ordered: same stream, or an event between them.  The library does not
+ * order them for you (that would need an event, i.e. a resource created at run time).
+ *
+ * Set-up.  The FIRST call on each device resolves the device address of the array (cudaGetSymbolAddress, with that
+ * device current -- the caller makes the device current, as for every call here) and remembers it; later calls on that
+ * device skip this step.  Make that first call during start-up, before any stream capture is begun -- and before the
+ * host application takes the rest of the GPU's memory: the CUDA driver creates the array when it loads this library's
+ * module on the device, which (CUDA loads modules lazily) happens at the first libsdtw call that touches the device.
+ * For the same reason the first launch of the sweep for each channel count d makes the driver load that kernel's code
+ * (a one-off 2 MiB step in the device's free memory, measured): call once per d you will use, at start-up.
+ *
+ *   Z, X_concat  dev, offsets HOST [N+1], gamma: as in sdtw_value_grad
+ *   out_values   dev [N] float32 (required), value_k in the caller's pair order
+ */
+#define SDTW_STATIC_SCRATCH_BYTES (32u << 20)
+#define SDTW_STATIC_MAX_PAIRS 64
+int sdtw_value_static(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                      float gamma, float* out_values, void* stream);
 
 /*
  * Host-buffer variants (all pointers HOST; pinned memory makes the copies asynchronous).  They copy the inputs to

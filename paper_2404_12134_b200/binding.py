@@ -32,6 +32,7 @@ SYMBOLS = {
     "sdtw_dtw_score": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _vp, _vp, _vp, _vp]),
     "sdtw_subdtw": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _vp, _vp, _vp, _vp]),
     "sdtw_gd_update": (ctypes.c_int, [_vp, _vp, _i64, _f32, _vp]),
+    "sdtw_value_static": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _vp]),
     "sdtw_value_grad_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_barycenter_host": (ctypes.c_int, [_vp, _i64, _i32, _vp, _i64p, _i32, _f32, _i32, _f32, _vp, _vp, _vp]),
     "sdtw_workspace_bytes": (ctypes.c_size_t, [_i64, _i32, _i64p, _i32, ctypes.c_int]),
@@ -58,6 +59,8 @@ for _name, (_res, _args) in SYMBOLS.items():
     _fn.restype, _fn.argtypes = _res, _args
 
 SDTW_OK, SDTW_ERR_INVALID_ARG, SDTW_ERR_UNSUPPORTED, SDTW_ERR_WORKSPACE, SDTW_ERR_CUDA = 0, -1, -2, -3, -4
+SDTW_ERR_STATIC_LIMIT = -5
+STATIC_SCRATCH_BYTES, STATIC_MAX_PAIRS = 32 << 20, 64     # sdtw_value_static (include/sdtw.h)
 
 
 class SdtwError(RuntimeError):
@@ -123,6 +126,26 @@ def sdtw_value_grad(Z, X_concat, offsets, gamma, out_values=None, out_grad=None,
         _check(_lib.sdtw_value_grad(_ptr(Z), m, d, _ptr(X), offp, N, float(gamma), _ptr(out_values),
                                     _ptr(out_grad) if want_grad else None, _stream(stream)))
     return out_values, (out_grad if want_grad else None)
+
+
+def sdtw_value_static(Z, X_concat, offsets, gamma, out_values, stream=None):
+    """Soft-DTW values of every pair, for callers that must not allocate device memory (a guest inside another
+    program's memory pool, a latency-bound loop, a fixed-footprint service): the library call behind this uses only its
+    built-in 32 MiB scratch array and the tensors passed in.  So `out_values` (float32, CUDA, one entry per pair) is
+    REQUIRED here -- this wrapper, too, allocates nothing on the device.  Problems beyond the array or beyond 64 pairs
+    raise SdtwError(SDTW_ERR_STATIC_LIMIT).  Calls on one GPU share the array: keep them stream-ordered.  Returns
+    out_values (bitwise what sdtw_value_grad(..., want_grad=False) computes)."""
+    Z = _dev_f32(Z, "Z")
+    X = _dev_f32(X_concat, "X_concat")
+    out_values = _dev_f32(out_values, "out_values")
+    m, d = _dims(Z)
+    off, offp, N = _offsets(offsets)
+    if out_values.numel() != N:
+        raise ValueError("out_values must have one entry per pair")
+    import torch
+    with torch.cuda.device(Z.device):
+        _check(_lib.sdtw_value_static(_ptr(Z), m, d, _ptr(X), offp, N, float(gamma), _ptr(out_values), _stream(stream)))
+    return out_values
 
 
 def sdtw_barycenter(Z_inout, X_concat, offsets, gamma, iters, step, out_values=None, out_objective=None, stream=None):

@@ -1204,6 +1204,84 @@ int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_co
     return SDTW_OK;
 }
 
+// ---- sdtw_value_static: the forward-only sweep with its scratch in a static device array (no allocation) ----------
+}  // extern "C"
+
+// The one scratch array of sdtw_value_static (include/sdtw.h).  It belongs to this library's CUDA module: each GPU the
+// module is loaded on holds its own copy until the process exits.  In HOST code the name g_static_scratch is only a
+// handle of the symbol -- not an address a kernel can use; the device address comes from cudaGetSymbolAddress
+// (static_scratch_ptr below).  DEVICE code may name the array directly (static_meta_kernel does).
+static __device__ __align__(256) unsigned char g_static_scratch[SDTW_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+// The per-pair schedule table, passed by value as a kernel argument so that no host-to-device copy is needed.
+struct StaticMeta { PairMeta pm[SDTW_STATIC_MAX_PAIRS]; };
+static_assert(sizeof(StaticMeta) <= 4000, "the schedule table must fit the kernel argument space");
+
+// Writes the schedule table into the scratch array at byte offset `off` (device code: names the array itself).
+__global__ void static_meta_kernel(const __grid_constant__ StaticMeta meta, int N, unsigned long long off) {
+    PairMeta* dst = reinterpret_cast<PairMeta*>(g_static_scratch + off);
+    for (int i = threadIdx.x; i < N; i += blockDim.x) dst[i] = meta.pm[i];
+}
+
+// Device address of g_static_scratch on the CURRENT device, resolved once per device (under g_mutex).
+int static_scratch_ptr(int dev, char** out) {
+    static char* ptr[64] = {};
+    if (!ptr[dev]) {
+        void* p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return SDTW_ERR_UNSUPPORTED;
+        ptr[dev] = static_cast<char*>(p);
+    }
+    *out = ptr[dev];
+    return SDTW_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int sdtw_value_static(const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets, int32_t N,
+                      float gamma, float* out_values, void* stream_) {
+    int rc = check_common(Z, m, d, X_concat, offsets, N, gamma);
+    if (rc) return rc;
+    if (!out_values) return SDTW_ERR_INVALID_ARG;
+    if (N > SDTW_STATIC_MAX_PAIRS) return SDTW_ERR_STATIC_LIMIT;
+    // a Plan that lives on this stack frame only: same layout as sdtw_value_grad(out_grad = NULL) with a boundary column
+    // per strip (no rings, so the layout does not depend on the device), the schedule table appended behind it
+    Plan pl;
+    rc = build_layout(m, d, offsets, N, false, pl.L, 1, 0);
+    if (rc) return rc;
+    const size_t off_pm = align_up(pl.L.total, 256);
+    if (off_pm + sizeof(PairMeta) * (size_t)N > (size_t)SDTW_STATIC_SCRATCH_BYTES) return SDTW_ERR_STATIC_LIMIT;
+    std::lock_guard<std::mutex> lock(g_mutex);
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    DeviceInfo di;
+    rc = get_device(di);
+    if (rc) return rc;
+    char* scratch = nullptr;
+    rc = static_scratch_ptr(di.dev, &scratch);      // first call on this device: cudaGetSymbolAddress
+    if (rc) return rc;
+    pl.dev = di.dev; pl.m = m; pl.d = d; pl.N = N; pl.want_grad = false;
+    pl.offsets.assign(offsets, offsets + N + 1);
+    pl.cells = (long long)offsets[N] * m;
+    pl.d_pm = reinterpret_cast<PairMeta*>(scratch + off_pm);
+    StaticMeta meta;
+    std::memset(&meta, 0, sizeof(meta));
+    for (int ps = 0; ps < N; ++ps) meta.pm[ps] = pl.L.pm[ps];
+    static_meta_kernel<<<1, 64, 0, stream>>>(meta, N, (unsigned long long)off_pm);
+    ++g_launches;
+    CUDA_TRY(cudaGetLastError());
+    // the sweep itself: evaluate() clears the counters and presets the boundary columns in its prologue launch, so the
+    // previous call's contents of the array do not matter.  Profiling would create events: off for this call.
+    const bool profile = g_profile;
+    g_profile = false;
+    rc = evaluate(pl, scratch, di, Z, X_concat, gamma, -1, out_values, nullptr, nullptr, nullptr, 0.f, stream);
+    g_profile = profile;
+    return rc;
+}
+
 // ---- workspace, status, instrumentation -------------------------------------------------------------------------
 size_t sdtw_workspace_bytes_ex(int64_t m, int32_t d, const int64_t* offsets, int32_t N, int want_grad, int64_t band) {
     Layout L;
@@ -1264,6 +1342,9 @@ const char* sdtw_status_string(int status) {
         case SDTW_ERR_UNSUPPORTED: return "unsupported (d > SDTW_MAX_D, size beyond limits, or device is not sm_100)";
         case SDTW_ERR_WORKSPACE: return "registered workspace too small";
         case SDTW_ERR_CUDA: return "CUDA runtime error (see sdtw_last_cuda_error)";
+        case SDTW_ERR_STATIC_LIMIT:
+            return "sdtw_value_static: more than SDTW_STATIC_MAX_PAIRS pairs, or the sweep needs more scratch than the built-in "
+                   "SDTW_STATIC_SCRATCH_BYTES array holds (use sdtw_value_grad with a registered workspace instead)";
     }
     return "unknown status";
 }
