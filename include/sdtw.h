@@ -44,7 +44,7 @@ extern "C" {
 #define SDTW_OK 0
 #define SDTW_ERR_INVALID_ARG (-1) /* NULL required pointer, m/d/N < 1, gamma <= 0 or non-finite, empty cycle, ... */
 #define SDTW_ERR_UNSUPPORTED (-2) /* d > SDTW_MAX_D, sizes beyond the stated limits, device is not sm_100        */
-#define SDTW_ERR_WORKSPACE (-3)   /* registered workspace smaller than sdtw_workspace_bytes()                    */
+#define SDTW_ERR_WORKSPACE (-3)   /* the workspace budget does not hold the call (or, with waves, one pair)      */
 #define SDTW_ERR_CUDA (-4)        /* a CUDA runtime call failed; see sdtw_last_cuda_error()                      */
 #define SDTW_ERR_STATIC_LIMIT (-5) /* sdtw_value_static: the problem needs more than the built-in scratch array holds */
 
@@ -244,7 +244,12 @@ int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_co
  * consecutive waves of pairs in the same workspace (pairs are independent): per-pair values are bitwise
  * the same, the gradients of the waves are added in wave order (float32 round-off against the unsplit call).  Only when
  * a single pair does not fit the budget: SDTW_ERR_WORKSPACE.  (sdtw_barycenter_backtracking, sdtw_barycenter_lbfgs and the
- * DTW calls do not split.)
+ * DTW calls do not split: they return SDTW_ERR_WORKSPACE when a registered workspace is too small.)  A split is silent;
+ * with the library-owned buffer the budget is the device's free memory at the time of the call, so a co-tenant that
+ * holds memory (a caching allocator) makes calls split into more waves: sdtw_last_wave_count() (sdtw_debug.h) tells.
+ * THREADS.  Calls are serialised by one library lock while they enqueue.  The two line-search calls (backtracking,
+ * L-BFGS) block on the stream once per trial and hold that lock for their whole run: other threads' libsdtw calls, on
+ * any device, wait until they return.
  * Forward-only calls (want_grad == 0) without a band keep O(chunks) boundary state per resident strip plus one
  * boundary column per unit of strips; a forward-only call WITH a band that excludes cells keeps a
  * full boundary column per strip: size its workspace with sdtw_workspace_bytes_ex(..., band).  The forward-only size

@@ -25,6 +25,10 @@ extern "C" {
  *                         evaluations they cover; clears the accumulators.  Any pointer may be NULL.
  */
 uint64_t sdtw_launch_count(void);
+/* Waves of pairs (sdtw.h, "WAVES") the calling thread's last sdtw_value_grad[_ex] / sdtw_barycenter[_ex] call was
+ * evaluated in: 1 = unsplit, 0 = no such call yet.  A call that splits does so silently (same values); a caller that
+ * shares the GPU with a caching allocator can watch this number to notice that its budget has become small. */
+int sdtw_last_wave_count(void);
 int sdtw_profile_enable(int on);
 int sdtw_profile_read(double* ms_forward, double* ms_backward, double* ms_other, int64_t* evaluations);
 

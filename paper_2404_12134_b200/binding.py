@@ -43,6 +43,7 @@ SYMBOLS = {
     "sdtw_status_string": (ctypes.c_char_p, [ctypes.c_int]),
     "sdtw_last_cuda_error": (ctypes.c_int, []),
     "sdtw_launch_count": (ctypes.c_uint64, []),
+    "sdtw_last_wave_count": (ctypes.c_int, []),
     "sdtw_profile_enable": (ctypes.c_int, [ctypes.c_int]),
     "sdtw_profile_read": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double)] * 3 + [_i64p]),
     "sdtw_tile_info": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int32)] * 5),
@@ -412,6 +413,11 @@ def sdtw_set_workspace_limit(nbytes: int = 0):
 
 def sdtw_launch_count() -> int:
     return int(_lib.sdtw_launch_count())
+
+
+def sdtw_last_wave_count() -> int:
+    """Waves of pairs this thread's last value_grad / barycenter call was split into (1 = unsplit)."""
+    return int(_lib.sdtw_last_wave_count())
 
 
 def sdtw_profile_enable(on: bool):

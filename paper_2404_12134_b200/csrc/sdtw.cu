@@ -35,6 +35,8 @@ thread_local int g_tail_strips = -1, g_tail_unit = 0;   // -1 = automatic (sdtw_
 thread_local const unsigned long long* g_last_stats = nullptr;   // device address of the last evaluation's reverse statistics
 thread_local uint64_t g_last_stats_gen = 0;   // ... valid while no workspace has been freed since (g_ws_gen)
 uint64_t g_ws_gen = 1;
+thread_local int g_last_waves = 0;          // waves the last sdtw_value_grad[_ex] / sdtw_barycenter[_ex] call of this thread was split into
+size_t g_plan_cap = 32;                     // plans kept (LRU); raised to hold every sub-plan of a call split into many waves
 
 // CUDA events bracketing the phases of one evaluation: start | prologue | forward | reverse | small kernels.
 // Owned by a ProfScope until the evaluation has been enqueued completely; an early return destroys them.
@@ -179,9 +181,11 @@ struct DeviceInfo { int dev = -1, sms = 0, cc_major = 0; bool ok = false; };
 
 int get_device(DeviceInfo& di) {
     static DeviceInfo cache[64];
+    static std::mutex cache_mutex;                  // the *_workspace_bytes queries come here without g_mutex
     int dev = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     if (dev < 0 || dev >= 64) return SDTW_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> cache_lock(cache_mutex);
     if (!cache[dev].ok) {
         cudaDeviceProp prop;
         CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
@@ -227,20 +231,28 @@ struct Plan {
 std::vector<Plan*> g_plans;
 uint64_t g_stamp = 0;
 
-int get_plan(const DeviceInfo& di, int64_t m, int32_t d, const int64_t* offsets, int32_t N, const float* weights, bool want_grad,
-             cudaStream_t stream, Plan** out, int vs_words = 1, int ring_ok = 0) {
-    const int dev = di.dev;
+// the cached plan of this problem, or null
+Plan* find_plan(int dev, int64_t m, int32_t d, const int64_t* offsets, int32_t N, const float* weights, bool want_grad,
+                int vs_words, int ring_ok) {
     for (Plan* pl : g_plans) {
         if (pl->dev == dev && pl->m == m && pl->d == d && pl->N == N && pl->want_grad == want_grad &&
             pl->vs_words == vs_words && pl->ring_ok == ring_ok &&
             std::memcmp(pl->offsets.data(), offsets, sizeof(int64_t) * (size_t)(N + 1)) == 0 &&
             (weights ? (!pl->weights.empty() && std::memcmp(pl->weights.data(), weights, sizeof(float) * (size_t)N) == 0)
-                     : pl->weights.empty())) {
-            pl->stamp = ++g_stamp;
-            CUDA_TRY(cudaStreamWaitEvent(stream, pl->uploaded, 0));
-            *out = pl;
-            return SDTW_OK;
-        }
+                     : pl->weights.empty()))
+            return pl;
+    }
+    return nullptr;
+}
+
+int get_plan(const DeviceInfo& di, int64_t m, int32_t d, const int64_t* offsets, int32_t N, const float* weights, bool want_grad,
+             cudaStream_t stream, Plan** out, int vs_words = 1, int ring_ok = 0) {
+    const int dev = di.dev;
+    if (Plan* hit = find_plan(dev, m, d, offsets, N, weights, want_grad, vs_words, ring_ok)) {
+        hit->stamp = ++g_stamp;
+        CUDA_TRY(cudaStreamWaitEvent(stream, hit->uploaded, 0));
+        *out = hit;
+        return SDTW_OK;
     }
     Plan* pl = new Plan();
     int rc = build_layout(m, d, offsets, N, want_grad, pl->L, vs_words, ring_ok == 2 ? -di.sms : (ring_ok ? di.sms : 0));
@@ -269,7 +281,7 @@ int get_plan(const DeviceInfo& di, int64_t m, int32_t d, const int64_t* offsets,
         return SDTW_ERR_CUDA;
     }
     pl->stamp = ++g_stamp;
-    if (g_plans.size() >= 32) {   // evict the least recently used plan
+    if (g_plans.size() >= g_plan_cap) {   // evict the least recently used plan
         auto it = std::min_element(g_plans.begin(), g_plans.end(), [](Plan* a, Plan* b) { return a->stamp < b->stamp; });
         cudaFree((*it)->d_pm);
         if ((*it)->d_w) cudaFree((*it)->d_w);
@@ -598,7 +610,7 @@ cudaStream_t g_capture_stream[64];
 
 bool graph_eligible(const Plan& pl) {
     return pl.cells <= GRAPH_MAX_CELLS && !g_profile && !g_dense_reverse && g_unit_strips == 0 && g_tail_strips < 0 &&
-           g_reverse_kernel < 0;
+           g_tail_unit == 0 && g_reverse_kernel < 0;
 }
 
 template <typename F>
@@ -677,6 +689,16 @@ size_t workspace_budget(int dev, size_t need) {
 // the largest of them.  SDTW_ERR_WORKSPACE if a single pair does not fit.
 int plan_waves(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, int ring_sms, size_t budget,
                std::vector<int>& bounds, size_t* max_bytes) {
+    // the split of the last problem is remembered (a descent loop asks for the same one every iteration; under g_mutex)
+    struct Memo { int64_t m = 0; int32_t d = 0, N = 0; bool want_grad = false; int ring_sms = 0; size_t budget = 0, max_bytes = 0;
+                  std::vector<int64_t> offsets; std::vector<int> bounds; };
+    static Memo memo;
+    if (memo.N == N && memo.m == m && memo.d == d && memo.want_grad == want_grad && memo.ring_sms == ring_sms &&
+        memo.budget == budget && std::memcmp(memo.offsets.data(), offsets, sizeof(int64_t) * (size_t)(N + 1)) == 0) {
+        bounds = memo.bounds;
+        *max_bytes = memo.max_bytes;
+        return SDTW_OK;
+    }
     std::vector<int64_t> sub;
     std::vector<int> candidates;                    // wave counts tried: 1 .. 8, then growing by a quarter, at last N
     for (int W = 1; W < N; W = (W < 8 ? W + 1 : W + W / 4)) candidates.push_back(W);
@@ -696,7 +718,12 @@ int plan_waves(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool wan
             mx = std::max(mx, L.total);
             ok = L.total <= budget;
         }
-        if (ok) { *max_bytes = mx; return SDTW_OK; }
+        if (ok) {
+            *max_bytes = mx;
+            memo.m = m; memo.d = d; memo.N = N; memo.want_grad = want_grad; memo.ring_sms = ring_sms; memo.budget = budget;
+            memo.max_bytes = mx; memo.offsets.assign(offsets, offsets + N + 1); memo.bounds = bounds;
+            return SDTW_OK;
+        }
     }
     return SDTW_ERR_WORKSPACE;
 }
@@ -708,6 +735,10 @@ int evaluate_waves(const DeviceInfo& di, const std::vector<int>& bounds, char* w
                    float* out_values, float* out_objective, float* G, float* Gtmp, double* obj64, cudaStream_t stream) {
     const int W = (int)bounds.size() - 1;
     const long long md = (long long)m * d;
+    // every wave has a sub-plan: keep them all cached, or each wave of each iteration would miss (allocation, upload and
+    // an eviction whose cudaFree synchronises the device)
+    g_plan_cap = std::max(g_plan_cap, (size_t)W + 16);
+    g_last_waves = W;
     std::vector<int64_t> sub;
     for (int w = 0; w < W; ++w) {
         const int k0 = bounds[w], k1 = bounds[w + 1];
@@ -761,12 +792,19 @@ int sdtw_value_grad_ex(const float* Z, int64_t m, int32_t d, const float* X_conc
     if (rc) return rc;
     const int ring_ok = (out_grad == nullptr && band_eff < 0) ? g_forward_rings : 0;
     const int ring_arg = ring_ok == 2 ? -di.sms : (ring_ok ? di.sms : 0);
-    {   // does the workspace of the whole pair set fit?  If not: waves of pairs
-        Layout L;
-        rc = build_layout(m, d, offsets, N, out_grad != nullptr, L, 1, ring_arg);
-        if (rc) return rc;
-        const size_t budget = workspace_budget(di.dev, L.total);
-        if (L.total > budget) {
+    g_last_waves = 1;
+    {   // does the workspace of the whole pair set fit?  If not: waves of pairs.  (A cached plan knows the size; only a
+        // new shape pays for a layout here.)
+        size_t total = 0;
+        if (const Plan* hit = find_plan(di.dev, m, d, offsets, N, weights, out_grad != nullptr, 1, ring_ok)) total = hit->L.total;
+        else {
+            Layout L;
+            rc = build_layout(m, d, offsets, N, out_grad != nullptr, L, 1, ring_arg);
+            if (rc) return rc;
+            total = L.total;
+        }
+        const size_t budget = workspace_budget(di.dev, total);
+        if (total > budget) {
             std::vector<int> bounds;
             size_t max_bytes = 0;
             rc = plan_waves(m, d, offsets, N, out_grad != nullptr, ring_arg, budget, bounds, &max_bytes);
@@ -818,12 +856,18 @@ int sdtw_barycenter_ex(float* Z_inout, int64_t m, int32_t d, const float* X_conc
     rc = get_device(di);
     if (rc) return rc;
     if (iters == 0) return SDTW_OK;
+    g_last_waves = 1;
     {   // waves of pairs when the workspace of the whole pair set does not fit (see evaluate_waves)
-        Layout L;
-        rc = build_layout(m, d, offsets, N, true, L);
-        if (rc) return rc;
-        const size_t budget = workspace_budget(di.dev, L.total);
-        if (L.total > budget) {
+        size_t total = 0;
+        if (const Plan* hit = find_plan(di.dev, m, d, offsets, N, weights, true, 1, 0)) total = hit->L.total;
+        else {
+            Layout L;
+            rc = build_layout(m, d, offsets, N, true, L);
+            if (rc) return rc;
+            total = L.total;
+        }
+        const size_t budget = workspace_budget(di.dev, total);
+        if (total > budget) {
             std::vector<int> bounds;
             size_t max_bytes = 0;
             rc = plan_waves(m, d, offsets, N, true, 0, budget, bounds, &max_bytes);
@@ -1340,7 +1384,9 @@ const char* sdtw_status_string(int status) {
         case SDTW_OK: return "ok";
         case SDTW_ERR_INVALID_ARG: return "invalid argument";
         case SDTW_ERR_UNSUPPORTED: return "unsupported (d > SDTW_MAX_D, size beyond limits, or device is not sm_100)";
-        case SDTW_ERR_WORKSPACE: return "registered workspace too small";
+        case SDTW_ERR_WORKSPACE:
+            return "workspace budget too small: the registered workspace (or the sdtw_set_workspace_limit / free-memory budget) "
+                   "does not hold this call, or, for calls that split into waves, not even one pair";
         case SDTW_ERR_CUDA: return "CUDA runtime error (see sdtw_last_cuda_error)";
         case SDTW_ERR_STATIC_LIMIT:
             return "sdtw_value_static: more than SDTW_STATIC_MAX_PAIRS pairs, or the sweep needs more scratch than the built-in "
@@ -1350,6 +1396,8 @@ const char* sdtw_status_string(int status) {
 }
 
 int sdtw_last_cuda_error(void) { return g_last_cuda_error; }
+
+int sdtw_last_wave_count(void) { return g_last_waves; }
 
 uint64_t sdtw_launch_count(void) {
     std::lock_guard<std::mutex> lock(g_mutex);

@@ -984,8 +984,9 @@ __global__ void dot_kernel(const float* __restrict__ a, const float* __restrict_
     }
     if (threadIdx.x == 0) *out = red[0];
 }
-// y = a x + b y  (b = 0: y = a x, y need not be initialised)
-__global__ void axpby_kernel(float* __restrict__ y, const float* __restrict__ x, long long count, float a, float b) {
+// y = a x + b y  (b = 0: y = a x, y need not be initialised).  x may BE y (the in-place scalings of the L-BFGS
+// recursion), so neither pointer is __restrict__: every thread reads element e before it writes it.
+__global__ void axpby_kernel(float* y, const float* x, long long count, float a, float b) {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e < count) y[e] = (b == 0.f) ? a * x[e] : fmaf(a, x[e], b * y[e]);
 }

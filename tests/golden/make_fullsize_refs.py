@@ -3,7 +3,7 @@
 fullsize_refs.json).  Calls ONLY the float64 oracle (oracle/) and the seeded input generator (synth) -- never the
 CUDA path.  Hours of CPU time for cfg 4; resumable (every oracle evaluation is cached under --state-dir).
 
-    python tests/golden/make_fullsize_refs.py [--cfg 3 4 5] [--threads T] [--state-dir DIR] [--only base|pert]
+    python tests/golden/make_fullsize_refs.py [--cfg 3 4 5] [--cfg5-all] [--threads T] [--state-dir DIR] [--only base|pert]
 
 What is stored (BASELINE.json north_star: "summed Soft-DTW value+gradient and the barycenter matching the float64
 oracle ... on all five configs"; cfg 1-2 are computed live by the tests, cfg 3-5 come from here):
@@ -11,7 +11,8 @@ oracle ... on all five configs"; cfg 1-2 are computed live by the tests, cfg 3-5
                  the objective history, the last evaluated per-pair values and the iterate Z after the configured
                  iterations of Z <- Z - step G (eq. 7; Z kept in float64 between iterations, reading C14)
                  at the step frozen in synth.CONFIGS (reading C12), after the contractivity check below has passed.
-  cfg 5          Soft-DTW values of 64 seeded pairs, 16 of them anomalous.
+  cfg 5          Soft-DTW values of all 1000 pairs (--cfg5-all), else of 64 seeded pairs, 16 of them anomalous
+                 (SURVEY.md 8(d)).
 Contractivity check (reading C13): the same descent is run from Z0 (1 + 1e-6 xi), xi ~ N(0, 1) seeded.
 If the two final iterates differ by more than 1e-4 (relative L2), i.e. the map amplifies a perturbation more than
 100 x, parity of the iterated map would measure chaos, not correctness: the step is halved and the check repeated;
@@ -151,17 +152,35 @@ def cfg5_sample(data):
 
 
 def make_cfg5(args):
+    """--cfg5-all: all 1000 values of the scoring sweep ("all 1000 values if the cache exists"; about
+    15 core-hours), else the 64-pair sample.  Computed in batches of pairs cached under --state-dir (resumable); the
+    output file is written only when every batch is there."""
     data = synth.make(5)
     cfg = data["cfg"]
-    ks = cfg5_sample(data)
+    ks = np.arange(cfg.N) if args.cfg5_all else cfg5_sample(data)
     off = data["offsets"]
-    chunks = [data["X"][off[k]:off[k + 1]] for k in ks]
-    o = np.zeros(len(ks) + 1, np.int64)
-    np.cumsum([len(c) for c in chunks], out=o[1:])
+    state = Path(args.state_dir)
+    state.mkdir(parents=True, exist_ok=True)
+    key0 = sha256_inputs(data)[:16] + sha256_oracle()[:16]
+    batch = max(8 * args.threads, 8)
+    values = np.zeros(len(ks), np.float64)
     t = time.time()
-    values, _ = oracle.value_grad(data["Z0"], np.concatenate(chunks), o, cfg.gamma, want_grad=False, mode="checkpointed",
-                                  nthreads=args.threads)
-    print(f"cfg 5: {len(ks)} values ({time.time() - t:.0f} s)", flush=True)
+    for b0 in range(0, len(ks), batch):
+        kb = ks[b0:b0 + batch]
+        f = state / f"cfg5_{key0}_{int(kb[0])}_{int(kb[-1])}_{len(kb)}.npy"
+        if f.exists():
+            values[b0:b0 + len(kb)] = np.load(f)
+            continue
+        chunks = [data["X"][off[k]:off[k + 1]] for k in kb]
+        o = np.zeros(len(kb) + 1, np.int64)
+        np.cumsum([len(c) for c in chunks], out=o[1:])
+        v, _ = oracle.value_grad(data["Z0"], np.concatenate(chunks), o, cfg.gamma, want_grad=False, mode="checkpointed",
+                                 nthreads=args.threads)
+        tmp = f.with_suffix(".tmp.npy")
+        np.save(tmp, v)
+        os.replace(tmp, f)
+        values[b0:b0 + len(kb)] = v
+        print(f"cfg 5: pairs {b0 + len(kb)} of {len(ks)} ({time.time() - t:.0f} s)", flush=True)
     np.savez(HERE / "fullsize_cfg5.npz", pairs=ks, values=values, anomalous=data["anomalous"][ks])
     return {"inputs_sha256": sha256_inputs(data), "pairs": int(len(ks)), "anomalous": int(data["anomalous"][ks].sum())}
 
@@ -173,6 +192,7 @@ def main():
     ap.add_argument("--state-dir", default="/tmp/sdtw_fullsize_refs")
     ap.add_argument("--only", choices=["base", "pert"], default=None,
                     help="compute only one of the two descents of a config into --state-dir (no output file is written)")
+    ap.add_argument("--cfg5-all", action="store_true", help="cfg 5: all N values instead of the 64-pair sample")
     args = ap.parse_args()
     oracle.build()
     meta_path = HERE / "fullsize_refs.json"

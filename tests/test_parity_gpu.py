@@ -7,8 +7,9 @@ Tolerances (BASELINE.json north_star):
                     the cancellation, not the arithmetic)
   summed gradient : ||G - G*||_2 <= 2e-3 ||G*||_2, and max_j |G_j - G*_j| <= 2e-3 max_j |G*_j| (a fault confined to
                     one strip-boundary column is invisible to the L2 norm); the worst column modulo 128 is printed
-  barycenter      : ||Z - Z*||_2 <= 2e-3 ||Z*||_2 after the configured iterations, and ||Z - Z*|| <= 5e-2 ||Z* - Z0||
-                    (error relative to the distance moved; the first one is nearly vacuous when Z barely moves)
+  barycenter      : ||Z - Z*||_2 <= 2e-3 ||Z*||_2 after the configured iterations, and ||Z - Z*|| <= 2e-3 ||Z* - Z0||
+                    (error relative to the distance moved; the first one is nearly vacuous when Z barely moves: at
+                    cfg 4 the descent moves Z by 8.7e-4 of its norm, so there the second bound is the one that holds)
 """
 import dataclasses
 import os
@@ -22,7 +23,7 @@ pytestmark = pytest.mark.gpu
 
 VAL_TOL, GRAD_TOL, BARY_TOL = 1e-4, 2e-3, 2e-3
 GRAD_MAX_TOL = 2e-3          # max-norm companion of the gradient bar
-MOVED_TOL = 5e-2             # barycenter error relative to the distance moved
+MOVED_TOL = 2e-3             # barycenter error relative to the distance moved
 STRICT_FLOOR = 0.05          # strict value ratio asserted where |v*| >= STRICT_FLOOR * gamma (n + m)
 
 
@@ -249,12 +250,14 @@ def test_waves_of_pairs_when_the_workspace_budget_is_small(B):
     step = 0.02 / cfg.N
     Zb0, vb0, ob0 = B.sdtw_barycenter(Z.clone(), X, data["offsets"], cfg.gamma, 3, step)
     vf0, _ = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
+    assert B.sdtw_last_wave_count() == 1                     # unsplit so far (include/sdtw_debug.h)
     need = B.sdtw_workspace_bytes(cfg.m, cfg.d, data["offsets"], True)
     n0 = B.sdtw_launch_count()
     try:
         B.sdtw_set_workspace_limit(need // 3)
         v1, g1, o1 = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, weights=w)
         launches = B.sdtw_launch_count() - n0
+        assert B.sdtw_last_wave_count() >= 4                 # the split is silent, but it can be observed
         Zb1, vb1, ob1 = B.sdtw_barycenter(Z.clone(), X, data["offsets"], cfg.gamma, 3, step)
         B.sdtw_set_workspace_limit(B.sdtw_workspace_bytes(cfg.m, cfg.d, data["offsets"], False) // 2)
         vf1, _ = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma, want_grad=False)
@@ -271,6 +274,40 @@ def test_waves_of_pairs_when_the_workspace_budget_is_small(B):
     moved = float(torch.linalg.norm(Zb0 - Z))
     assert float(torch.linalg.norm(Zb1 - Zb0)) <= 1e-5 * moved
     assert torch.allclose(ob1, ob0, rtol=1e-6) and torch.allclose(vb1, vb0, rtol=1e-6, atol=0)
+
+
+def test_more_than_256_pairs_unforced_throughput_reverse_kernel(B, oracle):
+    """300 cycles of cfg 2's shape: above LATENCY_KERNEL_MAX_PAIRS (sdtw.cu) the reverse pass is backward_kernel by the
+    library's own choice (no sdtw_set_reverse_kernel); values and summed gradient against the oracle."""
+    cfg = dataclasses.replace(synth.CONFIGS[2], N=300, name="300 pairs of cfg 2's shape")
+    data = synth.make(cfg)
+    B.sdtw_set_reverse_kernel(-1)
+    run_value_grad(B, oracle, data, cfg.name, mode="full")
+
+
+def test_one_pair_per_wave_more_waves_than_cached_plans(B):
+    """40 pairs under a budget that holds one pair at a time: 40 waves, more than the 32 plans the cache used to keep
+    (every wave of every iteration then re-allocated its plan).  Same values bit for bit, same descent to round-off."""
+    import torch
+    cfg = synth.scaled(synth.CONFIGS[2], 0.5, N=40)
+    data = synth.make(cfg)
+    Z, X = _dev(data["Z0"]), _dev(data["X"])
+    v0, g0 = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+    Zb0, vb0, ob0 = B.sdtw_barycenter(Z.clone(), X, data["offsets"], cfg.gamma, 4, cfg.step)
+    longest = int(np.argmax(data["lengths"]))
+    one = B.sdtw_workspace_bytes(cfg.m, cfg.d, np.array([0, data["lengths"][longest]], np.int64), True)
+    try:
+        B.sdtw_set_workspace_limit(one + one // 8)
+        v1, g1 = B.sdtw_value_grad(Z, X, data["offsets"], cfg.gamma)
+        assert B.sdtw_last_wave_count() == cfg.N
+        Zb1, vb1, ob1 = B.sdtw_barycenter(Z.clone(), X, data["offsets"], cfg.gamma, 4, cfg.step)
+        assert B.sdtw_last_wave_count() == cfg.N
+    finally:
+        B.sdtw_set_workspace_limit(0)
+    assert torch.equal(v0, v1)
+    assert rel_l2(g1.cpu().numpy(), g0.cpu().numpy()) <= 1e-6
+    assert float(torch.linalg.norm(Zb1 - Zb0)) <= 1e-5 * float(torch.linalg.norm(Zb0 - Z))
+    assert torch.allclose(ob1, ob0, rtol=1e-6)
 
 
 def test_argument_errors_leave_outputs_untouched(B):
