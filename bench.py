@@ -30,7 +30,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2404_12134_b200 import synth  # noqa: E402
+from paper_2404_12134_b200 import paper_setup, synth  # noqa: E402
 
 METRIC = "sdtw_fwd_bwd_dp_cells_per_s"
 UNIT = "cells/s"
@@ -229,8 +229,8 @@ def run_ours(args):
     dense = args.reverse == "dense"
     B.sdtw_set_reverse_mode(dense)
     if table3:
-        weights = B.eq7_weights(data["lengths"])
-        band = B.table1_band(cfg.m, data["lengths"])
+        weights = paper_setup.eq7_weights(data["lengths"])
+        band = paper_setup.table1_band(cfg.m, data["lengths"])
 
     Z = Z0.clone()
     G = torch.empty_like(Z)
@@ -526,8 +526,8 @@ def run_table3(args):
     data = synth.make(cfg)
     Z0 = torch.from_numpy(data["Z0"]).cuda()
     X = torch.from_numpy(data["X"]).cuda()
-    w = B.eq7_weights(data["lengths"])
-    band = B.table1_band(cfg.m, data["lengths"])
+    w = paper_setup.eq7_weights(data["lengths"])
+    band = paper_setup.table1_band(cfg.m, data["lengths"])
     step0 = 1.0 / float(np.sum(w))                      # first trial step of the steepest-descent iteration
     def optimise():
         Z = Z0.clone()

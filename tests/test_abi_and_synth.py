@@ -39,18 +39,24 @@ def test_library_exports_every_declared_symbol(binding):
     assert both == set(binding.SYMBOLS), both ^ set(binding.SYMBOLS)
 
 
-def test_binding_helpers_eq7_weights_and_table1_band(binding):
-    """binding.eq7_weights / table1_band against numbers written out by hand from eq. 7 (lambda_i / m_i,
-    lambda = 1 by default) and Table 1 (bandwidth = 0.6 x the longest signal length)."""
-    w = binding.eq7_weights([4, 8, 5])
+def test_paper_setup_helpers_eq7_weights_table1_band_default_length(binding):
+    """paper_setup.eq7_weights / table1_band / default_barycenter_length against numbers written out by hand from eq. 7
+    (lambda_i / m_i, lambda = 1 by default), Table 1 (bandwidth = 0.6 x the
+    longest signal length) and "by default m_b = max m_i".  They live outside binding.py, which only
+    marshals arguments and does not import them."""
+    from paper_2404_12134_b200 import paper_setup
+    assert not any(hasattr(binding, n) for n in ("eq7_weights", "table1_band", "segment_cycles", "paper_setup"))
+    assert paper_setup.default_barycenter_length([27000, 33000, 31000]) == 33000
+    assert paper_setup.default_barycenter_length(np.array([5])) == 5
+    w = paper_setup.eq7_weights([4, 8, 5])
     assert w.dtype == np.float32 and np.array_equal(w, np.array([0.25, 0.125, 0.2], np.float32))
-    w = binding.eq7_weights([4, 8, 5], lam=[2.0, 1.0, 0.5])
+    w = paper_setup.eq7_weights([4, 8, 5], lam=[2.0, 1.0, 0.5])
     assert np.array_equal(w, np.array([0.5, 0.125, 0.1], np.float32))
-    assert binding.table1_band(30000, [27000, 33000, 31000]) == 19800         # 0.6 x 33000
-    assert binding.table1_band(30000, [27000, 28000]) == 18000                # the barycenter is the longest: 0.6 x 30000
-    assert binding.table1_band(18385, [18385] * 5) == 11031                   # Table 3's length: floor(11031.0)
-    assert binding.table1_band(1001, [1001], 0.25) == 250                     # floor(250.25)
-    assert binding.table1_band(10, [10], 1.0) == 10
+    assert paper_setup.table1_band(30000, [27000, 33000, 31000]) == 19800         # 0.6 x 33000
+    assert paper_setup.table1_band(30000, [27000, 28000]) == 18000                # the barycenter is the longest: 0.6 x 30000
+    assert paper_setup.table1_band(18385, [18385] * 5) == 11031                   # Table 3's length: floor(11031.0)
+    assert paper_setup.table1_band(1001, [1001], 0.25) == 250                     # floor(250.25)
+    assert paper_setup.table1_band(10, [10], 1.0) == 10
 
 
 def test_status_strings_and_tile_info(binding):

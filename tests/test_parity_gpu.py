@@ -17,7 +17,7 @@ import os
 import numpy as np
 import pytest
 
-from paper_2404_12134_b200 import synth
+from paper_2404_12134_b200 import paper_setup, synth
 
 pytestmark = pytest.mark.gpu
 
@@ -245,7 +245,7 @@ def test_waves_of_pairs_when_the_workspace_budget_is_small(B):
     cfg = synth.scaled(synth.CONFIGS[4], 0.1, N=13)
     data = synth.make(cfg)
     Z, X = _dev(data["Z0"]), _dev(data["X"])
-    w = B.eq7_weights(data["lengths"])
+    w = paper_setup.eq7_weights(data["lengths"])
     v0, g0, o0 = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, weights=w)
     step = 0.02 / cfg.N
     Zb0, vb0, ob0 = B.sdtw_barycenter(Z.clone(), X, data["offsets"], cfg.gamma, 3, step)
@@ -544,12 +544,12 @@ def test_band_and_weights_value_grad(B, oracle, idx, scale, N, frac):
     data = synth.make(cfg)
     lens = data["lengths"]
     band = int(np.floor(frac * max(cfg.m, int(lens.max()))))     # Table 1: a fraction of the longest length
-    assert band == B.table1_band(cfg.m, lens, frac)
+    assert band == paper_setup.table1_band(cfg.m, lens, frac)
     assert band >= np.abs(lens - cfg.m).max() and band < min(cfg.m, lens.min()) - 1      # feasible, and it excludes cells
     rng = np.random.default_rng(idx)
     lam = rng.uniform(0.5, 2.0, size=N)
     w = (lam / lens).astype(np.float32)                           # eq. 7: lambda_k / n_k
-    assert np.array_equal(w, B.eq7_weights(lens, lam=lam))
+    assert np.array_equal(w, paper_setup.eq7_weights(lens, lam=lam))
     Z, X = _dev(data["Z0"]), _dev(data["X"])
     vals, G, obj = B.sdtw_value_grad_ex(Z, X, data["offsets"], cfg.gamma, weights=w, band=band)
     torch.cuda.synchronize()
@@ -575,7 +575,7 @@ def test_band_barycenter_weighted_descent(B, oracle):
     lens = data["lengths"]
     band = int(np.floor(0.6 * max(cfg.m, int(lens.max()))))      # Table 1 / eq. 7 restated here, not taken from the binding
     w = (1.0 / lens).astype(np.float32)
-    assert band == B.table1_band(cfg.m, lens, 0.6) and np.array_equal(w, B.eq7_weights(lens))
+    assert band == paper_setup.table1_band(cfg.m, lens, 0.6) and np.array_equal(w, paper_setup.eq7_weights(lens))
     step = 0.02 / cfg.N * float(np.mean(lens))                # eq. 7 divides by n_k: rescale the step accordingly
     iters = 3
     Z, vals, obj = B.sdtw_barycenter_ex(_dev(data["Z0"]), _dev(data["X"]), data["offsets"], cfg.gamma, iters, step,
@@ -639,7 +639,7 @@ def test_band_dense_reverse_and_schedule_are_bitwise_neutral(B):
     import torch
     cfg = synth.scaled(synth.CONFIGS[4], 0.1, N=6)
     data = synth.make(cfg)
-    band = B.table1_band(cfg.m, data["lengths"], 0.3)
+    band = paper_setup.table1_band(cfg.m, data["lengths"], 0.3)
     Z, X = _dev(data["Z0"]), _dev(data["X"])
     for kernel in (0, 1):
         try:
@@ -920,11 +920,11 @@ def test_segment_cycles_loop_matches_oracle_driven_loop(B, oracle):
         cyc = data["X"][data["offsets"][k]:data["offsets"][k + 1]]
         parts.append(cyc); truth.append((pos, pos + len(cyc) - 1)); pos += len(cyc)
     Y = np.concatenate(parts).astype(np.float32)
-    got = B.segment_cycles(_dev(Y), _dev(ref))
+    got = paper_setup.segment_cycles(_dev(Y), _dev(ref))
     def oracle_sub(r, w):
         v, a, b = oracle.subdtw_f32(r, w, np.array([0, len(w)]))
         return float(v[0]), int(a[0]), int(b[0])
-    want = B.segment_cycles(Y, ref, subdtw=oracle_sub)
+    want = paper_setup.segment_cycles(Y, ref, subdtw=oracle_sub)
     assert got == want
     print(f"[segmentation] {len(got)} cycles found: {[(s, e) for s, e, _ in got]}; built from {truth}")
     # every found cycle lies inside one of the cycles the stream was built from, and most of those are found
