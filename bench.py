@@ -37,26 +37,40 @@ UNIT = "cells/s"
 # roofline constants: MUFU (ex2/lg2/rcp) results per clock per SM on sm_100, SM count, max clock
 MUFU_PER_CLK_PER_SM = 16
 ALGO_MUFU_FWD, ALGO_MUFU_BWD = 3, 3          # algorithmic special-function evaluations per cell (2 ex2 + lg2; 3 ex2)
-PROFILE_ROUNDS = ("r2", "r1e")                # newest first: profiles/<round>_<kernel>_cfg<idx>[_<variant>]_full.txt
+PROFILE_ROUNDS = ("r3", "r2", "r1e")          # newest first: profiles/<round>_<kernel>_cfg<idx>[_<variant>]_full.txt
+STALE_TOL = 0.05                              # a capture whose kernel time differs from this run's by more is not used
 
 
-def ncu_traffic(kernel, cfg_index, variant=""):
+def ncu_traffic(kernel, cfg_index, variant="", kernel_ms=None):
     """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of `kernel` on config `cfg_index`, read from the
-    header of the committed `ncu --set full` summary under profiles/ (the "# raw:" lines); (None, None) when no
-    capture of that kernel / workload is committed."""
+    header of the committed `ncu --set full` summary under profiles/ (the "# raw:" lines).  The capture is tied to the
+    kernel that was timed by its own gpu__time_duration: if that differs from this run's CUDA-event time of the kernel
+    (`kernel_ms`) by more than STALE_TOL, the kernel has changed since the capture and the file is refused.
+    Returns (bytes or None, path or None, note)."""
+    note = "no committed capture of this kernel / workload"
     for rnd in PROFILE_ROUNDS:
         path = os.path.join(ROOT, "profiles", f"{rnd}_{kernel}_cfg{cfg_index}{'_' + variant if variant else ''}_full.txt")
         if not os.path.exists(path):
             continue
-        tot, seen = 0.0, 0
+        tot, seen, dur, commit = 0.0, 0, None, None
         for ln in open(path):
             f = ln.split()
             if len(f) == 5 and f[:2] == ["#", "raw:"] and f[2] in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
                 tot += float(f[4]) * {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}[f[3]]
                 seen += 1
-        if seen == 2:
-            return int(tot), os.path.relpath(path, ROOT)
-    return None, None
+            if len(f) == 5 and f[:3] == ["#", "raw:", "gpu__time_duration.sum"]:
+                dur = float(f[4]) * {"s": 1e3, "ms": 1.0, "us": 1e-3, "ns": 1e-6}.get(f[3], float("nan"))
+            if len(f) >= 3 and f[:2] == ["#", "commit:"]:
+                commit = f[2]
+        rel = os.path.relpath(path, ROOT)
+        if seen != 2:
+            continue
+        if kernel_ms is not None and dur is not None and abs(dur - kernel_ms) > STALE_TOL * kernel_ms:
+            note = f"{rel} refused: its launch took {dur:.2f} ms, this run's {kernel_ms:.2f} ms (kernel changed since the capture)"
+            continue
+        return int(tot), rel, (f"capture at commit {commit}, " if commit else "") + (
+            f"launch {dur:.2f} ms under ncu vs {kernel_ms:.2f} ms here" if dur is not None and kernel_ms is not None else "duration not recorded")
+    return None, None, note
 
 
 def workload_string(cfg):
@@ -177,6 +191,86 @@ def run_reference(args):
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
+
+
+# ---------------------------------------------------------------------------------------------- secondary workloads
+def measure_secondary(B, torch, dev, data4, mufu_peak, sms, sm_max_hz):
+    """The other workloads BASELINE.md section 5 quotes, measured in this process after the headline region (device-
+    resident inputs, CUDA events, one warm-up pass each; kernel times from the library's own event brackets):
+    cfg 5 forward-only scoring sweep, cfg 3 descent, cfg 4 with the dense reverse pass, cfg 5 d_score."""
+    def timed(fn, reps):
+        fn()                                                    # warm-up (first call of a shape also uploads its plan)
+        torch.cuda.synchronize()
+        B.sdtw_profile_enable(True)
+        B.sdtw_profile_read()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        prof = B.sdtw_profile_read()
+        B.sdtw_profile_enable(False)
+        n = max(prof["evaluations"], 1)
+        return e0.elapsed_time(e1) / reps, {"forward": prof["ms_forward"] / n, "reverse": prof["ms_backward"] / n,
+                                            "other": prof["ms_other"] / n}
+
+    def up(a):
+        return torch.from_numpy(a).to(dev)
+
+    out = {"note": "measured after the headline region in the same process; 1 warm-up + the stated repetitions; "
+                   "frac = algorithmic special functions (3 per forward cell, 3 per reverse cell) / kernel time / MUFU peak"}
+    # cfg 5: forward-only scoring sweep (rings)
+    d5 = synth.make(5)
+    c5, cells5 = d5["cfg"], synth.cells(d5)
+    Z5, X5 = up(d5["Z0"]), up(d5["X"])
+    v5 = torch.empty(c5.N, dtype=torch.float32, device=dev)
+    ms, k = timed(lambda: B.sdtw_value_grad(Z5, X5, d5["offsets"], c5.gamma, out_values=v5, want_grad=False), 2)
+    out["cfg5_forward_only"] = {"workload": workload_string(c5), "reps": 2, "ms_per_step": ms, "value": cells5 / (ms * 1e-3),
+                                "unit": UNIT, "kernel_ms": k, "forward_frac": ALGO_MUFU_FWD * cells5 / (k["forward"] * 1e-3) / mufu_peak,
+                                "workspace_gb": B.sdtw_workspace_bytes(c5.m, c5.d, d5["offsets"], False) / 1e9,
+                                "finite": bool(torch.isfinite(v5).all().item())}
+    # cfg 5: d_score (eq. 8), the DTW kernel; bound = instruction issue
+    ms, _ = timed(lambda: B.sdtw_dtw_score(Z5, X5, d5["offsets"]), 2)
+    algo = 6 + 2 * c5.d
+    out["cfg5_dtw_score"] = {"workload": workload_string(c5) + "; op = sdtw_dtw_score (eq. 8)", "reps": 2, "ms_per_step": ms,
+                             "value": cells5 / (ms * 1e-3), "unit": UNIT,
+                             "frac": algo * cells5 / (ms * 1e-3) / (128.0 * sms * sm_max_hz),
+                             "frac_note": f"{algo} thread-instructions per cell the recurrence needs / (128 per clk per SM x {sms} SMs x "
+                                          f"{sm_max_hz / 1e6:.0f} MHz)"}
+    del Z5, X5
+    # cfg 3: the configured descent (10 iterations, d = 4)
+    d3 = synth.make(3)
+    c3, cells3 = d3["cfg"], synth.cells(d3)
+    Z30, X3 = up(d3["Z0"]), up(d3["X"])
+    Z3 = Z30.clone()
+
+    def cfg3_descent():
+        Z3.copy_(Z30)
+        B.sdtw_barycenter(Z3, X3, d3["offsets"], c3.gamma, c3.iters, c3.step)
+    ms, k = timed(cfg3_descent, 2)
+    out["cfg3"] = {"workload": workload_string(c3), "reps": 2, "ms_per_step": ms / c3.iters, "value": cells3 / (ms / c3.iters * 1e-3),
+                   "unit": UNIT, "kernel_ms": k, "forward_frac": ALGO_MUFU_FWD * cells3 / (k["forward"] * 1e-3) / mufu_peak,
+                   "finite": bool(torch.isfinite(Z3).all().item()),
+                   "note": "few pairs (32) of 10k: a latency chain per pair, not a throughput case (DESIGN.md 5.4)"}
+    # cfg 4 with the dense reverse pass (every reverse cell visited: backward_kernel)
+    c4, cells4 = data4["cfg"], synth.cells(data4)
+    Z40, X4 = up(data4["Z0"]), up(data4["X"])
+    Z4 = Z40.clone()
+    B.sdtw_set_reverse_mode(True)
+    try:
+        def cfg4_dense():
+            Z4.copy_(Z40)
+            B.sdtw_barycenter(Z4, X4, data4["offsets"], c4.gamma, 1, c4.step)
+        ms, k = timed(cfg4_dense, 2)
+    finally:
+        B.sdtw_set_reverse_mode(False)
+    out["cfg4_reverse_dense"] = {"workload": workload_string(c4) + "; reverse pass visits every cell", "reps": 2, "ms_per_step": ms,
+                                 "value": cells4 / (ms * 1e-3), "unit": UNIT, "kernel_ms": k,
+                                 "forward_frac": ALGO_MUFU_FWD * cells4 / (k["forward"] * 1e-3) / mufu_peak,
+                                 "reverse_frac": ALGO_MUFU_BWD * cells4 / (k["reverse"] * 1e-3) / mufu_peak,
+                                 "step_frac": (ALGO_MUFU_FWD + ALGO_MUFU_BWD) * cells4 / (ms * 1e-3) / mufu_peak}
+    return out
 
 
 # ---------------------------------------------------------------------------------------------- our arm
@@ -381,15 +475,33 @@ def run_ours(args):
         else:
             dom, t_dom, achieved = "backward_kernel", t_bwd, ALGO_MUFU_BWD * visited_cells / t_bwd
         variant = ("dense" if dense else "") if not args.gamma else f"gamma{args.gamma:g}"
-        traffic, traffic_src = (None, None) if (world > 1 or table3) else ncu_traffic(dom, cfg.index, variant)
+        traffic, traffic_src, traffic_note = ((None, None, "not read for this run") if (world > 1 or table3) else
+                                              ncu_traffic(dom, cfg.index, variant, t_dom * 1e3))
         algo_total = ALGO_MUFU_FWD + (0 if forward_only else ALGO_MUFU_BWD)
+        # SURVEY.md 8(d), "HBM (algorithmic bytes)": inputs 4 d (n_k + m) per pair + strips 8/T per cell (T = strip
+        # width; written by the forward pass, read back by the reverse pass) + per-pair gradient partials 4 m d
+        T_strip = tile["strip_cols"]
+        rows_local = int(data["lengths"].sum())
+        algo_bytes = {"inputs": 4 * cfg.d * (rows_local + Nl * cfg.m),
+                      "strips": 0 if forward_only else int(8 * ncells_local / T_strip),
+                      "partials": 0 if forward_only else 4 * Nl * cfg.m * cfg.d}
+        algo_bytes_total = int(sum(algo_bytes.values()))
+        own_work = ALGO_MUFU_FWD * ncells_local + (0 if forward_only else ALGO_MUFU_BWD * visited_cells)
         roofline = {
             "bound": "alu", "kernel": dom, "achieved": achieved / 1e9, "peak": mufu_peak / 1e9, "unit": "GMUFU-op/s",
             "frac": achieved / mufu_peak,
-            "traffic": traffic, "traffic_source": traffic_src,
-            "algorithmic_bytes": None if forward_only else int(ncells_local * 0.375 + ncells_local * 4 / 128),
-            "algorithmic_bytes_note": "checkpoint records (0.375 B/cell) + strip-boundary column (4/128 B/cell) written by one "
-                                      "forward launch: this design's checkpoint volume (DESIGN.md 5.5)",
+            "traffic": traffic, "traffic_source": traffic_src, "traffic_note": traffic_note,
+            "algorithmic_bytes": algo_bytes_total, "algorithmic_bytes_parts": algo_bytes,
+            "algorithmic_bytes_note": f"SURVEY.md 8(d): inputs 4 d (sum n_k + N m) + strips 8/T B per cell at the built strip width "
+                                      f"T = {T_strip} + gradient partials 4 N m d, per evaluation",
+            "traffic_ratio": (traffic / algo_bytes_total) if traffic else None,
+            "design_checkpoint_bytes": None if forward_only else int(ncells_local * 0.375 + ncells_local * 4 / 128),
+            "design_checkpoint_bytes_note": "what THIS design's forward launch writes: warp-state records every 8 steps (0.375 B/cell) "
+                                            "+ strip-boundary column (4/128 B/cell), DESIGN.md 5.5; the reverse pass reads back only "
+                                            "the records of the chunks it visits",
+            "step_frac_own_work": (own_work / (ms_step * 1e-3) / mufu_peak) if world == 1 else None,
+            "step_frac_own_work_note": "whole step: (3 special functions per forward cell + 3 per VISITED reverse cell) / step "
+                                       "time / MUFU peak",
             "peak_source": "measured live: dependent ex2 / lg2 / rcp chains on every SM (sdtw_measure_mufu_peak), the slowest "
                            "of the three; MEASURED_PEAKS.json holds no ALU figure (DESIGN.md section 8)",
             "peak_derived": mufu_derived / 1e9,
@@ -407,6 +519,9 @@ def run_ours(args):
                 "cell (3 forward + 3 reverse); NOT a roofline fraction when the reverse pass skips cells: see reverse.visited_frac_of_cells",
             "checkpoint_hbm_gbs": None if forward_only else (2 * ws_bytes) / max(t_fwd + t_bwd, 1e-9) / 1e9,
         }
+        secondary = None
+        if (world == 1 and not args.skip_secondary and args.config == 4 and not table3 and args.gamma is None and not dense):
+            secondary = measure_secondary(B, torch, dev, data, mufu_peak, sms, sm_max_hz)
         cpu = None if args.skip_cpu else time_oracle(data)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -427,7 +542,7 @@ def run_ours(args):
                        "tile": tile},
             "barycenter_iter_s": ms_step * 1e-3,
             "objective": objective, "finite": finite,
-            "roofline": roofline, "cpu_baseline": cpu,
+            "roofline": roofline, "secondary": secondary, "cpu_baseline": cpu,
             "e2e": e2e,
             "gpu_launches": int(launches), "clocks": clocks,
         }
@@ -575,6 +690,8 @@ def main():
                     help="N > 1: weak = every rank its own pairs; strong = one problem partitioned by dist.partition_pairs")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs only: leave out the host-buffer leg")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs only: leave out the timed oracle leg")
+    ap.add_argument("--skip-secondary", action="store_true",
+                    help="leave out the secondary workloads (cfg 5 scoring / d_score, cfg 3, dense reverse) of the default line")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
