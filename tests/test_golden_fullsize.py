@@ -46,7 +46,11 @@ def test_golden_hashes_match_inputs_and_oracle_source(idx):
     assert float(gold["step"]) == cfg.step and int(gold["iters"]) == cfg.iters
     last = meta["contractivity"][-1]
     assert last["step"] == cfg.step and last["rel_out"] <= 1e-4 and abs(last["rel_in"] - 1e-6) < 5e-7
-    assert all(t["rel_out"] > 1e-4 for t in meta["contractivity"][:-1])       # every larger step tried had failed it
+    # Records before the last one, if the script had to halve the step, are failures of the check.  Today both configs
+    # hold ONE record, the frozen step's: the larger steps were screened out with the CUDA path before any oracle time
+    # was spent (C12 / C13), so "the first step that passes" is not an oracle-evidenced claim and is not made.
+    assert len(meta["contractivity"]) >= 1
+    assert all(t["rel_out"] > 1e-4 and t["step"] > cfg.step for t in meta["contractivity"][:-1])
     assert gold["grad0"].shape == (cfg.m, cfg.d) and gold["Z_final"].shape == (cfg.m, cfg.d)
     assert gold["values0"].shape == (cfg.N,) and len(gold["objective"]) == cfg.iters
     assert np.all(np.isfinite(gold["Z_final"])) and np.all(np.isfinite(gold["grad0"]))
