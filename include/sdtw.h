@@ -30,6 +30,14 @@
  *   - d is supported for 1 <= d <= SDTW_MAX_D (compiled maximum; SDTW_DTW_MAX_D for sdtw_dtw_score / sdtw_subdtw);
  *     1 <= n_k, m < 2^30; 1 <= N < 2^24.
  *   - There is no CPU fallback: on a device that is not compute capability 10.x the calls return SDTW_ERR_UNSUPPORTED.
+ *   - CO-RESIDENCY.  The forward, reverse and DTW kernels are persistent grids sized by the occupancy query so that every
+ *     CTA is resident at once; a CTA that waits for a strip-boundary value spins (with nanosleep back-off) on data words
+ *     another resident CTA writes.  That holds when the library has the SMs it was promised: a whole GPU, or a MIG
+ *     slice.  Where the CTAs of one grid may NOT all be resident -- another process time-slicing or sharing the SMs
+ *     through MPS with a limited active-thread percentage, a debugger single-stepping a CTA, a concurrent kernel of the
+ *     caller's that occupies SMs for as long as this grid waits for them -- a waiting CTA can wait for one that is not
+ *     scheduled, and the call then does not return: there is no time-out in the wait loops and no SDTW_ERR_* for this.
+ *     Kernels of the caller that merely run to completion beside the library's only delay it.
  */
 #ifndef SDTW_H_
 #define SDTW_H_
