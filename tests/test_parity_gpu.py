@@ -999,6 +999,34 @@ def test_lbfgs_descent_matches_oracle(B, oracle, idx, scale, N, iters, hist, ste
     check_values(vals.cpu().numpy(), vo, data["lengths"], cfg, f"{cfg.name} values at the final Z (L-BFGS)")
 
 
+def test_line_search_descents_in_the_throughput_regime(B, oracle):
+    """The line-search calls on a problem with more strips than resident forward warps (150 pairs x 33 strips against
+    148 SMs x 32 warps), where the forward kernel hands out CTA-full units with small tail units instead of one strip
+    per unit: backtracking and L-BFGS against the float64 oracle, as in the small cases above."""
+    import torch
+    cfg = dataclasses.replace(synth.CONFIGS[2], N=150, n_lo=500, n_hi=600, m=4100, name="150 short cycles vs m = 4100")
+    data = synth.make(cfg)
+    strips = -(-cfg.m // B.sdtw_tile_info()["strip_cols"]) * cfg.N
+    assert strips > torch.cuda.get_device_properties(0).multi_processor_count * 32
+    Z0, X = _dev(data["Z0"]), _dev(data["X"])
+    scale_f = np.sum(cfg.gamma * (data["lengths"] + cfg.m))
+    step0 = 4e-3
+    for name, run_gpu, run_cpu in (
+            ("backtracking", lambda: B.sdtw_barycenter_backtracking(Z0.clone(), X, data["offsets"], cfg.gamma, 3, step0),
+             lambda: oracle.barycenter_backtracking(data["Z0"], data["X"], data["offsets"], cfg.gamma, 3, step0, mode="checkpointed")),
+            ("L-BFGS", lambda: B.sdtw_barycenter_lbfgs(Z0.clone(), X, data["offsets"], cfg.gamma, 3, 3, step0),
+             lambda: oracle.barycenter_lbfgs(data["Z0"], data["X"], data["offsets"], cfg.gamma, 3, 3, step0, mode="checkpointed"))):
+        Z, vals, obj, steps, trials = run_gpu()
+        Zo, vo, oo, so, to = run_cpu()
+        print(f"[{cfg.name}, {name}] steps {steps.tolist()} (oracle {so.tolist()}), trials {trials.tolist()} ({to.tolist()}), "
+              f"objective {obj.tolist()} (oracle {oo.tolist()})")
+        assert np.array_equal(trials, to) and np.allclose(steps, so, rtol=1e-6)
+        assert np.all(np.diff(obj) < 0)
+        assert np.all(np.abs(obj - oo) <= 1e-4 * np.maximum(np.abs(oo), scale_f))
+        check_barycenter(Z.cpu().numpy(), Zo, data["Z0"], f"{cfg.name}, {name}")
+        check_values(vals.cpu().numpy(), vo, data["lengths"], cfg, f"{cfg.name}, {name}: values at the final Z")
+
+
 def test_lbfgs_without_history_is_the_backtracking_descent(B):
     import torch
     data = synth.make(2)
