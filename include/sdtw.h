@@ -251,8 +251,10 @@ int sdtw_barycenter_host(float* Z_inout, int64_t m, int32_t d, const float* X_co
  * workspace, else what the device has free -- sdtw_value_grad[_ex] and sdtw_barycenter[_ex] evaluate the pair set as
  * consecutive waves of pairs in the same workspace (pairs are independent): per-pair values are bitwise
  * the same, the gradients of the waves are added in wave order (float32 round-off against the unsplit call).  Only when
- * a single pair does not fit the budget: SDTW_ERR_WORKSPACE.  (sdtw_barycenter_backtracking, sdtw_barycenter_lbfgs and the
- * DTW calls do not split: they return SDTW_ERR_WORKSPACE when a registered workspace is too small.)  A split is silent;
+ * a single pair does not fit the budget: SDTW_ERR_WORKSPACE.  sdtw_dtw_score and sdtw_subdtw split the same way (against
+ * sdtw_dtw_workspace_bytes; every output is per pair, so every bit is that of the unsplit call).  The two line-search
+ * calls (sdtw_barycenter_backtracking, sdtw_barycenter_lbfgs) do NOT split -- an accepted trial's reverse sweep reuses the
+ * checkpoints of all pairs -- and return SDTW_ERR_WORKSPACE when a registered workspace is too small.  A split is silent;
  * with the library-owned buffer the budget is the device's free memory at the time of the call, so a co-tenant that
  * holds memory (a caching allocator) makes calls split into more waves: sdtw_last_wave_count() (sdtw_debug.h) tells.
  * THREADS.  Calls are serialised by one library lock while they enqueue.  The two line-search calls (backtracking,

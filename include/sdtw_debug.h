@@ -25,7 +25,7 @@ extern "C" {
  *                         evaluations they cover; clears the accumulators.  Any pointer may be NULL.
  */
 uint64_t sdtw_launch_count(void);
-/* Waves of pairs (sdtw.h, "WAVES") the calling thread's last sdtw_value_grad[_ex] / sdtw_barycenter[_ex] call was
+/* Waves of pairs (sdtw.h, "WAVES") the calling thread's last sdtw_value_grad[_ex] / sdtw_barycenter[_ex] / DTW call was
  * evaluated in: 1 = unsplit, 0 = no such call yet.  A call that splits does so silently (same values); a caller that
  * shares the GPU with a caching allocator can watch this number to notice that its budget has become small. */
 int sdtw_last_wave_count(void);

@@ -688,13 +688,13 @@ size_t workspace_budget(int dev, size_t need) {
 // bounds of the waves (bounds[0] = 0 < ... < bounds[W] = N) such that every wave's layout fits `budget`; *max_bytes =
 // the largest of them.  SDTW_ERR_WORKSPACE if a single pair does not fit.
 int plan_waves(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool want_grad, int ring_sms, size_t budget,
-               std::vector<int>& bounds, size_t* max_bytes) {
+               std::vector<int>& bounds, size_t* max_bytes, int vs_words = 1) {
     // the split of the last problem is remembered (a descent loop asks for the same one every iteration; under g_mutex)
-    struct Memo { int64_t m = 0; int32_t d = 0, N = 0; bool want_grad = false; int ring_sms = 0; size_t budget = 0, max_bytes = 0;
+    struct Memo { int64_t m = 0; int32_t d = 0, N = 0; bool want_grad = false; int ring_sms = 0, vs_words = 0; size_t budget = 0, max_bytes = 0;
                   std::vector<int64_t> offsets; std::vector<int> bounds; };
     static Memo memo;
     if (memo.N == N && memo.m == m && memo.d == d && memo.want_grad == want_grad && memo.ring_sms == ring_sms &&
-        memo.budget == budget && std::memcmp(memo.offsets.data(), offsets, sizeof(int64_t) * (size_t)(N + 1)) == 0) {
+        memo.vs_words == vs_words && memo.budget == budget && std::memcmp(memo.offsets.data(), offsets, sizeof(int64_t) * (size_t)(N + 1)) == 0) {
         bounds = memo.bounds;
         *max_bytes = memo.max_bytes;
         return SDTW_OK;
@@ -713,14 +713,14 @@ int plan_waves(int64_t m, int32_t d, const int64_t* offsets, int32_t N, bool wan
             sub.assign(offsets + k0, offsets + k1 + 1);
             for (auto& o : sub) o -= offsets[k0];
             Layout L;
-            const int rc = build_layout(m, d, sub.data(), k1 - k0, want_grad, L, 1, ring_sms);
+            const int rc = build_layout(m, d, sub.data(), k1 - k0, want_grad, L, vs_words, ring_sms);
             if (rc != SDTW_OK) return rc;
             mx = std::max(mx, L.total);
             ok = L.total <= budget;
         }
         if (ok) {
             *max_bytes = mx;
-            memo.m = m; memo.d = d; memo.N = N; memo.want_grad = want_grad; memo.ring_sms = ring_sms; memo.budget = budget;
+            memo.m = m; memo.d = d; memo.N = N; memo.want_grad = want_grad; memo.ring_sms = ring_sms; memo.vs_words = vs_words; memo.budget = budget;
             memo.max_bytes = mx; memo.offsets.assign(offsets, offsets + N + 1); memo.bounds = bounds;
             return SDTW_OK;
         }
@@ -1140,6 +1140,11 @@ int sdtw_barycenter(float* Z_inout, int64_t m, int32_t d, const float* X_concat,
                               out_objective, stream_);
 }
 
+// one launch of the DTW / Sub-DTW kernel over the pairs of `offsets` (a whole call, or one wave of it) in workspace `wsp`
+static int dtw_launch(bool sub, const DeviceInfo& di, char* wsp, const float* Z, int64_t m, int32_t d, const float* X_concat,
+                      const int64_t* offsets, int32_t N, float* out_val, int32_t* out_i0, float* out_score, int32_t* out_i1,
+                      cudaStream_t stream);
+
 static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const float* X_concat, const int64_t* offsets,
                       int32_t N, float* out_val, int32_t* out_i0, float* out_score, int32_t* out_i1, void* stream_) {
     int rc = check_common(Z, m, d, X_concat, offsets, N, 1.0f, SDTW_DTW_MAX_D);
@@ -1151,12 +1156,54 @@ static int dtw_common(bool sub, const float* Z, int64_t m, int32_t d, const floa
     DeviceInfo di;
     rc = get_device(di);
     if (rc) return rc;
-    Plan* pl = nullptr;
-    rc = get_plan(di, m, d, offsets, N, nullptr, false, stream, &pl, 2, g_forward_rings);
+    // WAVES (sdtw.h): pairs are independent and every output is per pair, so a pair set whose boundary state exceeds the
+    // budget is swept as consecutive waves of pairs in the same workspace; every output bit is that of the unsplit call
+    size_t total = 0;
+    const int ring_arg = g_forward_rings == 2 ? -di.sms : (g_forward_rings ? di.sms : 0);
+    if (const Plan* hit = find_plan(di.dev, m, d, offsets, N, nullptr, false, 2, g_forward_rings)) total = hit->L.total;
+    else {
+        Layout L0;
+        rc = build_layout(m, d, offsets, N, false, L0, 2, ring_arg);
+        if (rc) return rc;
+        total = L0.total;
+    }
+    g_last_waves = 1;
+    const size_t budget = workspace_budget(di.dev, total);
+    if (total <= budget) {
+        Workspace ws;
+        rc = ws.acquire(total, di.dev, stream);
+        if (rc) return rc;
+        return dtw_launch(sub, di, ws.ptr, Z, m, d, X_concat, offsets, N, out_val, out_i0, out_score, out_i1, stream);
+    }
+    std::vector<int> bounds;
+    size_t max_bytes = 0;
+    rc = plan_waves(m, d, offsets, N, false, ring_arg, budget, bounds, &max_bytes, 2);
     if (rc) return rc;
     Workspace ws;
-    rc = ws.acquire(pl->L.total, di.dev, stream);
+    rc = ws.acquire(max_bytes, di.dev, stream);
     if (rc) return rc;
+    const int W = (int)bounds.size() - 1;
+    g_plan_cap = std::max(g_plan_cap, (size_t)W + 16);
+    g_last_waves = W;
+    std::vector<int64_t> subo;
+    for (int w = 0; w < W; ++w) {
+        const int k0 = bounds[w], k1 = bounds[w + 1];
+        subo.assign(offsets + k0, offsets + k1 + 1);
+        for (auto& o : subo) o -= offsets[k0];
+        rc = dtw_launch(sub, di, ws.ptr, Z, m, d, X_concat + offsets[k0] * d, subo.data(), k1 - k0, out_val ? out_val + k0 : nullptr,
+                        out_i0 ? out_i0 + k0 : nullptr, out_score ? out_score + k0 : nullptr, out_i1 ? out_i1 + k0 : nullptr, stream);
+        if (rc) return rc;
+    }
+    return SDTW_OK;
+}
+
+static int dtw_launch(bool sub, const DeviceInfo& di, char* wsp, const float* Z, int64_t m, int32_t d, const float* X_concat,
+                      const int64_t* offsets, int32_t N, float* out_val, int32_t* out_i0, float* out_score, int32_t* out_i1,
+                      cudaStream_t stream) {
+    Plan* pl = nullptr;
+    int rc = get_plan(di, m, d, offsets, N, nullptr, false, stream, &pl, 2, g_forward_rings);
+    if (rc) return rc;
+    struct { char* ptr; } ws{wsp};
     const Layout& L = pl->L;
     DtwParams P{};
     P.Z = Z; P.X = X_concat; P.pm = pl->d_pm;

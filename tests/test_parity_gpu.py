@@ -310,6 +310,38 @@ def test_one_pair_per_wave_more_waves_than_cached_plans(B):
     assert torch.allclose(ob1, ob0, rtol=1e-6)
 
 
+def test_dtw_and_subdtw_calls_split_into_waves_bit_for_bit(B):
+    """include/sdtw.h, WAVES: sdtw_dtw_score / sdtw_subdtw under a budget below sdtw_dtw_workspace_bytes sweep the pairs
+    in waves; DTW, path length, score, Sub-DTW value, a*, b* are those of the unsplit call bit for bit (d = 1: the
+    32-warp instantiation; d = 3: a boundary column per strip)."""
+    import torch
+    for d in (1, 3):
+        cfg = dataclasses.replace(synth.scaled(synth.CONFIGS[5], 0.05, N=30), d=d, name=f"dtw waves d={d}")
+        data = synth.make(cfg)
+        Z, X = _dev(data["Z0"]), _dev(data["X"])
+        B.sdtw_set_forward_rings(0)                        # a column per strip: a workspace that grows with the pair count
+        try:
+            ref = B.sdtw_dtw_score(Z, X, data["offsets"])
+            assert B.sdtw_last_wave_count() == 1
+            sref = B.sdtw_subdtw(Z, X, data["offsets"])
+            need = B.sdtw_dtw_workspace_bytes(cfg.m, cfg.d, data["offsets"])
+            B.sdtw_set_workspace_limit(need // 4)
+            got = B.sdtw_dtw_score(Z, X, data["offsets"])
+            assert B.sdtw_last_wave_count() >= 4
+            sgot = B.sdtw_subdtw(Z, X, data["offsets"])
+            assert B.sdtw_last_wave_count() >= 4
+            B.sdtw_set_workspace_limit(256)                # not even one pair
+            with pytest.raises(B.SdtwError) as ei:
+                B.sdtw_dtw_score(Z, X, data["offsets"])
+            assert ei.value.status == B.SDTW_ERR_WORKSPACE
+        finally:
+            B.sdtw_set_workspace_limit(0)
+            B.sdtw_set_forward_rings(1)
+        torch.cuda.synchronize()
+        for a, b in zip(ref + sref, got + sgot):
+            assert torch.equal(a, b)
+
+
 def test_argument_errors_leave_outputs_untouched(B):
     import torch
     data = synth.make(1)
