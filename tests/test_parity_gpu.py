@@ -468,9 +468,10 @@ def test_cfg4_full_all_pairs_gradient_and_descent(B):
 
 
 @pytest.mark.timeout(1500)
-def test_cfg5_64_pairs_16_anomalous_full_size(B):
-    """cfg 5 (1000 cycles of 20-40k samples against m = 30000, forward only) in one call; 64 seeded pairs, 16 of them
-    anomalous, against the stored oracle values."""
+def test_cfg5_full_size_against_the_stored_oracle_values(B):
+    """cfg 5 (1000 cycles of 20-40k samples against m = 30000, forward only) in one call, against every oracle value
+    tests/golden/fullsize_cfg5.npz holds: all 1000 when it was written by `make_fullsize_refs.py --cfg5-all` (SURVEY.md
+    8(d); Step 3 of the paper, consumes every one), else the 64 seeded pairs, 16 of them anomalous."""
     import torch
     data = synth.make(5)
     cfg = data["cfg"]
@@ -481,7 +482,8 @@ def test_cfg5_64_pairs_16_anomalous_full_size(B):
     torch.cuda.synchronize()
     assert G is None and torch.isfinite(vals).all()
     v = vals.cpu().numpy()
-    check_values(v[ks], gold["values"], data["lengths"][ks], cfg, f"cfg5 full size, {len(ks)} pairs")
+    check_values(v[ks], gold["values"], data["lengths"][ks], cfg,
+                 f"cfg5 full size, {'ALL ' if len(ks) == cfg.N else ''}{len(ks)} pairs")
     assert np.median(v[data["anomalous"]]) > np.median(v[~data["anomalous"]])
 
 
