@@ -3,7 +3,7 @@
 fullsize_refs.json).  Calls ONLY the float64 oracle (oracle/) and the seeded input generator (synth) -- never the
 CUDA path.  Hours of CPU time for cfg 4; resumable (every oracle evaluation is cached under --state-dir).
 
-    python tests/golden/make_fullsize_refs.py [--cfg 3 4 5] [--cfg5-all] [--threads T] [--state-dir DIR] [--only base|pert]
+    python tests/golden/make_fullsize_refs.py [--cfg 3 4 5] [--cfg5-all | --cfg5-pairs P] [--threads T] [--state-dir DIR] [--only base|pert]
 
 What is stored (BASELINE.json north_star: "summed Soft-DTW value+gradient and the barycenter matching the float64
 oracle ... on all five configs"; cfg 1-2 are computed live by the tests, cfg 3-5 come from here):
@@ -12,7 +12,7 @@ oracle ... on all five configs"; cfg 1-2 are computed live by the tests, cfg 3-5
                  iterations of Z <- Z - step G (eq. 7; Z kept in float64 between iterations, reading C14)
                  at the step frozen in synth.CONFIGS (reading C12), after the contractivity check below has passed.
   cfg 5          Soft-DTW values of all 1000 pairs (--cfg5-all), else of 64 seeded pairs, 16 of them anomalous
-                 (SURVEY.md 8(d)).
+                 (--cfg5-pairs P: a seeded superset of P pairs with every anomalous cycle).
 Contractivity check (reading C13): the same descent is run from Z0 (1 + 1e-6 xi), xi ~ N(0, 1) seeded.
 If the two final iterates differ by more than 1e-4 (relative L2), i.e. the map amplifies a perturbation more than
 100 x, parity of the iterated map would measure chaos, not correctness: the step is halved and the check repeated;
@@ -141,13 +141,19 @@ def make_descent_config(idx, args):
             "moved_rel": rel_l2(Z, Z0), "grad0_l2": float(np.linalg.norm(G0)), "grad0_max": float(np.abs(G0).max())}
 
 
-def cfg5_sample(data):
-    """64 seeded pair indices, 16 of them anomalous (ascending)."""
+def cfg5_sample(data, pairs=CFG5_PAIRS):
+    """64 seeded pair indices, 16 of them anomalous (ascending).  With pairs > 64 (--cfg5-pairs) a superset of those:
+    every remaining anomalous cycle, then seeded normal ones up to `pairs`."""
     rng = np.random.Generator(np.random.PCG64(13005))
     anom = np.flatnonzero(data["anomalous"])
     norm = np.flatnonzero(~data["anomalous"])
     ks = np.concatenate([rng.choice(anom, CFG5_ANOMALOUS, replace=False),
                          rng.choice(norm, CFG5_PAIRS - CFG5_ANOMALOUS, replace=False)])
+    if pairs > CFG5_PAIRS:
+        more_anom = np.setdiff1d(anom, ks)
+        more_norm = np.random.Generator(np.random.PCG64(13006)).choice(
+            np.setdiff1d(norm, ks), pairs - CFG5_PAIRS - len(more_anom), replace=False)
+        ks = np.concatenate([ks, more_anom, more_norm])
     return np.sort(ks)
 
 
@@ -157,7 +163,7 @@ def make_cfg5(args):
     output file is written only when every batch is there."""
     data = synth.make(5)
     cfg = data["cfg"]
-    ks = np.arange(cfg.N) if args.cfg5_all else cfg5_sample(data)
+    ks = np.arange(cfg.N) if args.cfg5_all else cfg5_sample(data, args.cfg5_pairs)
     off = data["offsets"]
     state = Path(args.state_dir)
     state.mkdir(parents=True, exist_ok=True)
@@ -193,6 +199,8 @@ def main():
     ap.add_argument("--only", choices=["base", "pert"], default=None,
                     help="compute only one of the two descents of a config into --state-dir (no output file is written)")
     ap.add_argument("--cfg5-all", action="store_true", help="cfg 5: all N values instead of the 64-pair sample")
+    ap.add_argument("--cfg5-pairs", type=int, default=CFG5_PAIRS,
+                    help="cfg 5: size of the seeded sample (a superset of the 64-pair one; every anomalous cycle from 98 up)")
     args = ap.parse_args()
     oracle.build()
     meta_path = HERE / "fullsize_refs.json"
