@@ -471,7 +471,8 @@ def test_cfg4_full_all_pairs_gradient_and_descent(B):
 def test_cfg5_full_size_against_the_stored_oracle_values(B):
     """cfg 5 (1000 cycles of 20-40k samples against m = 30000, forward only) in one call, against every oracle value
     tests/golden/fullsize_cfg5.npz holds: all 1000 when it was written by `make_fullsize_refs.py --cfg5-all` (SURVEY.md
-    8(d); Step 3 of the paper, consumes every one), else the 64 seeded pairs, 16 of them anomalous."""
+    8(d); Step 3 of the paper, consumes every one), else a seeded sample of at least 64 pairs, 16 of them anomalous (as committed: 256 pairs with
+    all 50 anomalous cycles, `--cfg5-pairs 256`)."""
     import torch
     data = synth.make(5)
     cfg = data["cfg"]
